@@ -1,0 +1,166 @@
+"""Seeded synthetic inputs for the five BASELINE.json configs.
+
+This module serves BOTH the CUDA path and the CPU oracle with the *same* arrays.  It holds
+none of the method's arithmetic (no equilibrium, no collision, no streaming): it only draws
+fields with numpy.random.Generator(PCG64(seed)) in fp64 and builds node masks.  It imports
+neither the oracle nor the CUDA binding.
+
+Every workload stands in for a workload of the paper (which uses no public dataset):
+  c1  Taylor-Green vortex, D2Q9            <- PAPER.md section 3.7, 256^2 there
+  c2  force-driven channel, D3Q19 LBGK     <- duct flow of section 4.2
+  c3  MRT with 5 % random solid obstacles  <- MRT bar of Fig. 7 with complex geometry
+  c4  duct with four side walls, fp64      <- duct flow, DP case
+  c5  Shan-Chen spinodal decomposition     <- 254x100x100 periodic binary box
+
+Arrays are C-order [z][y][x] (x fastest); u is [D][z][y][x].
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass, field
+
+import numpy as np
+
+D2Q9, D3Q19 = 0, 1
+BGK, MRT, SC2 = 0, 1, 2
+F32, F64 = 0, 1
+
+
+def mrt_rates_d3q19(tau: float) -> list:
+    """c3 rate vector, reading A7 (moment order of reading A5)."""
+    s = 1.0 / tau
+    return [0.0, 1.19, 1.4, 0.0, 1.2, 0.0, 1.2, 0.0, 1.2, s, 1.4, s, 1.4, s, s, s, 1.98, 1.98, 1.98]
+
+
+def mrt_rates_d2q9(tau: float) -> list:
+    s = 1.0 / tau
+    return [0.0, 1.63, 1.14, 0.0, 1.92, 0.0, 1.92, s, s]
+
+
+@dataclass
+class Workload:
+    name: str
+    lattice: int
+    model: int
+    precision: int
+    nx: int
+    ny: int
+    nz: int
+    tau: tuple
+    steps: int
+    force: tuple = (0.0, 0.0, 0.0)
+    rates: list | None = None
+    sc_G: float = 0.0
+    sc_psi: int = 0
+    seed: int | None = None
+    mask: np.ndarray | None = None                 # uint8 [nz][ny][nx], 0 FLUID 1 SOLID
+    rho: list = field(default_factory=list)        # per component, fp64 [nz][ny][nx]
+    u: list = field(default_factory=list)          # per component, fp64 [D][nz][ny][nx]
+
+    @property
+    def D(self):
+        return 2 if self.lattice == D2Q9 else 3
+
+    @property
+    def Q(self):
+        return 9 if self.lattice == D2Q9 else 19
+
+    @property
+    def sites(self):
+        return self.nx * self.ny * self.nz
+
+    @property
+    def ncomp(self):
+        return 2 if self.model == SC2 else 1
+
+    def params(self) -> dict:
+        return dict(lattice=self.lattice, model=self.model, nx=self.nx, ny=self.ny, nz=self.nz,
+                    tau=self.tau, rates=self.rates, force=self.force, sc_G=self.sc_G, sc_psi=self.sc_psi)
+
+
+def c1_taylor_green(n: int = 128, steps: int = 1000, u0: float = 0.01, tau: float = 0.8,
+                    precision: int = F32) -> Workload:
+    k = 2.0 * np.pi / n
+    y, x = np.meshgrid(np.arange(n, dtype=np.float64), np.arange(n, dtype=np.float64), indexing="ij")
+    ux = -u0 * np.cos(k * x) * np.sin(k * y)
+    uy = u0 * np.sin(k * x) * np.cos(k * y)
+    w = Workload("c1_taylor_green_d2q9_bgk", D2Q9, BGK, precision, n, n, 1, (tau, tau), steps)
+    w.mask = np.zeros((1, n, n), np.uint8)
+    w.rho = [np.ones((1, n, n))]
+    w.u = [np.stack([ux, uy])[:, None, :, :].copy()]
+    return w
+
+
+def c2_channel(nx: int = 256, ny: int = 256, nz: int = 256, steps: int = 2000, tau: float = 0.6,
+               g: float = 1e-6, seed: int = 20131102, precision: int = F32) -> Workload:
+    rng = np.random.Generator(np.random.PCG64(seed))
+    w = Workload("c2_channel_d3q19_bgk", D3Q19, BGK, precision, nx, ny, nz, (tau, tau), steps,
+                 force=(g, 0.0, 0.0), seed=seed)
+    mask = np.zeros((nz, ny, nx), np.uint8)
+    mask[:, 0, :] = 1
+    mask[:, ny - 1, :] = 1
+    u = rng.uniform(-1e-3, 1e-3, (3, nz, ny, nx))
+    u[:, mask == 1] = 0.0
+    w.mask, w.rho, w.u = mask, [np.ones((nz, ny, nx))], [u]
+    return w
+
+
+def c3_mrt_obstacles(nx: int = 384, ny: int = 384, nz: int = 384, steps: int = 500, tau: float = 0.55,
+                     solid_fraction: float = 0.05, seed: int = 20131103, precision: int = F32) -> Workload:
+    rng = np.random.Generator(np.random.PCG64(seed))
+    w = Workload("c3_obstacles_d3q19_mrt", D3Q19, MRT, precision, nx, ny, nz, (tau, tau), steps,
+                 rates=mrt_rates_d3q19(tau), seed=seed)
+    mask = (rng.random((nz, ny, nx)) < solid_fraction).astype(np.uint8)
+    u = np.zeros((3, nz, ny, nx))
+    u[0] = 0.05
+    u[:, mask == 1] = 0.0
+    w.mask, w.rho, w.u = mask, [np.ones((nz, ny, nx))], [u]
+    return w
+
+
+def c4_duct(nx: int = 512, ny: int = 256, nz: int = 256, steps: int = 500, tau: float = 0.52,
+            g: float = 1e-7, precision: int = F64) -> Workload:
+    w = Workload("c4_duct_d3q19_bgk", D3Q19, BGK, precision, nx, ny, nz, (tau, tau), steps,
+                 force=(g, 0.0, 0.0))
+    mask = np.zeros((nz, ny, nx), np.uint8)
+    mask[:, 0, :] = 1
+    mask[:, ny - 1, :] = 1
+    mask[0, :, :] = 1
+    mask[nz - 1, :, :] = 1
+    w.mask, w.rho, w.u = mask, [np.ones((nz, ny, nx))], [np.zeros((3, nz, ny, nx))]
+    return w
+
+
+def c5_shan_chen(nx: int = 256, ny: int = 256, nz: int = 256, steps: int = 1000, G: float = 0.9,
+                 seed: int = 20131105, precision: int = F32) -> Workload:
+    rng = np.random.Generator(np.random.PCG64(seed))
+    w = Workload("c5_spinodal_d3q19_sc2", D3Q19, SC2, precision, nx, ny, nz, (1.0, 1.0), steps,
+                 sc_G=G, sc_psi=0, seed=seed)
+    n = rng.uniform(-0.01, 0.01, (nz, ny, nx))
+    w.mask = np.zeros((nz, ny, nx), np.uint8)
+    w.rho = [1.0 + n, 1.0 - n]
+    w.u = [np.zeros((3, nz, ny, nx)), np.zeros((3, nz, ny, nx))]
+    return w
+
+
+def random_state(lattice: int, nx: int, ny: int, nz: int, seed: int, solid_fraction: float = 0.0,
+                 du: float = 0.02, drho: float = 0.02, ncomp: int = 1):
+    """Generic seeded (mask, rho[], u[]) for parity tests at arbitrary (ragged) sizes."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    D = 2 if lattice == D2Q9 else 3
+    mask = (rng.random((nz, ny, nx)) < solid_fraction).astype(np.uint8)
+    rho, u = [], []
+    for _ in range(ncomp):
+        rho.append(1.0 + rng.uniform(-drho, drho, (nz, ny, nx)))
+        uu = rng.uniform(-du, du, (D, nz, ny, nx))
+        uu[:, mask == 1] = 0.0
+        u.append(uu)
+    return mask, rho, u
+
+
+CONFIGS = {
+    "c1": c1_taylor_green,
+    "c2": c2_channel,
+    "c3": c3_mrt_obstacles,
+    "c4": c4_duct,
+    "c5": c5_shan_chen,
+}

@@ -1,0 +1,510 @@
+"""Pins for the CPU oracle (oracle/lbm_oracle.c): everything here checks the oracle against
+something OTHER than itself -- values printed in the paper (tests/golden/), closed forms,
+conservation laws, special cases that reduce to a simpler model, brute force on tiny lattices.
+P:<n> = line n of the paper text; A<n> = reading n in DESIGN.md.
+
+No GPU needed; the whole file runs in well under a minute.
+"""
+import itertools
+import os
+from fractions import Fraction
+
+import numpy as np
+import pytest
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _uniform(o, rho0, u0):
+    nz, ny, nx = o.shape
+    rho = np.full(o.shape, rho0)
+    u = np.zeros((o.D,) + o.shape)
+    for a in range(o.D):
+        u[a] = u0[a]
+    return rho, u
+
+
+# ---------------------------------------------------------------- lattice tables, Table 1
+def _golden_weights():
+    out = {}
+    for line in open(os.path.join(GOLD, "table1_weights.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        name, *ws = line.split()
+        out[name] = [float(Fraction(w)) for w in ws]
+    return out
+
+
+@pytest.mark.parametrize("name,lat,Q,D", [("D2Q9", 0, 9, 2), ("D3Q19", 1, 19, 3)])
+def test_weights_match_table1_and_are_isotropic(orc, name, lat, Q, D):
+    e, w, opp = orc.lattice_tables(lat)
+    assert e.shape == (Q, 3)
+    gold = _golden_weights()[name]
+    n2 = (e ** 2).sum(1)
+    for i in range(Q):
+        assert w[i] == gold[n2[i]]                       # Table 1
+    assert len({tuple(v) for v in e}) == Q               # all velocities distinct
+    assert sorted(np.bincount(n2).tolist()) == sorted({9: [1, 4, 4], 19: [1, 6, 12]}[Q])
+    assert abs(w.sum() - 1.0) < 1e-15
+    assert np.allclose((w[:, None] * e).sum(0), 0.0, atol=1e-17)
+    # second- and fourth-order isotropy with c_s^2 = 1/3
+    d = np.eye(3)[:D, :D]
+    ed = e[:, :D].astype(float)
+    m2 = np.einsum("i,ia,ib->ab", w, ed, ed)
+    assert np.allclose(m2, d / 3.0, atol=1e-16)
+    m4 = np.einsum("i,ia,ib,ic,id->abcd", w, ed, ed, ed, ed)
+    iso = (np.einsum("ab,cd->abcd", d, d) + np.einsum("ac,bd->abcd", d, d) + np.einsum("ad,bc->abcd", d, d)) / 9.0
+    assert np.allclose(m4, iso, atol=1e-16)
+    # opposite table: e[opp[i]] = -e[i], involution
+    assert np.array_equal(e[opp], -e)
+    assert np.array_equal(opp[opp], np.arange(Q))
+    if D == 2:
+        assert np.all(e[:, 2] == 0)
+
+
+def test_velocity_order_is_reading_A2(orc):
+    e9, _, opp9 = orc.lattice_tables(0)
+    assert [tuple(v[:2]) for v in e9] == [(0, 0), (1, 0), (0, 1), (-1, 0), (0, -1), (1, 1), (-1, 1), (-1, -1), (1, -1)]
+    assert opp9.tolist() == [0, 3, 4, 1, 2, 7, 8, 5, 6]
+    e19, _, opp19 = orc.lattice_tables(1)
+    assert [tuple(v) for v in e19[:7]] == [(0, 0, 0), (1, 0, 0), (-1, 0, 0), (0, 1, 0), (0, -1, 0), (0, 0, 1), (0, 0, -1)]
+    assert opp19.tolist() == [0, 2, 1, 4, 3, 6, 5, 10, 9, 8, 7, 14, 13, 12, 11, 18, 17, 16, 15]
+
+
+# ---------------------------------------------------------------- equilibrium moments, eq. (1), (3)
+@pytest.mark.parametrize("lat", [0, 1])
+def test_equilibrium_moments_closed_form(orc, lat):
+    e, w, _ = orc.lattice_tables(lat)
+    D = 2 if lat == 0 else 3
+    rng = np.random.default_rng(7)
+    for _ in range(20):
+        rho = rng.uniform(0.5, 2.0)
+        v = np.zeros(3)
+        v[:D] = rng.uniform(-0.1, 0.1, D)
+        fe = orc.feq(lat, rho, v)
+        assert abs(fe.sum() - rho) < 4e-16 * rho * 4                         # P:274, eq. (1)
+        assert np.allclose((fe[:, None] * e).sum(0), rho * v, atol=1e-16)    # eq. (1)
+        P = np.einsum("i,ia,ib->ab", fe, e.astype(float), e.astype(float))
+        want = rho * (np.eye(3) / 3.0 + np.outer(v, v))
+        assert np.allclose(P[:D, :D], want[:D, :D], atol=1e-16)
+    # rest state is w_i * rho
+    assert np.allclose(orc.feq(lat, 1.0, np.zeros(3)), w, atol=0)
+
+
+# ---------------------------------------------------------------- fixed point and conservation
+@pytest.mark.parametrize("lat,model", [(0, 0), (1, 0), (1, 1), (0, 1)])
+def test_uniform_equilibrium_is_a_fixed_point(orc, lat, model):
+    from paper_1311_2404_b200 import workloads as W
+    shp = (5, 6, 1) if lat == 0 else (4, 5, 3)
+    rates = (W.mrt_rates_d2q9 if lat == 0 else W.mrt_rates_d3q19)(0.7) if model == 1 else None
+    o = orc.Oracle(lat, model, *shp, tau=0.7, rates=rates)
+    rho, u = _uniform(o, 1.3, (0.03, -0.02, 0.01))
+    o.init_equilibrium(rho, u)
+    f0 = o.get_distributions()
+    o.step(25)
+    assert np.max(np.abs(o.get_distributions() - f0)) < 5e-15      # 25 steps of round-off
+
+
+@pytest.mark.parametrize("model", [0, 1])
+def test_mass_conserved_with_solids_and_force(orc, model):
+    from paper_1311_2404_b200 import workloads as W
+    nx, ny, nz = 9, 7, 6
+    mask, rho, u = W.random_state(1, nx, ny, nz, seed=11, solid_fraction=0.15)
+    o = orc.Oracle(1, model, nx, ny, nz, tau=0.62, rates=W.mrt_rates_d3q19(0.62) if model else None,
+                   force=(2e-5, -1e-5, 3e-5))
+    o.set_geometry(mask)
+    o.init_equilibrium(rho[0], u[0])
+    m0 = o.macro()[0].sum()
+    o.step(200)
+    r, v = o.macro()
+    assert abs(r.sum() - m0) < 1e-12 * m0
+    assert np.all(r[mask == 1] == 0) and np.all(v[:, mask == 1] == 0)     # SOLID read-out convention
+
+
+@pytest.mark.parametrize("lat,model", [(0, 0), (1, 0), (1, 1)])
+def test_uniform_force_closed_form(orc, lat, model):
+    """Uniform state on a torus: v(n) = u0 + (n + 1/2) g exactly, rho unchanged (eq. 16; A13/A15)."""
+    from paper_1311_2404_b200 import workloads as W
+    shp = (4, 5, 1) if lat == 0 else (4, 5, 6)
+    g = (1e-5, -2e-5, 0.0 if lat == 0 else 3e-5)
+    u0 = (0.01, 0.02, 0.0 if lat == 0 else -0.015)
+    o = orc.Oracle(lat, model, *shp, tau=0.8, force=g, rates=W.mrt_rates_d3q19(0.8) if model else None)
+    o.init_equilibrium(*_uniform(o, 1.1, u0))
+    for n in (0, 1, 37):
+        if n:
+            o.step(n - (0 if n == 1 else 1))
+        r, v = o.macro()
+        assert np.max(np.abs(r - 1.1)) < 1e-14
+        for a in range(o.D):
+            assert np.max(np.abs(v[a] - (u0[a] + (n + 0.5) * g[a]))) < 1e-15
+
+
+def test_duct_early_time_equals_wall_free_run(orc):
+    """c4 shape: information travels <= 1 node/step, so nodes farther than t from every wall are
+    bit-identical to the wall-free uniform-force solution at step t."""
+    from paper_1311_2404_b200 import workloads as W
+    w = W.c4_duct(nx=6, ny=14, nz=12, steps=4, g=1e-7)
+    a = orc.Oracle(1, 0, 6, 14, 12, tau=0.52, force=w.force)
+    b = orc.Oracle(1, 0, 6, 14, 12, tau=0.52, force=w.force)
+    a.set_geometry(w.mask)
+    for o in (a, b):
+        o.init_equilibrium(w.rho[0], w.u[0])
+    t = 4
+    a.step(t)
+    b.step(t)
+    fa, fb = a.get_distributions(), b.get_distributions()
+    core = (slice(None), slice(1 + t, 12 - 1 - t), slice(1 + t, 14 - 1 - t), slice(None))
+    assert np.array_equal(fa[core], fb[core])
+    assert not np.array_equal(fa[:, 1, 1, :], fb[:, 1, 1, :])
+    vb = b.macro()[1]
+    assert np.max(np.abs(vb[0] - (t + 0.5) * 1e-7)) < 1e-15          # absolute round-off of sum f_i e_i
+
+
+# ---------------------------------------------------------------- Poiseuille (eq. 16-17)
+def _poiseuille(orc, lat, H, tau, g, steps):
+    ny = H + 2
+    shp = (3, ny, 1) if lat == 0 else (3, ny, 3)
+    o = orc.Oracle(lat, 0, *shp, tau=tau, force=(g, 0, 0))
+    mask = np.zeros(o.shape, np.uint8)
+    mask[:, 0, :] = 1
+    mask[:, ny - 1, :] = 1
+    o.set_geometry(mask)
+    o.init_equilibrium(*_uniform(o, 1.0, (0, 0, 0)))
+    o.step(steps)
+    r, v = o.macro()
+    return v[0][0, 1:ny - 1, 1], ny
+
+
+@pytest.mark.parametrize("lat", [0, 1])
+def test_poiseuille_parabola_plus_constant_slip(orc, lat):
+    """Steady force-driven channel between half-way bounce-back walls: the profile is the parabola
+    with walls half a link beyond the last fluid node plus a constant g(48 nu^2 - 1)/(8 nu)
+    (bounce-back literature), nu = (tau - 1/2)/3."""
+    g = 1e-6
+    for tau in (0.6, 0.8):
+        nu = (tau - 0.5) / 3.0
+        ux, ny = _poiseuille(orc, lat, 16, tau, g, 40000)
+        y = np.arange(1, ny - 1, dtype=float)
+        parab = g / (2 * nu) * (y - 0.5) * (ny - 1.5 - y)
+        slip = ux - parab
+        assert np.ptp(slip) < 1e-10 * ux.max()                      # constant across the channel (4e4 steps of round-off)
+        assert abs(slip.mean() - g * (48 * nu * nu - 1) / (8 * nu)) < 1e-9 * ux.max()
+
+
+def test_poiseuille_second_order_and_magic_tau(orc):
+    g, tau = 1e-6, 0.6
+    nu = (tau - 0.5) / 3.0
+    errs = []
+    for H, steps in ((16, 40000), (32, 160000)):
+        ux, ny = _poiseuille(orc, 0, H, tau, g, steps)
+        y = np.arange(1, ny - 1, dtype=float)
+        parab = g / (2 * nu) * (y - 0.5) * (ny - 1.5 - y)
+        errs.append(np.max(np.abs(ux - parab)) / parab.max())
+    assert 3.5 < errs[0] / errs[1] < 4.5                             # second order in 1/H
+    assert abs(errs[0] - 3.7e-3) < 1e-4
+    tau = 0.5 + np.sqrt(3.0) / 4.0                                    # (tau - 1/2)^2 = 3/16: exact walls
+    nu = (tau - 0.5) / 3.0
+    ux, ny = _poiseuille(orc, 0, 16, tau, g, 20000)
+    y = np.arange(1, ny - 1, dtype=float)
+    parab = g / (2 * nu) * (y - 0.5) * (ny - 1.5 - y)
+    assert np.max(np.abs(ux - parab)) < 1e-10 * parab.max()
+
+
+# ---------------------------------------------------------------- Taylor-Green (eq. 19; A10)
+def test_taylor_green_decay_rate(orc):
+    from paper_1311_2404_b200 import workloads as W
+    w = W.c1_taylor_green()
+    o = orc.Oracle(0, 0, w.nx, w.ny, 1, tau=0.8)
+    o.init_equilibrium(w.rho[0], w.u[0])
+    nu, k = (0.8 - 0.5) / 3.0, 2 * np.pi / 128
+
+    def energy():
+        r, v = o.macro()
+        return 0.5 * (v ** 2).sum()
+
+    e0 = energy()
+    o.step(1000)
+    e1 = energy()
+    want = np.exp(-2 * nu * k * k * 1000)            # velocity amplitude: exp(-nu |k|^2 t), |k|^2 = 2 k^2
+    assert abs(np.sqrt(e1 / e0) / want - 1.0) < 1e-3
+    r, v = o.macro()
+    # the velocity field keeps the analytic shape of eq. (19)
+    shape = w.u[0][:, 0] * np.sqrt(e1 / e0)
+    assert np.max(np.abs(v[:, 0] - shape)) < 2e-3 * 0.01
+    assert abs(r.sum() - 128 * 128) < 1e-12 * 128 * 128
+
+
+# ---------------------------------------------------------------- MRT (eq. 4; A5, A6)
+def test_mrt_matrix_rows_orthogonal_integer_with_golden_norms(orc):
+    M, Minv = orc.mrt_matrix(1)
+    lines = [l.split() for l in open(os.path.join(GOLD, "mrt_d3q19_rows.txt")) if l.strip() and not l.startswith("#")]
+    norms = np.array([float(x) for x in lines[0]])
+    G = M @ M.T
+    assert np.allclose(G, np.diag(norms), atol=1e-12)
+    assert np.array_equal(M, np.round(M)) and M.min() == -30 and M.max() == 12
+    assert np.count_nonzero(M) == 213
+    e, _, _ = orc.lattice_tables(1)
+    n2 = (e ** 2).sum(1)
+    for row, name in ((1, "e"), (2, "epsilon")):
+        vals = [float(x) for x in next(l for l in lines if l[0] == name)[1:]]
+        for link in range(3):
+            assert np.all(M[row, n2 == link] == vals[link])
+    assert np.allclose(Minv, M.T / norms[None, :], atol=1e-15)
+    assert np.allclose(Minv @ M, np.eye(19), atol=1e-14)
+    M9, Minv9 = orc.mrt_matrix(0)
+    assert np.allclose(M9 @ M9.T, np.diag([9, 36, 36, 6, 12, 6, 12, 4, 4]), atol=1e-12)
+    assert np.allclose(Minv9 @ M9, np.eye(9), atol=1e-14)
+    # conserved rows are the moments of eq. (1)
+    assert np.array_equal(M[0], np.ones(19)) and np.array_equal(M[[3, 5, 7]], e.T.astype(float))
+
+
+def test_mrt_equilibrium_moments_match_published_closed_forms(orc):
+    """m^eq = M f^eq (A6) against the closed forms published with the basis (d'Humieres et al. 2002
+    with w_eps = 3, w_epsj = -11/2, w_xx = -1/2 and rho_0 -> rho; Lallemand & Luo 2000 for D2Q9).
+    A wrong sign or coefficient in any row of M fails here."""
+    rng = np.random.default_rng(3)
+    M, _ = orc.mrt_matrix(1)
+    M9, _ = orc.mrt_matrix(0)
+    for _ in range(10):
+        rho = rng.uniform(0.7, 1.5)
+        v = rng.uniform(-0.1, 0.1, 3)
+        jx, jy, jz = rho * v
+        jj = (jx * jx + jy * jy + jz * jz) / rho
+        want = [rho, -11 * rho + 19 * jj, 3 * rho - 5.5 * jj,
+                jx, -2 / 3 * jx, jy, -2 / 3 * jy, jz, -2 / 3 * jz,
+                (2 * jx * jx - jy * jy - jz * jz) / rho, -0.5 * (2 * jx * jx - jy * jy - jz * jz) / rho,
+                (jy * jy - jz * jz) / rho, -0.5 * (jy * jy - jz * jz) / rho,
+                jx * jy / rho, jy * jz / rho, jx * jz / rho, 0, 0, 0]
+        assert np.allclose(M @ orc.feq(1, rho, v), want, atol=3e-15)
+        v2 = np.array([v[0], v[1], 0.0])
+        jx, jy = rho * v2[:2]
+        jj = (jx * jx + jy * jy) / rho
+        want9 = [rho, -2 * rho + 3 * jj, rho - 3 * jj, jx, -jx, jy, -jy, (jx * jx - jy * jy) / rho, jx * jy / rho]
+        assert np.allclose(M9 @ orc.feq(0, rho, v2), want9, atol=3e-15)
+
+
+@pytest.mark.parametrize("lat", [0, 1])
+def test_mrt_with_equal_rates_is_lbgk(orc, lat):
+    """S = omega I  =>  eq. (4) is the LBGK operator, with solids and a body force."""
+    from paper_1311_2404_b200 import workloads as W
+    shp = (9, 8, 1) if lat == 0 else (7, 6, 5)
+    tau = 0.7
+    mask, rho, u = W.random_state(lat, *shp, seed=5, solid_fraction=0.1)
+    Q = 9 if lat == 0 else 19
+    a = orc.Oracle(lat, 0, *shp, tau=tau, force=(1e-5, 2e-5, 0))
+    b = orc.Oracle(lat, 1, *shp, tau=tau, rates=[1 / tau] * Q, force=(1e-5, 2e-5, 0))
+    for o in (a, b):
+        o.set_geometry(mask)
+        o.init_equilibrium(rho[0], u[0])
+        o.step(100)
+    assert np.max(np.abs(a.get_distributions() - b.get_distributions())) < 5e-15
+
+
+def test_mrt_conserved_rates_are_irrelevant(orc):
+    from paper_1311_2404_b200 import workloads as W
+    mask, rho, u = W.random_state(1, 6, 5, 4, seed=9, solid_fraction=0.1)
+    r1 = W.mrt_rates_d3q19(0.6)
+    r2 = list(r1)
+    for k in (0, 3, 5, 7):
+        r2[k] = 1.7
+    outs = []
+    for r in (r1, r2):
+        o = orc.Oracle(1, 1, 6, 5, 4, tau=0.6, rates=r)
+        o.set_geometry(mask)
+        o.init_equilibrium(rho[0], u[0])
+        o.step(50)
+        outs.append(o.get_distributions())
+    assert np.max(np.abs(outs[0] - outs[1])) < 5e-15
+
+
+@pytest.mark.parametrize("case", ["ux(y)", "uy(z)", "uz(x)", "diag_xy", "diag_yz"])
+def test_mrt_shear_wave_viscosity(orc, case):
+    """The decay of a shear wave fixes which rows carry the shear rate 1/tau (rows 9, 11, 13, 14, 15
+    of A5) and nu = (tau - 1/2)/3; the other rates (1.19, 1.4, 1.2, 1.98) must not enter."""
+    from paper_1311_2404_b200 import workloads as W
+    n, tau, u0, T = 48, 0.8, 1e-3, 400
+    nu = (tau - 0.5) / 3.0
+    k = 2 * np.pi / n
+    ax = np.arange(n, dtype=float)
+    if case == "ux(y)":
+        shp = (2, n, 2); u = np.zeros((3, 2, n, 2)); u[0] = u0 * np.sin(k * ax)[None, :, None]; k2 = k * k
+    elif case == "uy(z)":
+        shp = (2, 2, n); u = np.zeros((3, n, 2, 2)); u[1] = u0 * np.sin(k * ax)[:, None, None]; k2 = k * k
+    elif case == "uz(x)":
+        shp = (n, 2, 2); u = np.zeros((3, 2, 2, n)); u[2] = u0 * np.sin(k * ax)[None, None, :]; k2 = k * k
+    elif case == "diag_xy":
+        shp = (n, n, 2); u = np.zeros((3, 2, n, n))
+        ph = np.sin(k * (ax[None, :] - ax[:, None]))                 # [y][x] -> sin(k (x - y))
+        u[0] = u0 * ph[None]; u[1] = u0 * ph[None]; k2 = 2 * k * k
+    else:
+        shp = (2, n, n); u = np.zeros((3, n, n, 2))
+        ph = np.sin(k * (ax[None, :] - ax[:, None]))                 # [z][y] -> sin(k (y - z))
+        u[1] = u0 * ph[:, :, None]; u[2] = u0 * ph[:, :, None]; k2 = 2 * k * k
+    o = orc.Oracle(1, 1, *shp, tau=tau, rates=W.mrt_rates_d3q19(tau))
+    o.init_equilibrium(np.ones(o.shape), u)
+    o.step(T)
+    _, v = o.macro()
+    ratio = np.sqrt((v ** 2).sum() / (u ** 2).sum())
+    nu_eff = -np.log(ratio) / (k2 * T)
+    assert abs(nu_eff / nu - 1.0) < 0.01
+
+
+# ---------------------------------------------------------------- streaming map / bounce-back (A8)
+@pytest.mark.parametrize("lat,shp", [(0, (5, 4, 1)), (0, (1, 3, 1)), (1, (4, 3, 5)), (1, (2, 1, 3)), (1, (8, 8, 8))])
+def test_stream_map_brute_force_push_formulation(orc, lat, shp):
+    """The oracle builds the map by PULL; rebuild it here by PUSH with explicit nested loops:
+    the post-collision value in slot (i, x) moves to (i, x + e_i), or, if that node is SOLID,
+    comes back to (ibar, x).  Both must agree, and on FLUID slots it is a permutation."""
+    nx, ny, nz = shp
+    e, _, opp = orc.lattice_tables(lat)
+    Q = len(e)
+    rng = np.random.default_rng(nx * 100 + ny * 10 + nz)
+    for frac in (0.0, 0.3):
+        mask = (rng.random((nz, ny, nx)) < frac).astype(np.uint8)
+        o = orc.Oracle(lat, 0, nx, ny, nz, tau=1.0)
+        o.set_geometry(mask)
+        got = o.stream_map()
+        N = nx * ny * nz
+        want = np.full((Q, N), -1, np.int64)
+        for z, y, x in itertools.product(range(nz), range(ny), range(nx)):
+            if mask[z, y, x]:
+                continue
+            n = (z * ny + y) * nx + x
+            for i in range(Q):
+                xx, yy, zz = (x + e[i][0]) % nx, (y + e[i][1]) % ny, (z + e[i][2]) % nz
+                if mask[zz, yy, xx]:
+                    want[opp[i], n] = i * N + n
+                else:
+                    want[i, (zz * ny + yy) * nx + xx] = i * N + n
+        assert np.array_equal(got, want)
+        fl = np.repeat((mask.ravel() == 0)[None, :], Q, 0)
+        assert np.all(got[~fl] == -1)
+        src = got[fl]
+        assert len(np.unique(src)) == src.size                       # injective
+        assert np.array_equal(np.sort(src), np.flatnonzero(fl.ravel()))  # onto the FLUID slots
+
+
+@pytest.mark.parametrize("lat,shp", [(0, (7, 6, 1)), (1, (5, 6, 4))])
+def test_step_against_numpy_roll_reference(orc, lat, shp):
+    """Independent tiny re-implementation in whole-array numpy (push by np.roll + bounce-back fix-up)."""
+    from paper_1311_2404_b200 import workloads as W
+    nx, ny, nz = shp
+    e, w, opp = orc.lattice_tables(lat)
+    Q, D = len(e), (2 if lat == 0 else 3)
+    mask, rho, u = W.random_state(lat, nx, ny, nz, seed=21, solid_fraction=0.2)
+    tau, g = 0.9, np.array([1e-4, -2e-4, 3e-4 if D == 3 else 0.0])
+    o = orc.Oracle(lat, 0, nx, ny, nz, tau=tau, force=g)
+    o.set_geometry(mask)
+    o.init_equilibrium(rho[0], u[0])
+    f = o.get_distributions().copy()
+    fluid = mask == 0
+    for _ in range(12):
+        r = f.sum(0)
+        j = np.einsum("qzyx,qa->azyx", f, e.astype(float))
+        v = j / r + 0.5 * g[:, None, None, None]
+        ev = np.einsum("qa,azyx->qzyx", e.astype(float), v)
+        vv = (v ** 2).sum(0)
+        fe = r * w[:, None, None, None] * (1 + 3 * ev + 4.5 * ev ** 2 - 1.5 * vv)
+        eg = e.astype(float) @ g
+        vg = np.einsum("a,azyx->zyx", g, v)
+        src = w[:, None, None, None] * r * (3 * (eg[:, None, None, None] - vg) + 9 * ev * eg[:, None, None, None])
+        fs = f + (fe - f) / tau + (1 - 0.5 / tau) * src
+        new = f.copy()
+        for i in range(Q):
+            moved = np.roll(fs[i], shift=(e[i][2], e[i][1], e[i][0]), axis=(0, 1, 2))
+            from_solid = np.roll(mask, shift=(e[i][2], e[i][1], e[i][0]), axis=(0, 1, 2)) == 1
+            new[i] = np.where(fluid, np.where(from_solid, fs[opp[i]], moved), f[i])
+        f = new
+    o.step(12)
+    got = o.get_distributions()
+    assert np.max(np.abs(got - f)[:, fluid]) < 1e-14
+    assert np.array_equal(got[:, ~fluid], f[:, ~fluid])              # SOLID nodes keep initial values
+
+
+# ---------------------------------------------------------------- Shan-Chen (eq. 10; A11, A13)
+def _sc(orc, shp, G=0.9, tau=(1.0, 1.0), psi=0, force=(0, 0, 0)):
+    return orc.Oracle(1, 2, *shp, tau=tau, sc_G=G, sc_psi=psi, force=force)
+
+
+def test_shan_chen_force_on_linear_gradient(orc):
+    """psi = rho, rho_A = a, rho_B = 1 + b x  =>  F_A = -G a b (sum_i w_i e_ix e_ix) = -G a b / 3 along x;
+    F_B = 0 away from the periodic seam.  Fixes the sign (A11), the weights and the neighbour direction."""
+    shp = (12, 4, 3)
+    o = _sc(orc, shp, G=0.9)
+    a, b = 0.8, 0.01
+    x = np.arange(12, dtype=float)[None, None, :] + np.zeros((3, 4, 12))
+    z3 = np.zeros((3,) + x.shape)
+    o.init_equilibrium(np.full(x.shape, a), z3, comp=0)
+    o.init_equilibrium(1 + b * x, z3, comp=1)
+    FA, FB = o.sc_force(0), o.sc_force(1)
+    inner = (slice(None), slice(None), slice(1, 11))
+    assert np.allclose(FA[0][inner], -0.9 * a * b / 3.0, atol=1e-16)
+    assert np.allclose(FA[1:], 0, atol=1e-17) and np.allclose(FB[:, :, :, 1:11], 0, atol=1e-17)
+    # psi = 1 - exp(-rho): first-order expansion in b
+    o2 = _sc(orc, shp, G=0.9, psi=1)
+    o2.init_equilibrium(np.full(x.shape, a), z3, comp=0)
+    o2.init_equilibrium(1 + 1e-5 * x, z3, comp=1)
+    FA2 = o2.sc_force(0)
+    want = -0.9 * (1 - np.exp(-a)) * np.exp(-(1 + 1e-5 * x)) * 1e-5 / 3.0
+    assert np.allclose(FA2[0][inner], want[inner], rtol=1e-8, atol=0)
+
+
+def test_shan_chen_conserves_component_mass_and_total_momentum(orc):
+    from paper_1311_2404_b200 import workloads as W
+    w = W.c5_shan_chen(nx=10, ny=9, nz=8, steps=200)
+    o = _sc(orc, (10, 9, 8), G=0.9, tau=(1.0, 0.8))
+    for s in range(2):
+        o.init_equilibrium(w.rho[s], w.u[s], comp=s)
+    m0 = [o.macro(s)[0].sum() for s in range(2)]
+    o.step(200)
+    mom = np.zeros(3)
+    for s in range(2):
+        r, v = o.macro(s)
+        assert abs(r.sum() - m0[s]) < 1e-12 * m0[s]
+        mom += (r * v).sum(axis=(1, 2, 3))
+    assert np.max(np.abs(mom)) < 1e-12
+
+
+def test_shan_chen_G0_equal_tau_sums_to_single_component_lbgk(orc):
+    """G = 0, tau_A = tau_B: f^eq is linear in rho at fixed velocity and u' is the barycentric
+    velocity, so f_A + f_B follows the single-component LBGK iteration exactly."""
+    from paper_1311_2404_b200 import workloads as W
+    shp = (6, 5, 4)
+    _, rho, u = W.random_state(1, *shp, seed=4, ncomp=2)
+    o = _sc(orc, shp, G=0.0, tau=(0.9, 0.9))
+    for s in range(2):
+        o.init_equilibrium(rho[s], u[s], comp=s)
+    ref = orc.Oracle(1, 0, *shp, tau=0.9)
+    ref.set_distributions(o.get_distributions(0) + o.get_distributions(1))
+    o.step(40)
+    ref.step(40)
+    assert np.max(np.abs(o.get_distributions(0) + o.get_distributions(1) - ref.get_distributions())) < 1e-14
+
+
+def test_shan_chen_vanishing_second_component_is_lbgk(orc):
+    from paper_1311_2404_b200 import workloads as W
+    shp = (6, 5, 4)
+    _, rho, u = W.random_state(1, *shp, seed=8)
+    o = _sc(orc, shp, G=0.9, tau=(0.75, 1.0))
+    o.init_equilibrium(rho[0], u[0], comp=0)
+    o.init_equilibrium(np.full(rho[0].shape, 1e-30), np.zeros_like(u[0]), comp=1)
+    ref = orc.Oracle(1, 0, *shp, tau=0.75)
+    ref.init_equilibrium(rho[0], u[0])
+    o.step(30)
+    ref.step(30)
+    assert np.max(np.abs(o.get_distributions(0) - ref.get_distributions())) < 1e-15
+
+
+def test_shan_chen_repulsive_sign_demixes(orc):
+    """Reading A11 (PARITY UNPINNED by the paper: no printed value): with F = -G psi psi' e and
+    G = 0.9 > 0 a noisy 50/50 mixture demixes (section 5.4 uses G = 0.9 for immiscible fluids)."""
+    from paper_1311_2404_b200 import workloads as W
+    w = W.c5_shan_chen(nx=16, ny=16, nz=16)
+    o = _sc(orc, (16, 16, 16), G=0.9)
+    for s in range(2):
+        o.init_equilibrium(w.rho[s], w.u[s], comp=s)
+    d0 = np.std(o.macro(0)[0] - o.macro(1)[0])
+    o.step(300)
+    d1 = np.std(o.macro(0)[0] - o.macro(1)[0])
+    assert d1 > 5 * d0
+    assert np.isfinite(o.get_distributions(0)).all()
