@@ -1,0 +1,126 @@
+/*
+ * lbm.h -- C ABI of the B200-native fused lattice Boltzmann stream-and-collide library
+ *          (liblbm_b200.so, sm_100a).  Method: arXiv 1311.2404 (Sailfish); P:<n> cites line n
+ *          of PAPER.md, A<n> cites a reading listed in DESIGN.md.
+ *
+ * Conventions (all calls)
+ *   - Return value: 0 = LBM_OK, < 0 = error code below.  Nothing throws, nothing aborts.
+ *     lbm_last_error(ctx) gives a human-readable string for the last failure on that context
+ *     (ctx == NULL: the last failure of lbm_workspace_bytes / lbm_create on this thread).
+ *   - Every pointer named d_* is a DEVICE pointer, every pointer named h_* is a HOST pointer.
+ *     The caller owns all memory, including the workspace: the library never allocates device
+ *     memory (PyTorch allocates it; "PyTorch ... only for device memory and streams").
+ *   - Arrays are C-order [z][y][x], x fastest.  `real` is float (LBM_F32) or double
+ *     (LBM_F64).  Scalar fields: real[nz][ny][nx].  Velocity: real[D][nz][ny][nx] (component
+ *     planes, D = 2 for D2Q9, 3 for D3Q19).  Distributions: real[Q][nz][ny][nx] in the velocity
+ *     order of reading A2 (lbm_lattice_info returns it).
+ *   - The lattice is a torus: every axis is periodic.  Walls exist only through the
+ *     node-type mask (0 = FLUID, 1 = SOLID); SOLID nodes are dry and reflect by half-way
+ *     bounce-back (reading A8).
+ *   - All work is enqueued on the CUDA stream given to lbm_create; calls are asynchronous with
+ *     respect to the host unless stated otherwise.  A context is not thread-safe.
+ *   - `comp` is 0 except for LBM_SC2 (0 = component A, 1 = component B).
+ */
+#ifndef LBM_B200_H
+#define LBM_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { LBM_OK = 0, LBM_EINVAL = -1, LBM_EUNSUPPORTED = -2, LBM_ENOMEM = -3, LBM_ECUDA = -4, LBM_ESTATE = -5 };
+enum { LBM_D2Q9 = 0, LBM_D3Q19 = 1 };            /* lattice, Table 1              */
+enum { LBM_BGK = 0, LBM_MRT = 1, LBM_SC2 = 2 };  /* model: SC2 = two LBGK components coupled
+                                                    by the Shan-Chen force       */
+enum { LBM_F32 = 0, LBM_F64 = 1 };               /* precision of storage and arithmetic      */
+enum { LBM_PSI_RHO = 0, LBM_PSI_1MEXP = 1 };     /* psi(rho) = rho | 1 - exp(-rho)   */
+enum { LBM_STORE_AB = 0, LBM_STORE_AA = 1 };     /* two copies | in-place AA */
+
+#define LBM_QMAX 19
+
+typedef struct lbm_ctx lbm_ctx;
+
+typedef struct {
+    uint32_t struct_size;     /* = sizeof(lbm_params); lets the ABI grow                           */
+    int32_t lattice;          /* LBM_D2Q9 | LBM_D3Q19                                              */
+    int32_t model;            /* LBM_BGK | LBM_MRT | LBM_SC2                                       */
+    int32_t precision;        /* LBM_F32 | LBM_F64                                                 */
+    int32_t nx, ny, nz;       /* lattice extents, each >= 1 (nz == 1 for D2Q9), nx*ny*nz < 2^31    */
+    double tau[2];            /* BGK/MRT: tau[0] > 0.5.  SC2: tau[0] = tau_A, tau[1] = tau_B       */
+    double rates[LBM_QMAX];   /* MRT: Q relaxation rates in the moment order of reading A5;
+                                 each in [0, 2]; ignored by the other models (eq. 4)        */
+    double force[3];          /* body acceleration g; force density F = rho g (eq. 16, reading A4) */
+    double sc_G;              /* Shan-Chen coupling G of eq. (10), sign per reading A11    */
+    int32_t sc_psi;           /* LBM_PSI_*                                                         */
+    int32_t store;            /* LBM_STORE_AB (default 0) | LBM_STORE_AA                           */
+} lbm_params;
+
+/* Static description of a lattice (Table 1; ordering = reading A2).
+ * e: int32[Q][3], w: double[Q], opp: int32[Q] (index of -e_i); any may be NULL.
+ * Writes Q and D.  Host pointers.  LBM_EINVAL on an unknown lattice. */
+int lbm_lattice_info(int32_t lattice, int32_t *Q, int32_t *D, int32_t *h_e, double *h_w, int32_t *h_opp);
+
+/* Bytes of device workspace a context with these parameters needs (distribution store,
+ * node-type/link encoding, Shan-Chen fields, staging for the host-buffer calls). */
+int lbm_workspace_bytes(const lbm_params *p, size_t *bytes);
+
+/* Create a context on the current CUDA device.  d_workspace: >= lbm_workspace_bytes, 256-byte
+ * aligned, owned by the caller and kept alive until lbm_destroy.  cuda_stream: a cudaStream_t
+ * (NULL = legacy default stream).  The geometry starts all-FLUID.
+ * Errors: LBM_EINVAL (bad enum/size/tau/rate, workspace too small or misaligned),
+ * LBM_EUNSUPPORTED (combination not built, e.g. MRT on SC2), LBM_ECUDA. */
+int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, void *cuda_stream, lbm_ctx **out);
+int lbm_destroy(lbm_ctx *ctx);
+
+/* Node types (reduced to FLUID/SOLID, reading A8).  d_mask: uint8[nz][ny][nx], 0 = FLUID,
+ * non-zero = SOLID.  Builds the internal link encoding (which of the Q pull sources are
+ * reflected).  Must be called before lbm_init_equilibrium / lbm_set_distributions if the
+ * geometry is not all-FLUID; calling it afterwards returns LBM_ESTATE. */
+int lbm_set_geometry(lbm_ctx *ctx, const uint8_t *d_mask);
+int lbm_get_geometry(lbm_ctx *ctx, uint8_t *d_mask);          /* writes 0/1 per node */
+
+/* f_i(x, 0) = f_i^eq(rho0(x), u0(x)), eq. (3), velocity used as given (A15).
+ * d_rho: real[N], d_u: real[D][N].  SOLID nodes are ignored. */
+int lbm_init_equilibrium(lbm_ctx *ctx, int comp, const void *d_rho, const void *d_u);
+
+/* Advance n >= 0 time steps; each step is one fused pull-stream + moments + equilibrium +
+ * collision (+ Guo source) + store pass over the lattice (Alg. 1; eqs. 1-4, 16-17);
+ * LBM_SC2 runs the macro-field pass and then the coupled collide pass (eq. 10).
+ * LBM_ESTATE if a component has not been initialised. */
+int lbm_step(lbm_ctx *ctx, int n);
+
+/* rho = sum_i f_i, velocity v of eq. (16) (includes g/2) from the current state.
+ * SC2: rho_s and the bare component velocity j_s / rho_s.  SOLID nodes: rho = 0, u = 0.
+ * d_rho: real[N] or NULL, d_u: real[D][N] or NULL. */
+int lbm_macro(lbm_ctx *ctx, int comp, void *d_rho, void *d_u);
+
+/* Test / checkpoint hooks.  Canonical state = pre-collision, post-streaming f_i(x, t) (what
+ * Alg. 1 line 4 loads; reading A9), real[Q][N].  get writes 0 on SOLID nodes; set ignores them. */
+int lbm_get_distributions(lbm_ctx *ctx, int comp, void *d_f);
+int lbm_set_distributions(lbm_ctx *ctx, int comp, const void *d_f);
+
+/* Streaming index map (reading A8): d_map int64[Q][N]; map[i][x] = i' * N + x' = the slot of the
+ * canonical post-collision array whose value becomes f_i(x, t+1): (i, x - e_i) if that node is
+ * FLUID, else (ibar, x); -1 where x is SOLID.  Computed by the same device routine the step
+ * kernels use for their gather. */
+int lbm_get_stream_map(lbm_ctx *ctx, int64_t *d_map);
+
+/* Whole path with HOST buffers (what bench.py's e2e leg times): H2D of mask, rho0, u0 per
+ * component -> set_geometry -> init_equilibrium -> step(n) -> macro(comp 0) -> D2H, then
+ * synchronises the stream.  h_mask may be NULL (all FLUID).  h_rho0 / h_u0: arrays of `ncomp`
+ * host pointers.  h_rho_out / h_u_out (component 0) may be NULL.  Resets the context state. */
+int lbm_run_host(lbm_ctx *ctx, const uint8_t *h_mask, const void *const *h_rho0, const void *const *h_u0,
+                 int n, void *h_rho_out, void *h_u_out);
+
+/* Time step counter since the last init/set, and number of kernels launched by this context. */
+int lbm_get_counters(const lbm_ctx *ctx, int64_t *steps, int64_t *launches);
+
+const char *lbm_last_error(const lbm_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LBM_B200_H */
