@@ -1,0 +1,227 @@
+// lbm_node.cuh -- register-resident per-node arithmetic of the fused update: moments (eq. 1,
+// P:85), Guo velocity shift (eq. 16), equilibrium (eq. 3), LBGK relaxation
+// (Alg. 1 l.13), MRT relaxation (eq. 4) and Guo source (eq. 17).
+//
+// Everything works on the DEVIATION h_i = f_i - w_i from the rest equilibrium at rho = 1 (the
+// round-off-minimising storage the paper recommends; reading A12).  The
+// collision is affine in f, so it carries over unchanged: sum_i h_i = rho - 1, sum_i h_i e_i = j,
+// h_i^eq = w_i (drho + rho (3 e.v + 4.5 (e.v)^2 - 1.5 v.v)).
+#pragma once
+#include "lbm_lattice.cuh"
+
+namespace lbm {
+
+// Parameters of one component's collision, passed to kernels by value (constant bank).
+template <typename T> struct Relax {
+    T inv_tau;        // 1 / tau
+    T src_scale;      // 1 - 1/(2 tau), prefactor of eq. (17)
+    T g[3];           // body acceleration
+    T cr[19];         // MRT: rate_k / |M_k|^2                 (relaxation, eq. 4)
+    T cs[19];         // MRT: (1 - rate_k / 2) / |M_k|^2       (source, reading A16)
+};
+
+template <class L, typename T> LBM_HD void moments(const T (&h)[L::Q], T &drho, T (&j)[3]) {
+    T s = h[0], jx = T(0), jy = T(0), jz = T(0);
+#pragma unroll
+    for (int i = 1; i < L::Q; i++) {
+        s += h[i];
+        if (L::ex(i) == 1) jx += h[i]; else if (L::ex(i) == -1) jx -= h[i];
+        if (L::ey(i) == 1) jy += h[i]; else if (L::ey(i) == -1) jy -= h[i];
+        if (L::ez(i) == 1) jz += h[i]; else if (L::ez(i) == -1) jz -= h[i];
+    }
+    drho = s; j[0] = jx; j[1] = jy; j[2] = jz;
+}
+
+template <class L, typename T> LBM_HD T e_dot(int i, const T (&a)[3]) {
+    T s = T(0);
+    if (L::ex(i) == 1) s += a[0]; else if (L::ex(i) == -1) s -= a[0];
+    if (L::ey(i) == 1) s += a[1]; else if (L::ey(i) == -1) s -= a[1];
+    if (L::ez(i) == 1) s += a[2]; else if (L::ez(i) == -1) s -= a[2];
+    return s;
+}
+
+// h_i^eq for all i, eq. (3) minus w_i.
+template <class L, typename T>
+LBM_HD void equilibrium_dev(T rho, T drho, const T (&v)[3], T (&heq)[L::Q]) {
+    const T vv15 = T(1.5) * (v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
+#pragma unroll
+    for (int i = 0; i < L::Q; i++) {
+        const T ev = e_dot<L, T>(i, v);
+        heq[i] = L::template w<T>(i) * (drho + rho * (T(3) * ev + T(4.5) * ev * ev - vv15));
+    }
+}
+
+// Bracket of eq. (17): w_i [3 (e_i - v) + 9 (e_i.v) e_i] . F
+template <class L, typename T>
+LBM_HD void guo_bracket(const T (&v)[3], const T (&F)[3], T (&src)[L::Q]) {
+    const T vF = v[0] * F[0] + v[1] * F[1] + v[2] * F[2];
+#pragma unroll
+    for (int i = 0; i < L::Q; i++) {
+        const T ev = e_dot<L, T>(i, v), eF = e_dot<L, T>(i, F);
+        src[i] = L::template w<T>(i) * (T(3) * (eF - vF) + T(9) * ev * eF);
+    }
+}
+
+// ---- MRT moment transforms (eq. 4; basis = reading A5) -------------------------------
+// m = M d and o = M^T r.  Rows of M are mutually orthogonal polynomials of e_i with small
+// integer entries; both transforms are hand-factored through the velocity-class sub-sums so the
+// pair costs ~170 flop instead of the ~1400 of two dense 19x19 products (keeps MRT HBM-bound).
+template <class L, typename T> struct Mrt;
+
+template <typename T> struct Mrt<D3Q19, T> {
+    static constexpr double norm(int k) {
+        constexpr double n[19] = {19, 2394, 252, 10, 40, 10, 40, 10, 40, 36, 72, 12, 24, 4, 4, 4, 8, 8, 8};
+        return n[k];
+    }
+    LBM_HD static void forward(const T (&d)[19], T (&m)[19]) {
+        const T Sx = d[1] + d[2], Dx = d[1] - d[2];
+        const T Sy = d[3] + d[4], Dy = d[3] - d[4];
+        const T Sz = d[5] + d[6], Dz = d[5] - d[6];
+        // xy diagonals 7 (+,+) 8 (-,+) 9 (+,-) 10 (-,-)
+        const T a1 = d[7] + d[10], a2 = d[8] + d[9], a3 = d[7] - d[10], a4 = d[9] - d[8];
+        const T Sxy = a1 + a2, Pxy = a1 - a2, Xxy = a3 + a4, Yxy = a3 - a4;
+        // xz diagonals 11 (+,+) 12 (-,+) 13 (+,-) 14 (-,-)
+        const T b1 = d[11] + d[14], b2 = d[12] + d[13], b3 = d[11] - d[14], b4 = d[13] - d[12];
+        const T Sxz = b1 + b2, Pxz = b1 - b2, Xxz = b3 + b4, Zxz = b3 - b4;
+        // yz diagonals 15 (+,+) 16 (-,+) 17 (+,-) 18 (-,-)
+        const T c1 = d[15] + d[18], c2 = d[16] + d[17], c3 = d[15] - d[18], c4 = d[17] - d[16];
+        const T Syz = c1 + c2, Pyz = c1 - c2, Yyz = c3 + c4, Zyz = c3 - c4;
+        const T A = Sx + Sy + Sz, B = Sxy + Sxz + Syz;
+        const T Xd = Xxy + Xxz, Yd = Yxy + Yyz, Zd = Zxz + Zyz;
+        const T axx = T(2) * Sx - Sy - Sz, dxx = Sxy + Sxz - T(2) * Syz;
+        const T aww = Sy - Sz, dww = Sxy - Sxz;
+        m[0] = d[0] + A + B;
+        m[1] = T(-30) * d[0] - T(11) * A + T(8) * B;
+        m[2] = T(12) * d[0] - T(4) * A + B;
+        m[3] = Dx + Xd;  m[4] = Xd - T(4) * Dx;
+        m[5] = Dy + Yd;  m[6] = Yd - T(4) * Dy;
+        m[7] = Dz + Zd;  m[8] = Zd - T(4) * Dz;
+        m[9] = axx + dxx;   m[10] = dxx - T(2) * axx;
+        m[11] = aww + dww;  m[12] = dww - T(2) * aww;
+        m[13] = Pxy; m[14] = Pyz; m[15] = Pxz;
+        m[16] = Xxy - Xxz; m[17] = Yyz - Yxy; m[18] = Zxz - Zyz;
+    }
+    // o_i = sum_k M[k][i] r_k
+    LBM_HD static void backward(const T (&r)[19], T (&o)[19]) {
+        const T ca = r[0] - T(11) * r[1] - T(4) * r[2];   // axis class
+        const T cd = r[0] + T(8) * r[1] + r[2];           // diagonal class
+        o[0] = r[0] - T(30) * r[1] + T(12) * r[2];
+        const T ax = ca + T(2) * (r[9] - T(2) * r[10]), lx = r[3] - T(4) * r[4];
+        const T t1 = T(2) * r[10] - r[9], t2 = r[11] - T(2) * r[12];
+        const T ay = ca + t1 + t2, ly = r[5] - T(4) * r[6];
+        const T az = ca + t1 - t2, lz = r[7] - T(4) * r[8];
+        o[1] = ax + lx; o[2] = ax - lx;
+        o[3] = ay + ly; o[4] = ay - ly;
+        o[5] = az + lz; o[6] = az - lz;
+        const T qx = r[3] + r[4], qy = r[5] + r[6], qz = r[7] + r[8];
+        const T s9 = r[9] + r[10], s11 = r[11] + r[12];
+        {   // xy: cd + sx(qx + r16) + sy(qy - r17) + s9 + s11 + sx sy r13
+            const T base = cd + s9 + s11, X = qx + r[16], Y = qy - r[17];
+            const T p = base + r[13], q = base - r[13];
+            o[7] = p + X + Y; o[10] = p - X - Y; o[8] = q - X + Y; o[9] = q + X - Y;
+        }
+        {   // xz: cd + sx(qx - r16) + sz(qz + r18) + s9 - s11 + sx sz r15
+            const T base = cd + s9 - s11, X = qx - r[16], Z = qz + r[18];
+            const T p = base + r[15], q = base - r[15];
+            o[11] = p + X + Z; o[14] = p - X - Z; o[12] = q - X + Z; o[13] = q + X - Z;
+        }
+        {   // yz: cd + sy(qy + r17) + sz(qz - r18) - 2 s9 + sy sz r14
+            const T base = cd - T(2) * s9, Y = qy + r[17], Z = qz - r[18];
+            const T p = base + r[14], q = base - r[14];
+            o[15] = p + Y + Z; o[18] = p - Y - Z; o[16] = q - Y + Z; o[17] = q + Y - Z;
+        }
+    }
+};
+
+// D2Q9 (reading A5): rows 1; -4+3n^2; 4-21n^2/2+9n^4/2; ex; (-5+3n^2)ex; ey; (-5+3n^2)ey;
+// ex^2-ey^2; ex ey.  9x9 is small enough to unroll as constants.
+template <typename T> struct Mrt<D2Q9, T> {
+    static constexpr double norm(int k) {
+        constexpr double n[9] = {9, 36, 36, 6, 12, 6, 12, 4, 4};
+        return n[k];
+    }
+    LBM_HD static constexpr int M(int k, int i) {
+        const int x = D2Q9::ex(i), y = D2Q9::ey(i), n2 = x * x + y * y;
+        return k == 0 ? 1
+             : k == 1 ? -4 + 3 * n2
+             : k == 2 ? (8 - 21 * n2 + 9 * n2 * n2) / 2
+             : k == 3 ? x
+             : k == 4 ? (-5 + 3 * n2) * x
+             : k == 5 ? y
+             : k == 6 ? (-5 + 3 * n2) * y
+             : k == 7 ? x * x - y * y
+             : x * y;
+    }
+    LBM_HD static void forward(const T (&d)[9], T (&m)[9]) {
+#pragma unroll
+        for (int k = 0; k < 9; k++) {
+            T s = T(0);
+#pragma unroll
+            for (int i = 0; i < 9; i++) if (M(k, i) != 0) s += T(M(k, i)) * d[i];
+            m[k] = s;
+        }
+    }
+    LBM_HD static void backward(const T (&r)[9], T (&o)[9]) {
+#pragma unroll
+        for (int i = 0; i < 9; i++) {
+            T s = T(0);
+#pragma unroll
+            for (int k = 0; k < 9; k++) if (M(k, i) != 0) s += T(M(k, i)) * r[k];
+            o[i] = s;
+        }
+    }
+};
+
+// ---- collision: h (pre-collision deviations) -> h* (post-collision), in place ---------------
+// rho, drho = rho - 1, v = velocity entering f^eq and eq. (17) (reading A3), F = force density.
+template <class L, typename T, bool MRT, bool FORCE>
+LBM_HD void collide(T (&h)[L::Q], T rho, T drho, const T (&v)[3], const T (&F)[3], const Relax<T> &rp) {
+    constexpr int Q = L::Q;
+    T heq[Q];
+    equilibrium_dev<L, T>(rho, drho, v, heq);
+    if constexpr (!MRT) {
+        if constexpr (FORCE) {
+            T src[Q];
+            guo_bracket<L, T>(v, F, src);
+#pragma unroll
+            for (int i = 0; i < Q; i++) h[i] = h[i] + (heq[i] - h[i]) * rp.inv_tau + rp.src_scale * src[i];
+        } else {
+#pragma unroll
+            for (int i = 0; i < Q; i++) h[i] = h[i] + (heq[i] - h[i]) * rp.inv_tau;
+        }
+    } else {
+        T d[Q], m[Q];
+#pragma unroll
+        for (int i = 0; i < Q; i++) d[i] = heq[i] - h[i];
+        Mrt<L, T>::forward(d, m);
+#pragma unroll
+        for (int k = 0; k < Q; k++) m[k] *= rp.cr[k];
+        if constexpr (FORCE) {
+            T src[Q], ms[Q];
+            guo_bracket<L, T>(v, F, src);
+            Mrt<L, T>::forward(src, ms);
+#pragma unroll
+            for (int k = 0; k < Q; k++) m[k] += rp.cs[k] * ms[k];
+        }
+        Mrt<L, T>::backward(m, d);
+#pragma unroll
+        for (int i = 0; i < Q; i++) h[i] += d[i];
+    }
+}
+
+// Single-component node update: moments, F = rho g, v = j/rho + g/2 (eq. 16), collide.
+template <class L, typename T, bool MRT, bool FORCE>
+LBM_HD void update_node(T (&h)[L::Q], const Relax<T> &rp) {
+    T drho, j[3];
+    moments<L, T>(h, drho, j);
+    const T rho = T(1) + drho, inv_rho = T(1) / rho;
+    T v[3], F[3];
+#pragma unroll
+    for (int a = 0; a < 3; a++) {
+        F[a] = FORCE ? rho * rp.g[a] : T(0);
+        v[a] = FORCE ? (j[a] + T(0.5) * F[a]) * inv_rho : j[a] * inv_rho;
+    }
+    collide<L, T, MRT, FORCE>(h, rho, drho, v, F, rp);
+}
+
+}  // namespace lbm
