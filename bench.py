@@ -1,0 +1,261 @@
+#!/usr/bin/env python
+"""bench.py -- MLUPS of the fused LBM stream-and-collide step on B200 (BASELINE.json metric).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config c2] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path (rows a1-a8 of DESIGN.md; a9-a11 for c5) over the
+whole lattice of the config, i.e. one LBM time step.  Default workload: configs[1] = c2, D3Q19
+LBGK fp32 256^3 channel with Guo force -- the configuration the metric is quoted on.  Inputs are
+seeded synthetic fields (paper_1311_2404_b200/workloads.py) standing in for the paper's duct flow.
+
+The path does not shard (north_star: one GPU, no halo exchange): with --gpus N > 1 every rank runs
+an independent replica ("replicas only") and `value` is the sum over ranks.
+
+One JSON line on stdout (rank 0).  --impl reference times the CPU oracle instead.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+from paper_1311_2404_b200 import workloads as W  # noqa: E402
+
+METRIC = "MLUPS on 1 B200 and achieved HBM GB/s as % of peak (D3Q19 LBGK fp32)"
+UNIT = "MLUPS"
+# ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum per step_kernel launch at c2
+# (profiles/): filled in from the committed capture; None until one exists for the config.
+NCU_TRAFFIC_BYTES = {}
+
+
+def algorithmic_bytes_per_site(w) -> float:
+    """SURVEY 8(d) / DESIGN.md: 2*Q*sizeof(real) + 1 mask byte; Shan-Chen two-pass floor 472 (fp32)."""
+    s = 4 if w.precision == W.F32 else 8
+    if w.model == W.SC2:
+        return 2 * w.Q * s + 2 * s + (2 * 2 * w.Q * s + 2 * s)  # pass 1 + pass 2
+    return 2 * w.Q * s + 1
+
+
+def measured_peak():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def sample_workload(cfg: str):
+    """Bounded sample of the config for the CPU oracle: same recipe, same nx*ny cross-section,
+    a thin z-slab (the torus closes it), so one oracle step costs ~0.25 s per 2M sites."""
+    full = W.CONFIGS[cfg]()
+    if full.lattice == W.D2Q9:
+        return full, "the full %dx%d lattice" % (full.nx, full.ny)
+    nz = max(4, (1 << 21) // (full.nx * full.ny))
+    w = W.CONFIGS[cfg](full.nx, full.ny, nz)
+    return w, "%dx%dx%d z-slab of the %dx%dx%d workload, same seeded recipe" % (w.nx, w.ny, w.nz, full.nx, full.ny, full.nz)
+
+
+def time_oracle(cfg: str, steps: int, warmup: int):
+    from oracle import oracle
+    w, what = sample_workload(cfg)
+    ref = oracle.Oracle(**w.params())
+    ref.set_geometry(w.mask)
+    for s in range(w.ncomp):
+        ref.init_equilibrium(w.rho[s], w.u[s], comp=s)
+    ref.step(warmup)
+    t0 = time.perf_counter()
+    ref.step(steps)
+    dt = time.perf_counter() - t0
+    return dict(value=w.sites * steps / dt / 1e6, unit=UNIT, cores=oracle.num_threads(), kind="oracle",
+                sample="%s, %d steps (%.1f s)" % (what, steps, dt)), dt, w
+
+
+def config_dict(w, cfg, extra=None):
+    d = {"workload": "%s: %s %s %s %dx%dx%d" % (cfg, "D2Q9" if w.lattice == W.D2Q9 else "D3Q19",
+                                                 ["LBGK", "MRT", "Shan-Chen 2xLBGK"][w.model],
+                                                 "fp32" if w.precision == W.F32 else "fp64", w.nx, w.ny, w.nz),
+         "tau": list(w.tau)[: w.ncomp], "force": list(w.force), "seed": w.seed,
+         "solid_fraction": float(w.mask.mean()), "store": "AB, SoA real[Q][N]",
+         "parallelism": "replicas only (path does not shard)"}
+    d.update(extra or {})
+    return d
+
+
+def run_reference(args):
+    """CPU oracle arm: rank 0 only; each step is one oracle step over the bounded sample."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    steps = min(args.steps, 60)
+    cb, dt, w = time_oracle(args.config, steps, min(args.warmup, 3))
+    line = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus,
+            "steps": steps, "warmup": min(args.warmup, 3), "ms_per_step": dt / steps * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": config_dict(w, args.config, {"sample": cb["sample"]}),
+            "cpu_baseline": cb, "gpu_launches": 0,
+            "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
+                                       "--format=csv,noheader,nounits", "-lms", "50"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.p.terminate()
+        self.p.wait()
+        self.f.seek(0)
+        rows = [r.split(",") for r in self.f.read().strip().splitlines() if r.count(",") >= 6]
+        self.f.close()
+        os.unlink(self.f.name)
+        if not rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        sm = sorted(float(r[0]) for r in rows)
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for k, n in enumerate(names) if any(r[3 + k].strip() == "Active" for r in rows)]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(rows[0][1]), "samples": len(rows),
+                "power_w_max": max(float(r[2]) for r in rows), "reasons": reasons}
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_1311_2404_b200 import binding
+
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    binding.load()  # no fallback: raises if the CUDA library is missing
+
+    K, Wm = args.steps, max(args.warmup, 3)
+    w = W.CONFIGS[args.config]()
+    sim = binding.from_workload(w, device=dev)
+    sim.set_geometry(w.mask)
+    for s in range(w.ncomp):
+        sim.init_equilibrium(w.rho[s], w.u[s], comp=s)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    # ---- device-resident: K steps between CUDA events on the context's stream -------------------
+    sim.step(Wm)
+    l0 = sim.counters()[1]
+    barrier()
+    clocks = ClockSampler(local)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    reps = []
+    for _ in range(args.repeats):
+        barrier()
+        e0.record(sim.stream)
+        sim.step(K)
+        e1.record(sim.stream)
+        barrier()
+        reps.append(e0.elapsed_time(e1))
+    clk = clocks.stop()
+    launches = (sim.counters()[1] - l0) // args.repeats
+    ms = float(np.median(reps))
+    t = torch.tensor([ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms = float(t.item())
+    rho, _ = sim.macro()
+    assert bool(torch.isfinite(rho).all()), "state went non-finite during the timed steps"
+
+    # ---- end to end through lbm_run_host: pinned host inputs -> H2D -> init -> K steps -> D2H ------
+    tdt = torch.float32 if w.precision == W.F32 else torch.float64
+    h_mask = torch.from_numpy(w.mask).pin_memory()
+    h_rho = [torch.from_numpy(r).to(tdt).pin_memory() for r in w.rho]
+    h_u = [torch.from_numpy(u).to(tdt).pin_memory() for u in w.u]
+    o_rho = torch.empty(sim.shape, dtype=tdt).pin_memory()
+    o_u = torch.empty((sim.D,) + sim.shape, dtype=tdt).pin_memory()
+    sim.run_host(h_mask, h_rho, h_u, Wm, o_rho, o_u)
+    barrier()
+    t0 = time.perf_counter()
+    sim.run_host(h_mask, h_rho, h_u, K, o_rho, o_u)  # synchronises the stream before returning
+    e2e_s = time.perf_counter() - t0
+    barrier()
+    t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e_s = float(t.item())
+    h2d = h_mask.numel() + sum(x.numel() * x.element_size() for x in h_rho + h_u)
+    d2h = o_rho.numel() * o_rho.element_size() + o_u.numel() * o_u.element_size()
+    assert bool(torch.isfinite(o_rho).all())
+
+    if rank == 0:
+        peak, which = measured_peak()
+        bps = algorithmic_bytes_per_site(w)
+        achieved = bps * w.sites * K / (ms * 1e-3) / 1e9  # per-launch bytes / per-launch time
+        kernel = "sc_fields_kernel + sc_step_kernel" if w.model == W.SC2 else "step_kernel"
+        cb = None
+        if world == 1 and not args.no_cpu_baseline:
+            cb, _, _ = time_oracle(args.config, args.cpu_steps, 1)
+        line = {"metric": METRIC, "value": w.sites * K * world / (ms * 1e-3) / 1e6, "unit": UNIT,
+                "n_gpus": world, "steps": K, "warmup": Wm, "ms_per_step": ms / K, "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "f32" if w.precision == W.F32 else "f64",
+                "data": "synthetic",
+                "config": config_dict(w, args.config, {
+                    "l2": "working set %.2f GB per step >> 126 MB L2 (no flush needed)" % (bps * w.sites / 1e9),
+                    "timing": "median of %d repeats of K steps, CUDA events on the ctx stream" % args.repeats,
+                    "repeats_ms": reps}),
+                "clocks": clk,
+                "e2e": {"value": w.sites * K * world / e2e_s / 1e6, "unit": UNIT,
+                        "h2d_bytes_per_step": h2d / K, "d2h_bytes_per_step": d2h / K,
+                        "note": "one lbm_run_host call = H2D(mask, rho0, u0) + init + K steps + macro + D2H(rho, u); bytes amortised over K"},
+                "gpu_launches": int(launches),
+                "roofline": {"bound": "hbm", "kernel": kernel, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                             "frac": achieved / peak, "peak_source": which,
+                             "bytes_per_site": bps, "sites_per_launch": w.sites,
+                             "traffic": NCU_TRAFFIC_BYTES.get(args.config)},
+                "cpu_baseline": cb}
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="c2", choices=sorted(W.CONFIGS))
+    ap.add_argument("--repeats", type=int, default=1)
+    ap.add_argument("--cpu-steps", type=int, default=40, help="oracle steps on the bounded sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

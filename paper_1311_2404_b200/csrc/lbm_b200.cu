@@ -1,0 +1,429 @@
+// lbm_b200.cu -- the C ABI of include/lbm.h: argument checking, workspace carving, kernel
+// dispatch over <lattice, real, model, force>.  All arithmetic of the method lives in the
+// kernels (lbm_kernels.cuh / lbm_node.cuh); nothing here touches oracle/.
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+#include "../../include/lbm.h"
+#include "lbm_kernels.cuh"
+
+using namespace lbm;
+
+namespace {
+
+thread_local char g_err[256] = "";
+
+constexpr size_t ALIGN = 256;
+inline size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
+
+struct Layout {
+    size_t store[2][2], type, link, psi[2], stage_mask, stage_rho, stage_u, total;
+};
+
+struct Vtbl;
+
+}  // namespace
+
+struct lbm_ctx {
+    lbm_params p;
+    int Q, D, ncomp;
+    size_t rs;  // sizeof(real)
+    Geom g;
+    cudaStream_t stream;
+    char *ws;
+    Layout lay;
+    int cur;  // which of the two buffers holds the current state (AB)
+    bool inited[2];
+    bool geometry_frozen;
+    int64_t steps, launches;
+    int block_x;
+    const Vtbl *vt;
+    char err[256];
+};
+
+namespace {
+
+struct Vtbl {
+    int (*set_geometry)(lbm_ctx *, const uint8_t *);
+    int (*init_equilibrium)(lbm_ctx *, int, const void *, const void *);
+    int (*step)(lbm_ctx *, int);
+    int (*macro)(lbm_ctx *, int, void *, void *);
+    int (*get_distributions)(lbm_ctx *, int, void *);
+    int (*set_distributions)(lbm_ctx *, int, const void *);
+    int (*get_stream_map)(lbm_ctx *, int64_t *);
+};
+
+int fail(lbm_ctx *c, int code, const char *fmt, const char *detail = "") {
+    char *dst = c ? c->err : g_err;
+    snprintf(dst, 256, fmt, detail);
+    return code;
+}
+
+int check_launch(lbm_ctx *c, const char *what) {
+    c->launches++;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) {
+        snprintf(c->err, sizeof c->err, "%s: %s", what, cudaGetErrorString(e));
+        return LBM_ECUDA;
+    }
+    return LBM_OK;
+}
+
+int validate(const lbm_params *p, int *Q, int *D) {
+    if (!p) return fail(nullptr, LBM_EINVAL, "params is NULL");
+    if (p->struct_size != sizeof(lbm_params)) return fail(nullptr, LBM_EINVAL, "struct_size != sizeof(lbm_params)");
+    if (p->lattice != LBM_D2Q9 && p->lattice != LBM_D3Q19) return fail(nullptr, LBM_EINVAL, "unknown lattice");
+    if (p->model < LBM_BGK || p->model > LBM_SC2) return fail(nullptr, LBM_EINVAL, "unknown model");
+    if (p->precision != LBM_F32 && p->precision != LBM_F64) return fail(nullptr, LBM_EINVAL, "unknown precision");
+    if (p->store != LBM_STORE_AB && p->store != LBM_STORE_AA) return fail(nullptr, LBM_EINVAL, "unknown store");
+    if (p->nx < 1 || p->ny < 1 || p->nz < 1) return fail(nullptr, LBM_EINVAL, "extents must be >= 1");
+    if (p->lattice == LBM_D2Q9 && p->nz != 1) return fail(nullptr, LBM_EINVAL, "D2Q9 needs nz == 1");
+    if ((double)p->nx * p->ny * p->nz >= 2147483648.0) return fail(nullptr, LBM_EINVAL, "nx*ny*nz must be < 2^31");
+    const int nt = p->model == LBM_SC2 ? 2 : 1;
+    for (int s = 0; s < nt; s++)
+        if (!(p->tau[s] > 0.5)) return fail(nullptr, LBM_EINVAL, "tau must be > 0.5");
+    *Q = p->lattice == LBM_D2Q9 ? 9 : 19;
+    *D = p->lattice == LBM_D2Q9 ? 2 : 3;
+    if (p->model == LBM_MRT)
+        for (int k = 0; k < *Q; k++)
+            if (!(p->rates[k] >= 0.0 && p->rates[k] <= 2.0)) return fail(nullptr, LBM_EINVAL, "MRT rates must be in [0, 2]");
+    for (int a = 0; a < 3; a++)
+        if (!(p->force[a] == p->force[a])) return fail(nullptr, LBM_EINVAL, "force is NaN");
+    if (p->model == LBM_SC2 && p->sc_psi != LBM_PSI_RHO && p->sc_psi != LBM_PSI_1MEXP)
+        return fail(nullptr, LBM_EINVAL, "unknown sc_psi");
+    if (p->lattice == LBM_D2Q9 && p->force[2] != 0.0) return fail(nullptr, LBM_EINVAL, "D2Q9 force has no z component");
+    if (p->store == LBM_STORE_AA) return fail(nullptr, LBM_EUNSUPPORTED, "AA store not built (AB only)");
+    if (p->ny > 65535 || p->nz > 65535) return fail(nullptr, LBM_EUNSUPPORTED, "ny and nz must be <= 65535");
+    return LBM_OK;
+}
+
+void make_layout(const lbm_params *p, int Q, int D, Layout *L) {
+    const size_t N = (size_t)p->nx * p->ny * p->nz, rs = p->precision == LBM_F32 ? 4 : 8;
+    const int nc = p->model == LBM_SC2 ? 2 : 1;
+    size_t off = 0;
+    memset(L, 0, sizeof *L);
+    for (int s = 0; s < nc; s++)
+        for (int b = 0; b < 2; b++) { L->store[s][b] = off; off += align_up(Q * N * rs); }
+    L->type = off; off += align_up(N);
+    L->link = off; off += align_up(4 * N);
+    if (nc == 2)
+        for (int s = 0; s < 2; s++) { L->psi[s] = off; off += align_up(N * rs); }
+    L->stage_mask = off; off += align_up(N);
+    L->stage_rho = off; off += align_up(N * rs);
+    L->stage_u = off; off += align_up(D * N * rs);
+    L->total = off;
+}
+
+template <typename T> T *at(lbm_ctx *c, size_t off) { return reinterpret_cast<T *>(c->ws + off); }
+
+dim3 grid_of(const lbm_ctx *c) { return dim3((c->g.nx + c->block_x - 1) / c->block_x, c->g.ny, c->g.nz); }
+
+template <typename T> Relax<T> make_relax(const lbm_ctx *c, int comp) {
+    Relax<T> r;
+    const double tau = c->p.tau[comp];
+    r.inv_tau = T(1.0 / tau);
+    r.src_scale = T(1.0 - 0.5 / tau);
+    for (int a = 0; a < 3; a++) r.g[a] = T(c->p.force[a]);
+    for (int k = 0; k < 19; k++) r.cr[k] = r.cs[k] = T(0);
+    return r;
+}
+
+// ---- per <lattice, real> implementation -------------------------------------------------------
+template <class L, typename T> struct Impl {
+    static const T *src(lbm_ctx *c, int s) { return at<T>(c, c->lay.store[s][c->cur]); }
+    static T *dst(lbm_ctx *c, int s) { return at<T>(c, c->lay.store[s][c->cur ^ 1]); }
+    static uint8_t *type(lbm_ctx *c) { return at<uint8_t>(c, c->lay.type); }
+    static uint32_t *link(lbm_ctx *c) { return at<uint32_t>(c, c->lay.link); }
+
+    static int set_geometry(lbm_ctx *c, const uint8_t *d_mask) {
+        build_links_kernel<L><<<grid_of(c), c->block_x, 0, c->stream>>>(c->g, d_mask, type(c), link(c));
+        return check_launch(c, "build_links_kernel");
+    }
+
+    static int init_equilibrium(lbm_ctx *c, int s, const void *rho, const void *u) {
+        init_equilibrium_kernel<L, T><<<grid_of(c), c->block_x, 0, c->stream>>>(
+            c->g, type(c), link(c), (const T *)rho, (const T *)u, at<T>(c, c->lay.store[s][c->cur]));
+        return check_launch(c, "init_equilibrium_kernel");
+    }
+
+    static int set_distributions(lbm_ctx *c, int s, const void *f) {
+        set_distributions_kernel<L, T><<<grid_of(c), c->block_x, 0, c->stream>>>(
+            c->g, type(c), link(c), (const T *)f, at<T>(c, c->lay.store[s][c->cur]));
+        return check_launch(c, "set_distributions_kernel");
+    }
+
+    static int get_distributions(lbm_ctx *c, int s, void *f) {
+        get_distributions_kernel<L, T><<<grid_of(c), c->block_x, 0, c->stream>>>(c->g, type(c), link(c), src(c, s), (T *)f);
+        return check_launch(c, "get_distributions_kernel");
+    }
+
+    static int macro(lbm_ctx *c, int s, void *rho, void *u) {
+        const bool sc = c->p.model == LBM_SC2;  // SC2: bare component velocity (lbm.h)
+        macro_kernel<L, T><<<grid_of(c), c->block_x, 0, c->stream>>>(
+            c->g, type(c), link(c), src(c, s), (T *)rho, (T *)u, sc ? T(0) : T(0.5 * c->p.force[0]),
+            sc ? T(0) : T(0.5 * c->p.force[1]), sc ? T(0) : T(0.5 * c->p.force[2]));
+        return check_launch(c, "macro_kernel");
+    }
+
+    static int get_stream_map(lbm_ctx *c, int64_t *map) {
+        stream_map_kernel<L><<<grid_of(c), c->block_x, 0, c->stream>>>(c->g, type(c), link(c), map);
+        return check_launch(c, "stream_map_kernel");
+    }
+
+    template <bool MRT, bool FORCE> static int step_single(lbm_ctx *c, int n, const Relax<T> &rp) {
+        const dim3 grid = grid_of(c);
+        for (int t = 0; t < n; t++) {
+            step_kernel<L, T, MRT, FORCE><<<grid, c->block_x, 0, c->stream>>>(c->g, type(c), link(c), src(c, 0), dst(c, 0), rp);
+            if (int rc = check_launch(c, "step_kernel")) return rc;
+            c->cur ^= 1;
+            c->steps++;
+        }
+        return LBM_OK;
+    }
+
+    template <int PSI> static int step_sc(lbm_ctx *c, int n) {
+        const dim3 grid = grid_of(c);
+        const Relax<T> rA = make_relax<T>(c, 0), rB = make_relax<T>(c, 1);
+        T *pA = at<T>(c, c->lay.psi[0]), *pB = at<T>(c, c->lay.psi[1]);
+        for (int t = 0; t < n; t++) {
+            sc_fields_kernel<L, T, PSI><<<grid, c->block_x, 0, c->stream>>>(c->g, type(c), link(c), src(c, 0), src(c, 1), pA, pB);
+            if (int rc = check_launch(c, "sc_fields_kernel")) return rc;
+            sc_step_kernel<L, T, PSI><<<grid, c->block_x, 0, c->stream>>>(
+                c->g, type(c), link(c), src(c, 0), src(c, 1), dst(c, 0), dst(c, 1), pA, pB, rA, rB, T(c->p.sc_G));
+            if (int rc = check_launch(c, "sc_step_kernel")) return rc;
+            c->cur ^= 1;
+            c->steps++;
+        }
+        return LBM_OK;
+    }
+
+    static int step(lbm_ctx *c, int n) {
+        if (c->p.model == LBM_SC2) return c->p.sc_psi == LBM_PSI_RHO ? step_sc<0>(c, n) : step_sc<1>(c, n);
+        Relax<T> rp = make_relax<T>(c, 0);
+        const bool force = c->p.force[0] != 0.0 || c->p.force[1] != 0.0 || c->p.force[2] != 0.0;
+        if (c->p.model == LBM_MRT) {
+            for (int k = 0; k < L::Q; k++) {  // M^-1 = M^T diag(1/|M_k|^2): rows are orthogonal (A5)
+                rp.cr[k] = T(c->p.rates[k] / Mrt<L, T>::norm(k));
+                rp.cs[k] = T((1.0 - 0.5 * c->p.rates[k]) / Mrt<L, T>::norm(k));
+            }
+            return force ? step_single<true, true>(c, n, rp) : step_single<true, false>(c, n, rp);
+        }
+        return force ? step_single<false, true>(c, n, rp) : step_single<false, false>(c, n, rp);
+    }
+
+    static const Vtbl *table() {
+        static const Vtbl vt = {&Impl::set_geometry, &Impl::init_equilibrium, &Impl::step, &Impl::macro,
+                                &Impl::get_distributions, &Impl::set_distributions, &Impl::get_stream_map};
+        return &vt;
+    }
+};
+
+const Vtbl *select_impl(const lbm_params *p) {
+    if (p->lattice == LBM_D2Q9) return p->precision == LBM_F32 ? Impl<D2Q9, float>::table() : Impl<D2Q9, double>::table();
+    return p->precision == LBM_F32 ? Impl<D3Q19, float>::table() : Impl<D3Q19, double>::table();
+}
+
+int pick_block_x(int nx) {
+    if (const char *e = getenv("LBM_BLOCK_X")) {
+        const int v = atoi(e);
+        if (v >= 32 && v <= 256 && v % 32 == 0) return v;
+    }
+    if (nx % 256 == 0) return 256;
+    if (nx % 128 == 0) return 128;
+    if (nx <= 256) return (nx + 31) / 32 * 32;
+    return 128;
+}
+
+}  // namespace
+
+// ---- exported C ABI ---------------------------------------------------------------------------
+#define LBM_API extern "C" __attribute__((visibility("default")))
+#define CHECK_CTX(c) do { if (!(c)) return fail(nullptr, LBM_EINVAL, "ctx is NULL"); } while (0)
+#define CHECK_COMP(c, s) do { if ((s) < 0 || (s) >= (c)->ncomp) return fail((c), LBM_EINVAL, "comp out of range"); } while (0)
+
+LBM_API int lbm_lattice_info(int32_t lattice, int32_t *Q, int32_t *D, int32_t *h_e, double *h_w, int32_t *h_opp) {
+    auto fill = [&](auto Ltag) {
+        using L = decltype(Ltag);
+        if (Q) *Q = L::Q;
+        if (D) *D = L::D;
+        for (int i = 0; i < L::Q; i++) {
+            if (h_e) { h_e[3 * i] = L::ex(i); h_e[3 * i + 1] = L::ey(i); h_e[3 * i + 2] = L::ez(i); }
+            if (h_w) h_w[i] = L::template w<double>(i);
+            if (h_opp) h_opp[i] = L::opp(i);
+        }
+    };
+    if (lattice == LBM_D2Q9) fill(D2Q9{});
+    else if (lattice == LBM_D3Q19) fill(D3Q19{});
+    else return fail(nullptr, LBM_EINVAL, "unknown lattice");
+    return LBM_OK;
+}
+
+LBM_API int lbm_workspace_bytes(const lbm_params *p, size_t *bytes) {
+    int Q, D;
+    if (int rc = validate(p, &Q, &D)) return rc;
+    if (!bytes) return fail(nullptr, LBM_EINVAL, "bytes is NULL");
+    Layout lay;
+    make_layout(p, Q, D, &lay);
+    *bytes = lay.total;
+    return LBM_OK;
+}
+
+LBM_API int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, void *cuda_stream, lbm_ctx **out) {
+    int Q, D;
+    if (int rc = validate(p, &Q, &D)) return rc;
+    if (!out) return fail(nullptr, LBM_EINVAL, "out is NULL");
+    *out = nullptr;
+    Layout lay;
+    make_layout(p, Q, D, &lay);
+    if (!d_workspace || bytes < lay.total) return fail(nullptr, LBM_EINVAL, "workspace NULL or smaller than lbm_workspace_bytes");
+    if (reinterpret_cast<uintptr_t>(d_workspace) % ALIGN) return fail(nullptr, LBM_EINVAL, "workspace must be 256-byte aligned");
+    lbm_ctx *c = new (std::nothrow) lbm_ctx();
+    if (!c) return fail(nullptr, LBM_ENOMEM, "host allocation failed");
+    c->p = *p;
+    c->Q = Q; c->D = D; c->ncomp = p->model == LBM_SC2 ? 2 : 1;
+    c->rs = p->precision == LBM_F32 ? 4 : 8;
+    c->g.nx = p->nx; c->g.ny = p->ny; c->g.nz = p->nz; c->g.N = (int64_t)p->nx * p->ny * p->nz;
+    c->stream = static_cast<cudaStream_t>(cuda_stream);
+    c->ws = static_cast<char *>(d_workspace);
+    c->lay = lay;
+    c->block_x = pick_block_x(p->nx);
+    c->vt = select_impl(p);
+    c->err[0] = 0;
+    // geometry starts all-FLUID: type = BULK, link = 0
+    cudaError_t e = cudaMemsetAsync(c->ws + lay.type, 0, (size_t)c->g.N, c->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(c->ws + lay.link, 0, 4 * (size_t)c->g.N, c->stream);
+    if (e != cudaSuccess) {
+        fail(nullptr, LBM_ECUDA, "cudaMemsetAsync: %s", cudaGetErrorString(e));
+        delete c;
+        return LBM_ECUDA;
+    }
+    *out = c;
+    return LBM_OK;
+}
+
+LBM_API int lbm_destroy(lbm_ctx *c) {
+    CHECK_CTX(c);
+    delete c;
+    return LBM_OK;
+}
+
+LBM_API int lbm_set_geometry(lbm_ctx *c, const uint8_t *d_mask) {
+    CHECK_CTX(c);
+    if (!d_mask) return fail(c, LBM_EINVAL, "d_mask is NULL");
+    if (c->geometry_frozen) return fail(c, LBM_ESTATE, "lbm_set_geometry after the state was initialised");
+    return c->vt->set_geometry(c, d_mask);
+}
+
+LBM_API int lbm_get_geometry(lbm_ctx *c, uint8_t *d_mask) {
+    CHECK_CTX(c);
+    if (!d_mask) return fail(c, LBM_EINVAL, "d_mask is NULL");
+    get_geometry_kernel<<<grid_of(c), c->block_x, 0, c->stream>>>(c->g, at<uint8_t>(c, c->lay.type), d_mask);
+    return check_launch(c, "get_geometry_kernel");
+}
+
+static void mark_initialised(lbm_ctx *c, int comp) {
+    c->inited[comp] = true;
+    c->geometry_frozen = true;
+    c->steps = 0;
+}
+
+LBM_API int lbm_init_equilibrium(lbm_ctx *c, int comp, const void *d_rho, const void *d_u) {
+    CHECK_CTX(c);
+    CHECK_COMP(c, comp);
+    if (!d_rho || !d_u) return fail(c, LBM_EINVAL, "d_rho / d_u is NULL");
+    if (int rc = c->vt->init_equilibrium(c, comp, d_rho, d_u)) return rc;
+    mark_initialised(c, comp);
+    return LBM_OK;
+}
+
+LBM_API int lbm_set_distributions(lbm_ctx *c, int comp, const void *d_f) {
+    CHECK_CTX(c);
+    CHECK_COMP(c, comp);
+    if (!d_f) return fail(c, LBM_EINVAL, "d_f is NULL");
+    if (int rc = c->vt->set_distributions(c, comp, d_f)) return rc;
+    mark_initialised(c, comp);
+    return LBM_OK;
+}
+
+static int check_state(lbm_ctx *c) {
+    for (int s = 0; s < c->ncomp; s++)
+        if (!c->inited[s]) return fail(c, LBM_ESTATE, "a component has not been initialised");
+    return LBM_OK;
+}
+
+LBM_API int lbm_step(lbm_ctx *c, int n) {
+    CHECK_CTX(c);
+    if (n < 0) return fail(c, LBM_EINVAL, "n < 0");
+    if (int rc = check_state(c)) return rc;
+    return c->vt->step(c, n);
+}
+
+LBM_API int lbm_macro(lbm_ctx *c, int comp, void *d_rho, void *d_u) {
+    CHECK_CTX(c);
+    CHECK_COMP(c, comp);
+    if (!c->inited[comp]) return fail(c, LBM_ESTATE, "component has not been initialised");
+    if (!d_rho && !d_u) return LBM_OK;
+    return c->vt->macro(c, comp, d_rho, d_u);
+}
+
+LBM_API int lbm_get_distributions(lbm_ctx *c, int comp, void *d_f) {
+    CHECK_CTX(c);
+    CHECK_COMP(c, comp);
+    if (!d_f) return fail(c, LBM_EINVAL, "d_f is NULL");
+    if (!c->inited[comp]) return fail(c, LBM_ESTATE, "component has not been initialised");
+    return c->vt->get_distributions(c, comp, d_f);
+}
+
+LBM_API int lbm_get_stream_map(lbm_ctx *c, int64_t *d_map) {
+    CHECK_CTX(c);
+    if (!d_map) return fail(c, LBM_EINVAL, "d_map is NULL");
+    return c->vt->get_stream_map(c, d_map);
+}
+
+#define CUDA_TRY(c, call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { \
+    snprintf((c)->err, sizeof (c)->err, "%s: %s", #call, cudaGetErrorString(e_)); return LBM_ECUDA; } } while (0)
+
+LBM_API int lbm_run_host(lbm_ctx *c, const uint8_t *h_mask, const void *const *h_rho0, const void *const *h_u0,
+                         int n, void *h_rho_out, void *h_u_out) {
+    CHECK_CTX(c);
+    if (n < 0 || !h_rho0 || !h_u0) return fail(c, LBM_EINVAL, "bad arguments to lbm_run_host");
+    for (int s = 0; s < c->ncomp; s++)
+        if (!h_rho0[s] || !h_u0[s]) return fail(c, LBM_EINVAL, "h_rho0[s] / h_u0[s] is NULL");
+    const size_t N = (size_t)c->g.N, rs = c->rs;
+    uint8_t *d_mask = at<uint8_t>(c, c->lay.stage_mask);
+    char *d_rho = c->ws + c->lay.stage_rho, *d_u = c->ws + c->lay.stage_u;
+    // reset: new geometry allowed, nothing initialised
+    c->geometry_frozen = false;
+    c->inited[0] = c->inited[1] = false;
+    c->cur = 0;
+    if (h_mask) {
+        CUDA_TRY(c, cudaMemcpyAsync(d_mask, h_mask, N, cudaMemcpyHostToDevice, c->stream));
+    } else {
+        CUDA_TRY(c, cudaMemsetAsync(d_mask, 0, N, c->stream));
+    }
+    if (int rc = lbm_set_geometry(c, d_mask)) return rc;
+    for (int s = 0; s < c->ncomp; s++) {
+        CUDA_TRY(c, cudaMemcpyAsync(d_rho, h_rho0[s], N * rs, cudaMemcpyHostToDevice, c->stream));
+        CUDA_TRY(c, cudaMemcpyAsync(d_u, h_u0[s], c->D * N * rs, cudaMemcpyHostToDevice, c->stream));
+        if (int rc = lbm_init_equilibrium(c, s, d_rho, d_u)) return rc;
+    }
+    if (int rc = lbm_step(c, n)) return rc;
+    if (h_rho_out || h_u_out) {
+        if (int rc = lbm_macro(c, 0, h_rho_out ? d_rho : nullptr, h_u_out ? d_u : nullptr)) return rc;
+        if (h_rho_out) CUDA_TRY(c, cudaMemcpyAsync(h_rho_out, d_rho, N * rs, cudaMemcpyDeviceToHost, c->stream));
+        if (h_u_out) CUDA_TRY(c, cudaMemcpyAsync(h_u_out, d_u, c->D * N * rs, cudaMemcpyDeviceToHost, c->stream));
+    }
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    return LBM_OK;
+}
+
+LBM_API int lbm_get_counters(const lbm_ctx *c, int64_t *steps, int64_t *launches) {
+    CHECK_CTX(c);
+    if (steps) *steps = c->steps;
+    if (launches) *launches = c->launches;
+    return LBM_OK;
+}
+
+LBM_API const char *lbm_last_error(const lbm_ctx *c) { return c ? c->err : g_err; }

@@ -1,0 +1,136 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element on the
+same seeded inputs.  Bars (BASELINE.json north_star): after 100 steps max |f_gpu - f_oracle| over
+FLUID slots <= 1e-5 (fp32) / 1e-12 (fp64); node masks and streaming index maps bit-exact."""
+import numpy as np
+import pytest
+
+from paper_1311_2404_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL = {W.F32: 1e-5, W.F64: 1e-12}
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1311_2404_b200 import binding
+    binding.load()  # fails loudly if liblbm_b200.so is missing: there is no fallback
+    return binding
+
+
+def make_pair(B, orc, w):
+    """(gpu context, oracle) for workload w, same geometry and initial fields."""
+    sim = B.from_workload(w)
+    ref = orc.Oracle(**w.params())
+    if w.mask is not None:
+        sim.set_geometry(w.mask)
+        ref.set_geometry(w.mask)
+    for s in range(w.ncomp):
+        sim.init_equilibrium(w.rho[s], w.u[s], comp=s)
+        ref.init_equilibrium(w.rho[s], w.u[s], comp=s)
+    return sim, ref
+
+
+def max_err(sim, ref, w, comp=0):
+    f_gpu = sim.get_distributions(comp).cpu().numpy().astype(np.float64)
+    f_ref = ref.get_distributions(comp)
+    fluid = (w.mask == 0) if w.mask is not None else np.ones(ref.shape, bool)
+    return np.abs(f_gpu - f_ref)[:, fluid].max()
+
+
+def check_parity(B, orc, w, steps=100):
+    sim, ref = make_pair(B, orc, w)
+    # the oracle gets the inputs in fp64, the GPU in w.precision: compare the *initial* state too
+    for s in range(w.ncomp):
+        assert max_err(sim, ref, w, s) <= (1e-7 if w.precision == W.F32 else 1e-15)
+    sim.step(steps)
+    ref.step(steps)
+    errs = [max_err(sim, ref, w, s) for s in range(w.ncomp)]
+    assert max(errs) <= TOL[w.precision], errs
+    # macro fields through the ABI as well
+    for s in range(w.ncomp):
+        rho_g, u_g = sim.macro(s)
+        rho_r, u_r = ref.macro(s)
+        tol = 1e-5 if w.precision == W.F32 else 1e-12
+        assert np.abs(rho_g.cpu().numpy() - rho_r).max() <= tol
+        assert np.abs(u_g.cpu().numpy() - u_r).max() <= tol
+    sim.close()
+    return errs
+
+
+# ---- the five configs at sizes the oracle finishes in seconds (several blocks + ragged tails) ---
+def test_c1_taylor_green_d2q9_full_size(B, orc):
+    check_parity(B, orc, W.c1_taylor_green())  # 128 x 128 is the full config
+
+
+@pytest.mark.parametrize("shape", [(96, 40, 24), (50, 37, 29), (300, 9, 7)])
+def test_c2_channel_bgk_force_fp32(B, orc, shape):
+    check_parity(B, orc, W.c2_channel(*shape))
+
+
+@pytest.mark.parametrize("precision", [W.F32, W.F64])
+@pytest.mark.parametrize("shape", [(64, 48, 40), (45, 31, 22)])
+def test_c3_mrt_random_solids(B, orc, shape, precision):
+    check_parity(B, orc, W.c3_mrt_obstacles(*shape, precision=precision))
+
+
+@pytest.mark.parametrize("shape", [(64, 32, 32), (70, 21, 19)])
+def test_c4_duct_fp64(B, orc, shape):
+    check_parity(B, orc, W.c4_duct(*shape))
+
+
+@pytest.mark.parametrize("precision", [W.F32, W.F64])
+@pytest.mark.parametrize("shape", [(48, 40, 32), (35, 30, 21)])
+def test_c5_shan_chen(B, orc, shape, precision):
+    check_parity(B, orc, W.c5_shan_chen(*shape, precision=precision))
+
+
+# ---- combinations outside the configs -------------------------------------------------------------
+def generic(lattice, model, precision, shape, seed, solid=0.1, **kw):
+    nx, ny, nz = shape
+    ncomp = 2 if model == W.SC2 else 1
+    mask, rho, u = W.random_state(lattice, nx, ny, nz, seed, solid_fraction=solid, ncomp=ncomp)
+    w = W.Workload("generic", lattice, model, precision, nx, ny, nz, kw.pop("tau", (0.7, 0.9)), 100, **kw)
+    w.mask, w.rho, w.u = mask, rho, u
+    return w
+
+
+@pytest.mark.parametrize("precision", [W.F32, W.F64])
+def test_mrt_with_force_and_solids_d3q19(B, orc, precision):
+    check_parity(B, orc, generic(W.D3Q19, W.MRT, precision, (40, 33, 18), 11, rates=W.mrt_rates_d3q19(0.7),
+                                 force=(1e-5, -2e-5, 3e-5)))
+
+
+@pytest.mark.parametrize("model", [W.BGK, W.MRT])
+@pytest.mark.parametrize("precision", [W.F32, W.F64])
+def test_d2q9_models_with_force_and_solids(B, orc, model, precision):
+    check_parity(B, orc, generic(W.D2Q9, model, precision, (70, 45, 1), 12, rates=W.mrt_rates_d2q9(0.7),
+                                 force=(2e-5, -1e-5, 0.0)))
+
+
+@pytest.mark.parametrize("lattice,shape", [(W.D2Q9, (40, 36, 1)), (W.D3Q19, (33, 20, 17))])
+@pytest.mark.parametrize("psi", [0, 1])
+def test_shan_chen_variants(B, orc, lattice, shape, psi):
+    """tau_A != tau_B, body force, solids (psi = 0 there, A14), both pseudopotentials."""
+    w = generic(lattice, W.SC2, W.F64, shape, 13, solid=0.05, tau=(0.8, 1.1), sc_G=0.7, sc_psi=psi,
+                force=(1e-5, 2e-5, 0.0))
+    check_parity(B, orc, w)
+
+
+@pytest.mark.parametrize("shape", [(1, 1, 1), (2, 1, 1), (1, 3, 2), (3, 2, 1), (33, 1, 1)])
+def test_degenerate_extents(B, orc, shape):
+    """Tori of extent 1 and 2: a node is its own neighbour / has the same neighbour on both sides."""
+    check_parity(B, orc, generic(W.D3Q19, W.BGK, W.F64, shape, 14, solid=0.0, force=(1e-5, 0, 0)), steps=20)
+
+
+def test_all_solid_and_all_fluid(B, orc):
+    w = generic(W.D3Q19, W.BGK, W.F64, (9, 8, 7), 15, solid=0.0)
+    check_parity(B, orc, w, steps=10)
+    w.mask[:] = 1
+    sim, ref = make_pair(B, orc, w)
+    sim.step(3)
+    rho, u = sim.macro()
+    assert float(rho.abs().max()) == 0.0 and float(u.abs().max()) == 0.0
+    assert (sim.get_stream_map().cpu().numpy() == -1).all()
