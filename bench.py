@@ -248,7 +248,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="c2", choices=sorted(W.CONFIGS))
     ap.add_argument("--repeats", type=int, default=1)
-    ap.add_argument("--cpu-steps", type=int, default=40, help="oracle steps on the bounded sample")
+    ap.add_argument("--cpu-steps", type=int, default=250, help="oracle steps on the bounded sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
