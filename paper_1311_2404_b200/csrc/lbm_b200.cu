@@ -38,7 +38,9 @@ struct lbm_ctx {
     bool inited[2];
     bool geometry_frozen;
     int64_t steps, launches;
-    int block_x;
+    int block_x;        // one-node-per-thread kernels: 1-D block along x
+    int vec;            // nodes per thread of the step kernels (1, 2 or 4 consecutive x)
+    int block_threads;  // threads per block of the step kernels
     const Vtbl *vt;
     char err[256];
 };
@@ -131,6 +133,21 @@ template <typename T> Relax<T> make_relax(const lbm_ctx *c, int comp) {
 }
 
 // ---- per <lattice, real> implementation -------------------------------------------------------
+struct Launch { dim3 grid, block; };
+
+// Step kernels: V nodes per thread along x, 2-D blocks (bx packs) x (by rows).
+Launch span_launch(const lbm_ctx *c, int V) {
+    const int nxv = c->g.nx / V;
+    const int bx = nxv > 32 ? 64 : 32;
+    int by = c->block_threads / bx;
+    if (by < 1) by = 1;
+    while (by > 1 && by / 2 >= c->g.ny) by /= 2;
+    Launch l;
+    l.block = dim3(bx, by, 1);
+    l.grid = dim3((nxv + bx - 1) / bx, (c->g.ny + by - 1) / by, c->g.nz);
+    return l;
+}
+
 template <class L, typename T> struct Impl {
     static const T *src(lbm_ctx *c, int s) { return at<T>(c, c->lay.store[s][c->cur]); }
     static T *dst(lbm_ctx *c, int s) { return at<T>(c, c->lay.store[s][c->cur ^ 1]); }
@@ -144,25 +161,25 @@ template <class L, typename T> struct Impl {
 
     static int init_equilibrium(lbm_ctx *c, int s, const void *rho, const void *u) {
         init_equilibrium_kernel<L, T><<<grid_of(c), c->block_x, 0, c->stream>>>(
-            c->g, type(c), link(c), (const T *)rho, (const T *)u, at<T>(c, c->lay.store[s][c->cur]));
+            c->g, type(c), (const T *)rho, (const T *)u, at<T>(c, c->lay.store[s][c->cur]));
         return check_launch(c, "init_equilibrium_kernel");
     }
 
     static int set_distributions(lbm_ctx *c, int s, const void *f) {
         set_distributions_kernel<L, T><<<grid_of(c), c->block_x, 0, c->stream>>>(
-            c->g, type(c), link(c), (const T *)f, at<T>(c, c->lay.store[s][c->cur]));
+            c->g, type(c), (const T *)f, at<T>(c, c->lay.store[s][c->cur]));
         return check_launch(c, "set_distributions_kernel");
     }
 
     static int get_distributions(lbm_ctx *c, int s, void *f) {
-        get_distributions_kernel<L, T><<<grid_of(c), c->block_x, 0, c->stream>>>(c->g, type(c), link(c), src(c, s), (T *)f);
+        get_distributions_kernel<L, T><<<grid_of(c), c->block_x, 0, c->stream>>>(c->g, type(c), src(c, s), (T *)f);
         return check_launch(c, "get_distributions_kernel");
     }
 
     static int macro(lbm_ctx *c, int s, void *rho, void *u) {
         const bool sc = c->p.model == LBM_SC2;  // SC2: bare component velocity (lbm.h)
         macro_kernel<L, T><<<grid_of(c), c->block_x, 0, c->stream>>>(
-            c->g, type(c), link(c), src(c, s), (T *)rho, (T *)u, sc ? T(0) : T(0.5 * c->p.force[0]),
+            c->g, type(c), src(c, s), (T *)rho, (T *)u, sc ? T(0) : T(0.5 * c->p.force[0]),
             sc ? T(0) : T(0.5 * c->p.force[1]), sc ? T(0) : T(0.5 * c->p.force[2]));
         return check_launch(c, "macro_kernel");
     }
@@ -172,10 +189,10 @@ template <class L, typename T> struct Impl {
         return check_launch(c, "stream_map_kernel");
     }
 
-    template <bool MRT, bool FORCE> static int step_single(lbm_ctx *c, int n, const Relax<T> &rp) {
-        const dim3 grid = grid_of(c);
+    template <int V, bool MRT, bool FORCE> static int step_single_v(lbm_ctx *c, int n, const Relax<T> &rp) {
+        const Launch l = span_launch(c, V);
         for (int t = 0; t < n; t++) {
-            step_kernel<L, T, MRT, FORCE><<<grid, c->block_x, 0, c->stream>>>(c->g, type(c), link(c), src(c, 0), dst(c, 0), rp);
+            step_kernel<L, T, V, MRT, FORCE><<<l.grid, l.block, 0, c->stream>>>(c->g, type(c), link(c), src(c, 0), dst(c, 0), rp);
             if (int rc = check_launch(c, "step_kernel")) return rc;
             c->cur ^= 1;
             c->steps++;
@@ -183,20 +200,35 @@ template <class L, typename T> struct Impl {
         return LBM_OK;
     }
 
-    template <int PSI> static int step_sc(lbm_ctx *c, int n) {
-        const dim3 grid = grid_of(c);
+    template <bool MRT, bool FORCE> static int step_single(lbm_ctx *c, int n, const Relax<T> &rp) {
+        if constexpr (sizeof(T) == 4) {
+            if (c->vec == 4) return step_single_v<4, MRT, FORCE>(c, n, rp);
+        }
+        if (c->vec == 2) return step_single_v<2, MRT, FORCE>(c, n, rp);
+        return step_single_v<1, MRT, FORCE>(c, n, rp);
+    }
+
+    template <int V, int PSI> static int step_sc_v(lbm_ctx *c, int n) {
+        const Launch l = span_launch(c, V);
         const Relax<T> rA = make_relax<T>(c, 0), rB = make_relax<T>(c, 1);
         T *pA = at<T>(c, c->lay.psi[0]), *pB = at<T>(c, c->lay.psi[1]);
         for (int t = 0; t < n; t++) {
-            sc_fields_kernel<L, T, PSI><<<grid, c->block_x, 0, c->stream>>>(c->g, type(c), link(c), src(c, 0), src(c, 1), pA, pB);
+            sc_fields_kernel<L, T, V, PSI><<<l.grid, l.block, 0, c->stream>>>(c->g, type(c), src(c, 0), src(c, 1), pA, pB);
             if (int rc = check_launch(c, "sc_fields_kernel")) return rc;
-            sc_step_kernel<L, T, PSI><<<grid, c->block_x, 0, c->stream>>>(
+            sc_step_kernel<L, T, V, PSI><<<l.grid, l.block, 0, c->stream>>>(
                 c->g, type(c), link(c), src(c, 0), src(c, 1), dst(c, 0), dst(c, 1), pA, pB, rA, rB, T(c->p.sc_G));
             if (int rc = check_launch(c, "sc_step_kernel")) return rc;
             c->cur ^= 1;
             c->steps++;
         }
         return LBM_OK;
+    }
+
+    template <int PSI> static int step_sc(lbm_ctx *c, int n) {
+        if constexpr (sizeof(T) == 4) {  // fp64 with two components and V = 2 would spill
+            if (c->vec >= 2) return step_sc_v<2, PSI>(c, n);
+        }
+        return step_sc_v<1, PSI>(c, n);
     }
 
     static int step(lbm_ctx *c, int n) {
@@ -223,6 +255,23 @@ template <class L, typename T> struct Impl {
 const Vtbl *select_impl(const lbm_params *p) {
     if (p->lattice == LBM_D2Q9) return p->precision == LBM_F32 ? Impl<D2Q9, float>::table() : Impl<D2Q9, double>::table();
     return p->precision == LBM_F32 ? Impl<D3Q19, float>::table() : Impl<D3Q19, double>::table();
+}
+
+int env_int(const char *name, int dflt, int lo, int hi) {
+    if (const char *e = getenv(name)) {
+        const int v = atoi(e);
+        if (v >= lo && v <= hi) return v;
+    }
+    return dflt;
+}
+
+// Nodes per thread: the widest pack (16 bytes) that divides nx; LBM_VEC overrides downwards.
+int pick_vec(const lbm_params *p) {
+    const int widest = p->precision == LBM_F32 ? 4 : 2;
+    int v = env_int("LBM_VEC", widest, 1, widest);
+    if (v == 3) v = 2;
+    while (v > 1 && p->nx % v) v /= 2;
+    return v;
 }
 
 int pick_block_x(int nx) {
@@ -289,6 +338,8 @@ LBM_API int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, voi
     c->ws = static_cast<char *>(d_workspace);
     c->lay = lay;
     c->block_x = pick_block_x(p->nx);
+    c->vec = pick_vec(p);
+    c->block_threads = env_int("LBM_BLOCK_THREADS", 128, 32, 256);
     c->vt = select_impl(p);
     c->err[0] = 0;
     // geometry starts all-FLUID: type = BULK, link = 0

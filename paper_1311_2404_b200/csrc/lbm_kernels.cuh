@@ -1,10 +1,13 @@
 // lbm_kernels.cuh -- sm_100a kernels of the fused stream-and-collide path (Alg. 1).
 //
 // Store: structure of arrays real[Q][N], x fastest, holding
-// the DEVIATION h = f - w (reading A12) of the POST-collision populations (reading A9): the
-// step kernel pulls h*_i(x - e_i) (or, behind a SOLID neighbour, its own h*_ibar(x): half-way
-// bounce-back, reading A8), collides in registers and writes h*(x) to the other buffer
-// with aligned, fully coalesced stores.  Every slot is read once and written once per step.
+// the DEVIATION h = f - w (reading A12) of the POST-collision populations (reading A9).
+//   * load side: f_i(x, t+1) is ALWAYS pulled from slot (i, x - e_i); no per-link selects.
+//   * store side: a node writes its post-collision h*_i(x) to (i, x) with aligned vector stores;
+//     for every link whose pull source x - e_i is SOLID (half-way bounce-back, reading
+//     A8) it also writes h*_ibar(x) into the otherwise unused slot (i, x - e_i) of that SOLID
+//     node, which is exactly what the pull of the next step must return.  SOLID nodes write
+//     nothing, so each slot has one writer and is read once and written once per step.
 #pragma once
 #include <cuda_runtime.h>
 #include "lbm_node.cuh"
@@ -47,23 +50,36 @@ template <class L> __device__ __forceinline__ int shift(int i, int s, const Nbr 
     if (ez == 1) d += o.zp; else if (ez == -1) d += o.zm;
     return d;
 }
-
-// THE gather rule (reading A8): slot (i' * N + x') of the post-collision store that supplies
-// f_i(x, t+1).  Used by the step kernels, the read-out kernels and lbm_get_stream_map alike.
-template <class L>
-__device__ __forceinline__ int64_t source_slot(int i, int n, int64_t N, const Nbr &o, uint32_t link) {
-    return ((link >> i) & 1u) ? (int64_t)L::opp(i) * N + n
-                              : (int64_t)i * N + (n + shift<L>(i, -1, o));
+// y/z part only (multiples of nx: keeps 16-byte alignment of vector accesses)
+template <class L> __device__ __forceinline__ int shift_yz(int i, int s, const Nbr &o) {
+    int d = 0;
+    const int ey = s * L::ey(i), ez = s * L::ez(i);
+    if (ey == 1) d += o.yp; else if (ey == -1) d += o.ym;
+    if (ez == 1) d += o.zp; else if (ez == -1) d += o.zm;
+    return d;
 }
 
+// THE streaming rule (reading A8), used by the step kernels' store side and by
+// lbm_get_stream_map alike: is population i of a node with link word `link` reflected?
+__device__ __forceinline__ bool reflected(uint32_t link, int i) { return (link >> i) & 1u; }
+
+// Store-side half of the rule: after writing h*(x), feed every reflected link.
 template <class L, typename T>
-__device__ __forceinline__ void gather(const T *__restrict__ src, int n, int64_t N, const Nbr &o,
-                                       uint32_t link, T (&h)[L::Q]) {
+__device__ __forceinline__ void feed_reflected_links(T *__restrict__ dst, int n, int64_t N, const Nbr &o,
+                                                     uint32_t link, const T (&h)[L::Q]) {
 #pragma unroll
-    for (int i = 0; i < L::Q; i++) h[i] = __ldg(src + source_slot<L>(i, n, N, o, link));
+    for (int i = 1; i < L::Q; i++)
+        if (reflected(link, i)) dst[(int64_t)i * N + (n + shift<L>(i, -1, o))] = h[L::opp(i)];
 }
 
-// Thread -> node: 1-D blocks along x, grid (ceil(nx/BX), ny, nz).
+// Load-side half: plain pull.
+template <class L, typename T>
+__device__ __forceinline__ void gather(const T *__restrict__ src, int n, int64_t N, const Nbr &o, T (&h)[L::Q]) {
+#pragma unroll
+    for (int i = 0; i < L::Q; i++) h[i] = __ldg(src + ((int64_t)i * N + (n + shift<L>(i, -1, o))));
+}
+
+// Thread -> node for the one-node-per-thread kernels: 1-D blocks along x.
 __device__ __forceinline__ bool thread_node(const Geom &g, int &x, int &y, int &z, int &n) {
     x = blockIdx.x * blockDim.x + threadIdx.x;
     y = blockIdx.y;
@@ -103,58 +119,189 @@ __global__ void stream_map_kernel(Geom g, const uint8_t *__restrict__ type, cons
     const Nbr o = neighbours(g, x, y, z);
     const uint32_t w = (t == NODE_BOUNDARY) ? link[n] : 0u;
 #pragma unroll
-    for (int i = 0; i < L::Q; i++)
-        map[(int64_t)i * g.N + n] = (t == NODE_SOLID) ? int64_t(-1) : source_slot<L>(i, n, g.N, o, w);
+    for (int i = 0; i < L::Q; i++) {
+        int64_t s = reflected(w, i) ? (int64_t)L::opp(i) * g.N + n : (int64_t)i * g.N + (n + shift<L>(i, -1, o));
+        map[(int64_t)i * g.N + n] = (t == NODE_SOLID) ? int64_t(-1) : s;
+    }
+}
+
+// ---- V consecutive x-nodes per thread, 16-byte (or 8-byte) global accesses -------------------
+template <typename T, int V> struct Pack;
+template <typename T> struct Pack<T, 1> {
+    static __device__ __forceinline__ void ld(const T *p, T (&a)[1]) { a[0] = __ldg(p); }
+    static __device__ __forceinline__ void st(T *p, const T (&a)[1]) { __stcs(p, a[0]); }
+    static __device__ __forceinline__ void stp(T *p, const T (&a)[1]) { *p = a[0]; }
+};
+template <> struct Pack<float, 2> {
+    static __device__ __forceinline__ void ld(const float *p, float (&a)[2]) {
+        const float2 v = __ldg(reinterpret_cast<const float2 *>(p)); a[0] = v.x; a[1] = v.y;
+    }
+    static __device__ __forceinline__ void st(float *p, const float (&a)[2]) {
+        __stcs(reinterpret_cast<float2 *>(p), make_float2(a[0], a[1]));
+    }
+    static __device__ __forceinline__ void stp(float *p, const float (&a)[2]) {
+        *reinterpret_cast<float2 *>(p) = make_float2(a[0], a[1]);
+    }
+};
+template <> struct Pack<float, 4> {
+    static __device__ __forceinline__ void ld(const float *p, float (&a)[4]) {
+        const float4 v = __ldg(reinterpret_cast<const float4 *>(p)); a[0] = v.x; a[1] = v.y; a[2] = v.z; a[3] = v.w;
+    }
+    static __device__ __forceinline__ void st(float *p, const float (&a)[4]) {
+        __stcs(reinterpret_cast<float4 *>(p), make_float4(a[0], a[1], a[2], a[3]));
+    }
+    static __device__ __forceinline__ void stp(float *p, const float (&a)[4]) {
+        *reinterpret_cast<float4 *>(p) = make_float4(a[0], a[1], a[2], a[3]);
+    }
+};
+template <> struct Pack<double, 2> {
+    static __device__ __forceinline__ void ld(const double *p, double (&a)[2]) {
+        const double2 v = __ldg(reinterpret_cast<const double2 *>(p)); a[0] = v.x; a[1] = v.y;
+    }
+    static __device__ __forceinline__ void st(double *p, const double (&a)[2]) {
+        __stcs(reinterpret_cast<double2 *>(p), make_double2(a[0], a[1]));
+    }
+    static __device__ __forceinline__ void stp(double *p, const double (&a)[2]) {
+        *reinterpret_cast<double2 *>(p) = make_double2(a[0], a[1]);
+    }
+};
+
+// A thread's V nodes: x0 .. x0+V-1 of row (y, z); nx % V == 0 so a pack never straddles a row.
+struct Span {
+    int x0, y, z;
+    int row;     // node index of (0, y, z)
+    int xm, xp;  // x-coordinate left of x0 and right of x0+V-1 on the torus
+    Nbr o;       // o.xm / o.xp unused here (per-node x offsets differ inside the pack)
+};
+
+template <int V> __device__ __forceinline__ bool thread_span(const Geom &g, Span &s) {
+    s.x0 = (blockIdx.x * blockDim.x + threadIdx.x) * V;
+    s.y = blockIdx.y * blockDim.y + threadIdx.y;
+    s.z = blockIdx.z;
+    if (s.x0 >= g.nx || s.y >= g.ny) return false;
+    s.row = (s.z * g.ny + s.y) * g.nx;
+    s.xm = (s.x0 == 0) ? g.nx - 1 : s.x0 - 1;
+    s.xp = (s.x0 + V == g.nx) ? 0 : s.x0 + V;
+    s.o = neighbours(g, 1, s.y, s.z);
+    return true;
+}
+
+// Pull for V nodes (row a2): e_x = 0 planes with one aligned vector load; e_x = +-1 planes with
+// the aligned vector of the source row plus ONE scalar for the element that falls outside the
+// pack (an L1 hit: the neighbouring thread's vector load brings the same sector).
+template <class L, typename T, int V>
+__device__ __forceinline__ void gather_span(const T *__restrict__ src, int64_t N, const Span &s, T (&h)[V][L::Q]) {
+#pragma unroll
+    for (int i = 0; i < L::Q; i++) {
+        const T *row = src + ((int64_t)i * N + (s.row + shift_yz<L>(i, -1, s.o)));
+        if (L::ex(i) == 0) {
+            T a[V];
+            Pack<T, V>::ld(row + s.x0, a);
+#pragma unroll
+            for (int k = 0; k < V; k++) h[k][i] = a[k];
+        } else if (L::ex(i) == 1) {  // source x - 1
+            h[0][i] = __ldg(row + s.xm);
+            if (V > 1) {
+                T a[V];
+                Pack<T, V>::ld(row + s.x0, a);
+#pragma unroll
+                for (int k = 1; k < V; k++) h[k][i] = a[k - 1];
+            }
+        } else {  // source x + 1
+            h[V - 1][i] = __ldg(row + s.xp);
+            if (V > 1) {
+                T a[V];
+                Pack<T, V>::ld(row + s.x0, a);
+#pragma unroll
+                for (int k = 0; k < V - 1; k++) h[k][i] = a[k + 1];
+            }
+        }
+    }
+}
+
+// Node types of the pack as one word (byte k = node k).
+template <int V> __device__ __forceinline__ uint32_t load_types(const uint8_t *__restrict__ type, int n0) {
+    if (V == 4) return __ldg(reinterpret_cast<const uint32_t *>(type + n0));
+    if (V == 2) return __ldg(reinterpret_cast<const uint16_t *>(type + n0));
+    return __ldg(type + n0);
+}
+template <int V> __device__ __forceinline__ bool all_solid(uint32_t t) {
+    return t == (V == 4 ? 0x01010101u : V == 2 ? 0x0101u : 0x01u);
+}
+
+// Store for V nodes (row a8) + the reflected links of BOUNDARY nodes.
+template <class L, typename T, int V>
+__device__ __forceinline__ void store_span(T *__restrict__ dst, const Geom &g, const Span &s, uint32_t types,
+                                           const uint32_t *__restrict__ link, const T (&h)[V][L::Q]) {
+    const int n0 = s.row + s.x0;
+    if ((types & 0x01010101u) == 0) {  // no SOLID node in the pack: aligned vector stores
+#pragma unroll
+        for (int i = 0; i < L::Q; i++) {
+            T a[V];
+#pragma unroll
+            for (int k = 0; k < V; k++) a[k] = h[k][i];
+            Pack<T, V>::st(dst + ((int64_t)i * g.N + n0), a);
+        }
+    } else {  // SOLID slots belong to their neighbours' reflected links: do not touch them
+#pragma unroll
+        for (int k = 0; k < V; k++)
+            if (((types >> (8 * k)) & 0xffu) != NODE_SOLID) {
+#pragma unroll
+                for (int i = 0; i < L::Q; i++) dst[(int64_t)i * g.N + (n0 + k)] = h[k][i];
+            }
+    }
+    if (types & 0x02020202u) {
+#pragma unroll
+        for (int k = 0; k < V; k++)
+            if (((types >> (8 * k)) & 0xffu) == NODE_BOUNDARY) {
+                Nbr o = s.o;
+                const int x = s.x0 + k;
+                o.xm = (x == 0) ? (g.nx - 1) : -1;
+                o.xp = (x == g.nx - 1) ? -(g.nx - 1) : 1;
+                feed_reflected_links<L, T>(dst, n0 + k, g.N, o, __ldg(link + n0 + k), h[k]);
+            }
+    }
 }
 
 // ---- the fused step: pull-stream + moments + equilibrium + collision (+ Guo) + store ---------
-// Rows a1-a8 of DESIGN.md.  One node per thread; Q independent loads are issued before first
-// use (bytes in flight), stores are aligned and streaming (each slot is touched once per step).
-template <class L, typename T, bool MRT, bool FORCE>
+// Rows a1-a8 of DESIGN.md.  All loads of the pack are issued before first use (bytes in flight).
+template <class L, typename T, int V, bool MRT, bool FORCE>
 __global__ void __launch_bounds__(256)
 step_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restrict__ link,
             const T *__restrict__ src, T *__restrict__ dst, Relax<T> rp) {
-    int x, y, z, n;
-    if (!thread_node(g, x, y, z, n)) return;
-    const uint8_t t = type[n];
-    if (t == NODE_SOLID) return;
-    const uint32_t w = (t == NODE_BOUNDARY) ? link[n] : 0u;
-    const Nbr o = neighbours(g, x, y, z);
-    T h[L::Q];
-    gather<L, T>(src, n, g.N, o, w, h);
-    update_node<L, T, MRT, FORCE>(h, rp);
+    Span s;
+    if (!thread_span<V>(g, s)) return;
+    const uint32_t types = load_types<V>(type, s.row + s.x0);
+    if (all_solid<V>(types)) return;
+    T h[V][L::Q];
+    gather_span<L, T, V>(src, g.N, s, h);
 #pragma unroll
-    for (int i = 0; i < L::Q; i++) __stcs(dst + (int64_t)i * g.N + n, h[i]);
+    for (int k = 0; k < V; k++) update_node<L, T, MRT, FORCE>(h[k], rp);
+    store_span<L, T, V>(dst, g, s, types, link, h);
 }
 
 // ---- canonical <-> internal conversions (off the hot loop; reading A9) ----------------------
-// canonical f_i(x,t) -> store: S[source_slot(i,x)] = f_i(x) - w_i (inverse of the gather; the
-// gather is a permutation of FLUID slots, so every FLUID slot is written exactly once).
+// canonical f_i(x,t) -> store: S[(i, x - e_i)] = f_i(x) - w_i, the inverse of the pull.  Slot
+// (i, y) is written by x = y + e_i only, so every slot a FLUID node will pull is written once.
 template <class L, typename T>
-__global__ void set_distributions_kernel(Geom g, const uint8_t *__restrict__ type,
-                                         const uint32_t *__restrict__ link, const T *__restrict__ f,
+__global__ void set_distributions_kernel(Geom g, const uint8_t *__restrict__ type, const T *__restrict__ f,
                                          T *__restrict__ store) {
     int x, y, z, n;
     if (!thread_node(g, x, y, z, n)) return;
-    const uint8_t t = type[n];
-    if (t == NODE_SOLID) return;
-    const uint32_t w = (t == NODE_BOUNDARY) ? link[n] : 0u;
+    if (type[n] == NODE_SOLID) return;
     const Nbr o = neighbours(g, x, y, z);
 #pragma unroll
     for (int i = 0; i < L::Q; i++)
-        store[source_slot<L>(i, n, g.N, o, w)] = f[(int64_t)i * g.N + n] - L::template w<T>(i);
+        store[(int64_t)i * g.N + (n + shift<L>(i, -1, o))] = f[(int64_t)i * g.N + n] - L::template w<T>(i);
 }
 
 // f_i(x,0) = f_i^eq(rho0, u0), eq. (3) (reading A15), scattered like above.
 template <class L, typename T>
-__global__ void init_equilibrium_kernel(Geom g, const uint8_t *__restrict__ type,
-                                        const uint32_t *__restrict__ link, const T *__restrict__ rho0,
+__global__ void init_equilibrium_kernel(Geom g, const uint8_t *__restrict__ type, const T *__restrict__ rho0,
                                         const T *__restrict__ u0, T *__restrict__ store) {
     int x, y, z, n;
     if (!thread_node(g, x, y, z, n)) return;
-    const uint8_t t = type[n];
-    if (t == NODE_SOLID) return;
-    const uint32_t w = (t == NODE_BOUNDARY) ? link[n] : 0u;
+    if (type[n] == NODE_SOLID) return;
     const Nbr o = neighbours(g, x, y, z);
     const T rho = rho0[n];
     T v[3] = {T(0), T(0), T(0)};
@@ -163,43 +310,37 @@ __global__ void init_equilibrium_kernel(Geom g, const uint8_t *__restrict__ type
     T heq[L::Q];
     equilibrium_dev<L, T>(rho, rho - T(1), v, heq);
 #pragma unroll
-    for (int i = 0; i < L::Q; i++) store[source_slot<L>(i, n, g.N, o, w)] = heq[i];
+    for (int i = 0; i < L::Q; i++) store[(int64_t)i * g.N + (n + shift<L>(i, -1, o))] = heq[i];
 }
 
 template <class L, typename T>
-__global__ void get_distributions_kernel(Geom g, const uint8_t *__restrict__ type,
-                                         const uint32_t *__restrict__ link, const T *__restrict__ store,
+__global__ void get_distributions_kernel(Geom g, const uint8_t *__restrict__ type, const T *__restrict__ store,
                                          T *__restrict__ f) {
     int x, y, z, n;
     if (!thread_node(g, x, y, z, n)) return;
-    const uint8_t t = type[n];
-    if (t == NODE_SOLID) {
+    if (type[n] == NODE_SOLID) {
 #pragma unroll
         for (int i = 0; i < L::Q; i++) f[(int64_t)i * g.N + n] = T(0);
         return;
     }
-    const uint32_t w = (t == NODE_BOUNDARY) ? link[n] : 0u;
     const Nbr o = neighbours(g, x, y, z);
     T h[L::Q];
-    gather<L, T>(store, n, g.N, o, w, h);
+    gather<L, T>(store, n, g.N, o, h);
 #pragma unroll
     for (int i = 0; i < L::Q; i++) f[(int64_t)i * g.N + n] = h[i] + L::template w<T>(i);
 }
 
-// rho = sum f, v = (j + F/2)/rho (eq. 1, eq. 16).  half_g = g/2 (0 for SC2).
+// rho = sum f, v = (j + F/2)/rho (eq. 1, eq. 16).  hg = g/2 (0 for SC2).
 template <class L, typename T>
-__global__ void macro_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restrict__ link,
-                             const T *__restrict__ store, T *__restrict__ rho_out, T *__restrict__ u_out,
-                             T hgx, T hgy, T hgz) {
+__global__ void macro_kernel(Geom g, const uint8_t *__restrict__ type, const T *__restrict__ store,
+                             T *__restrict__ rho_out, T *__restrict__ u_out, T hgx, T hgy, T hgz) {
     int x, y, z, n;
     if (!thread_node(g, x, y, z, n)) return;
-    const uint8_t t = type[n];
     T rho = T(0), v[3] = {T(0), T(0), T(0)};
-    if (t != NODE_SOLID) {
-        const uint32_t w = (t == NODE_BOUNDARY) ? link[n] : 0u;
+    if (type[n] != NODE_SOLID) {
         const Nbr o = neighbours(g, x, y, z);
         T h[L::Q], drho, j[3];
-        gather<L, T>(store, n, g.N, o, w, h);
+        gather<L, T>(store, n, g.N, o, h);
         moments<L, T>(h, drho, j);
         rho = T(1) + drho;
         const T hg[3] = {hgx, hgy, hgz};
@@ -226,29 +367,44 @@ template <typename T, int PSI> __device__ __forceinline__ T psi_one() {
 }
 
 // Pass 1 (row a9): psi fields of both components from the time-t state.  SOLID: psi = 0 (A14).
-template <class L, typename T, int PSI>
+template <class L, typename T, int V, int PSI>
 __global__ void __launch_bounds__(256)
-sc_fields_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restrict__ link,
-                 const T *__restrict__ srcA, const T *__restrict__ srcB, T *__restrict__ psiA,
-                 T *__restrict__ psiB) {
-    int x, y, z, n;
-    if (!thread_node(g, x, y, z, n)) return;
-    const uint8_t t = type[n];
-    if (t == NODE_SOLID) { psiA[n] = -psi_one<T, PSI>(); psiB[n] = -psi_one<T, PSI>(); return; }
-    const uint32_t w = (t == NODE_BOUNDARY) ? link[n] : 0u;
-    const Nbr o = neighbours(g, x, y, z);
-    T sA = T(0), sB = T(0);
+sc_fields_kernel(Geom g, const uint8_t *__restrict__ type, const T *__restrict__ srcA,
+                 const T *__restrict__ srcB, T *__restrict__ psiA, T *__restrict__ psiB) {
+    Span s;
+    if (!thread_span<V>(g, s)) return;
+    const int n0 = s.row + s.x0;
+    const uint32_t types = load_types<V>(type, n0);
+    T pa[V], pb[V];
+    if (all_solid<V>(types)) {
 #pragma unroll
-    for (int i = 0; i < L::Q; i++) {
-        const int64_t s = source_slot<L>(i, n, g.N, o, w);
-        sA += __ldg(srcA + s);
-        sB += __ldg(srcB + s);
+        for (int k = 0; k < V; k++) pa[k] = pb[k] = -psi_one<T, PSI>();
+    } else {
+        T h[V][L::Q];
+        gather_span<L, T, V>(srcA, g.N, s, h);
+#pragma unroll
+        for (int k = 0; k < V; k++) {
+            T sum = h[k][0];
+#pragma unroll
+            for (int i = 1; i < L::Q; i++) sum += h[k][i];
+            pa[k] = psi_dev<T, PSI>(sum);
+        }
+        gather_span<L, T, V>(srcB, g.N, s, h);
+#pragma unroll
+        for (int k = 0; k < V; k++) {
+            T sum = h[k][0];
+#pragma unroll
+            for (int i = 1; i < L::Q; i++) sum += h[k][i];
+            pb[k] = psi_dev<T, PSI>(sum);
+            if (((types >> (8 * k)) & 0xffu) == NODE_SOLID) pa[k] = pb[k] = -psi_one<T, PSI>();
+        }
     }
-    psiA[n] = psi_dev<T, PSI>(sA);
-    psiB[n] = psi_dev<T, PSI>(sB);
+    // plain stores: pass 2 re-reads the fields right away (L2-resident)
+    Pack<T, V>::stp(psiA + n0, pa);
+    Pack<T, V>::stp(psiB + n0, pb);
 }
 
-// sum_i w_i psi(x + e_i) e_i over the neighbour field (18 L1/L2-served reads), in units of 1/36.
+// sum_i w_i psi(x + e_i) e_i over the neighbour field (18 L1/L2-served reads).
 template <class L, typename T>
 __device__ __forceinline__ void psi_gradient(const T *__restrict__ psi, int n, const Nbr &o, T (&S)[3]) {
     T ax[3] = {T(0), T(0), T(0)}, dg[3] = {T(0), T(0), T(0)};
@@ -269,46 +425,50 @@ __device__ __forceinline__ void psi_gradient(const T *__restrict__ psi, int n, c
 
 // Pass 2 (rows a10-a11): both components in one kernel: gather, moments, common velocity u'
 // (P:188), forces (eq. 10, sign A11) + body force, v_s = u' + F_s / (2 rho_s), LBGK + Guo (A13).
-template <class L, typename T, int PSI>
+template <class L, typename T, int V, int PSI>
 __global__ void __launch_bounds__(256)
 sc_step_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restrict__ link,
                const T *__restrict__ srcA, const T *__restrict__ srcB, T *__restrict__ dstA,
                T *__restrict__ dstB, const T *__restrict__ psiA, const T *__restrict__ psiB,
                Relax<T> rpA, Relax<T> rpB, T G) {
-    int x, y, z, n;
-    if (!thread_node(g, x, y, z, n)) return;
-    const uint8_t t = type[n];
-    if (t == NODE_SOLID) return;
-    const uint32_t w = (t == NODE_BOUNDARY) ? link[n] : 0u;
-    const Nbr o = neighbours(g, x, y, z);
-    T hA[L::Q], hB[L::Q];
-    gather<L, T>(srcA, n, g.N, o, w, hA);
-    gather<L, T>(srcB, n, g.N, o, w, hB);
-    T SA[3], SB[3];
-    psi_gradient<L, T>(psiA, n, o, SA);
-    psi_gradient<L, T>(psiB, n, o, SB);
-    T dA, dB, jA[3], jB[3];
-    moments<L, T>(hA, dA, jA);
-    moments<L, T>(hB, dB, jB);
-    const T rA = T(1) + dA, rB = T(1) + dB;
-    const T pA = psi_dev<T, PSI>(dA) + psi_one<T, PSI>(), pB = psi_dev<T, PSI>(dB) + psi_one<T, PSI>();
-    const T inv_den = T(1) / (rA * rpA.inv_tau + rB * rpB.inv_tau);
-    const T irA = T(0.5) / rA, irB = T(0.5) / rB;
-    T vA[3], vB[3], FA[3], FB[3];
+    Span s;
+    if (!thread_span<V>(g, s)) return;
+    const int n0 = s.row + s.x0;
+    const uint32_t types = load_types<V>(type, n0);
+    if (all_solid<V>(types)) return;
+    T hA[V][L::Q], hB[V][L::Q];
+    gather_span<L, T, V>(srcA, g.N, s, hA);
+    gather_span<L, T, V>(srcB, g.N, s, hB);
 #pragma unroll
-    for (int a = 0; a < 3; a++) {
-        const T up = (jA[a] * rpA.inv_tau + jB[a] * rpB.inv_tau) * inv_den;
-        FA[a] = -G * pA * SB[a] + rA * rpA.g[a];
-        FB[a] = -G * pB * SA[a] + rB * rpB.g[a];
-        vA[a] = up + FA[a] * irA;
-        vB[a] = up + FB[a] * irB;
+    for (int k = 0; k < V; k++) {
+        Nbr o = s.o;
+        const int x = s.x0 + k;
+        o.xm = (x == 0) ? (g.nx - 1) : -1;
+        o.xp = (x == g.nx - 1) ? -(g.nx - 1) : 1;
+        T SA[3], SB[3];
+        psi_gradient<L, T>(psiA, n0 + k, o, SA);
+        psi_gradient<L, T>(psiB, n0 + k, o, SB);
+        T dA, dB, jA[3], jB[3];
+        moments<L, T>(hA[k], dA, jA);
+        moments<L, T>(hB[k], dB, jB);
+        const T rA = T(1) + dA, rB = T(1) + dB;
+        const T pA = psi_dev<T, PSI>(dA) + psi_one<T, PSI>(), pB = psi_dev<T, PSI>(dB) + psi_one<T, PSI>();
+        const T inv_den = T(1) / (rA * rpA.inv_tau + rB * rpB.inv_tau);
+        const T irA = T(0.5) / rA, irB = T(0.5) / rB;
+        T vA[3], vB[3], FA[3], FB[3];
+#pragma unroll
+        for (int a = 0; a < 3; a++) {
+            const T up = (jA[a] * rpA.inv_tau + jB[a] * rpB.inv_tau) * inv_den;
+            FA[a] = -G * pA * SB[a] + rA * rpA.g[a];
+            FB[a] = -G * pB * SA[a] + rB * rpB.g[a];
+            vA[a] = up + FA[a] * irA;
+            vB[a] = up + FB[a] * irB;
+        }
+        collide<L, T, false, true>(hA[k], rA, dA, vA, FA, rpA);
+        collide<L, T, false, true>(hB[k], rB, dB, vB, FB, rpB);
     }
-    collide<L, T, false, true>(hA, rA, dA, vA, FA, rpA);
-#pragma unroll
-    for (int i = 0; i < L::Q; i++) __stcs(dstA + (int64_t)i * g.N + n, hA[i]);
-    collide<L, T, false, true>(hB, rB, dB, vB, FB, rpB);
-#pragma unroll
-    for (int i = 0; i < L::Q; i++) __stcs(dstB + (int64_t)i * g.N + n, hB[i]);
+    store_span<L, T, V>(dstA, g, s, types, link, hA);
+    store_span<L, T, V>(dstB, g, s, types, link, hB);
 }
 
 }  // namespace lbm

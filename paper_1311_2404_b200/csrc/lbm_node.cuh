@@ -177,19 +177,40 @@ template <typename T> struct Mrt<D2Q9, T> {
 template <class L, typename T, bool MRT, bool FORCE>
 LBM_HD void collide(T (&h)[L::Q], T rho, T drho, const T (&v)[3], const T (&F)[3], const Relax<T> &rp) {
     constexpr int Q = L::Q;
-    T heq[Q];
-    equilibrium_dev<L, T>(rho, drho, v, heq);
     if constexpr (!MRT) {
-        if constexpr (FORCE) {
-            T src[Q];
-            guo_bracket<L, T>(v, F, src);
+        // LBGK (Alg. 1 l.13) + eq. (17), evaluated per +/- pair of directions: with e_ibar = -e_i
+        // the equilibrium and the source split into a part even in e_i (shared by the pair) and a
+        // part odd in e_i (opposite signs), which halves the arithmetic per node.
+        const T om = rp.inv_tau, keep = T(1) - rp.inv_tau, sc = rp.src_scale;
+        const T base = drho - rho * (T(1.5) * (v[0] * v[0] + v[1] * v[1] + v[2] * v[2]));
+        const T r45 = T(4.5) * rho, r3 = T(3) * rho;
+        const T vF3 = FORCE ? T(3) * (v[0] * F[0] + v[1] * F[1] + v[2] * F[2]) : T(0);
+        {
+            T a = om * L::template w<T>(0) * base;
+            if constexpr (FORCE) a -= sc * L::template w<T>(0) * vF3;
+            h[0] = keep * h[0] + a;
+        }
 #pragma unroll
-            for (int i = 0; i < Q; i++) h[i] = h[i] + (heq[i] - h[i]) * rp.inv_tau + rp.src_scale * src[i];
-        } else {
-#pragma unroll
-            for (int i = 0; i < Q; i++) h[i] = h[i] + (heq[i] - h[i]) * rp.inv_tau;
+        for (int i = 1; i < Q; i++) {
+            if (i < L::opp(i)) {
+                const int j = L::opp(i);
+                const T wo = om * L::template w<T>(i);
+                const T ev = e_dot<L, T>(i, v);
+                T even = wo * (base + r45 * ev * ev);
+                T odd = wo * (r3 * ev);
+                if constexpr (FORCE) {
+                    const T ws = sc * L::template w<T>(i);
+                    const T eF = e_dot<L, T>(i, F);
+                    even += ws * (T(9) * ev * eF - vF3);
+                    odd += ws * (T(3) * eF);
+                }
+                h[i] = keep * h[i] + (even + odd);
+                h[j] = keep * h[j] + (even - odd);
+            }
         }
     } else {
+        T heq[Q];
+        equilibrium_dev<L, T>(rho, drho, v, heq);
         T d[Q], m[Q];
 #pragma unroll
         for (int i = 0; i < Q; i++) d[i] = heq[i] - h[i];
