@@ -89,7 +89,9 @@ int lbm_init_equilibrium(lbm_ctx *ctx, int comp, const void *d_rho, const void *
 /* Advance n >= 0 time steps; each step is one fused pull-stream + moments + equilibrium +
  * collision (+ Guo source) + store pass over the lattice (Alg. 1; eqs. 1-4, 16-17);
  * LBM_SC2 runs the macro-field pass and then the coupled collide pass (eq. 10).
- * LBM_ESTATE if a component has not been initialised. */
+ * LBM_ESTATE if a component has not been initialised.  Asynchronous, except that the first call
+ * after lbm_set_geometry synchronises the stream once (it reads back how many nodes are not
+ * bulk fluid to pick the kernel variant). */
 int lbm_step(lbm_ctx *ctx, int n);
 
 /* rho = sum_i f_i, velocity v of eq. (16) (includes g/2) from the current state.

@@ -19,7 +19,7 @@ constexpr size_t ALIGN = 256;
 inline size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
 
 struct Layout {
-    size_t store[2][2], type, link, psi[2], stage_mask, stage_rho, stage_u, total;
+    size_t store[2][2], type, link, counters, psi[2], stage_mask, stage_rho, stage_u, total;
 };
 
 struct Vtbl;
@@ -37,6 +37,7 @@ struct lbm_ctx {
     int cur;  // which of the two buffers holds the current state (AB)
     bool inited[2];
     bool geometry_frozen;
+    bool vec_pending;   // geometry changed: re-pick `vec` from the non-bulk node count at the next step
     int64_t steps, launches;
     int block_x;        // one-node-per-thread kernels: 1-D block along x
     int vec;            // nodes per thread of the step kernels (1, 2 or 4 consecutive x)
@@ -110,6 +111,7 @@ void make_layout(const lbm_params *p, int Q, int D, Layout *L) {
         for (int b = 0; b < 2; b++) { L->store[s][b] = off; off += align_up(Q * N * rs); }
     L->type = off; off += align_up(N);
     L->link = off; off += align_up(4 * N);
+    L->counters = off; off += ALIGN;
     if (nc == 2)
         for (int s = 0; s < 2; s++) { L->psi[s] = off; off += align_up(N * rs); }
     L->stage_mask = off; off += align_up(N);
@@ -155,7 +157,10 @@ template <class L, typename T> struct Impl {
     static uint32_t *link(lbm_ctx *c) { return at<uint32_t>(c, c->lay.link); }
 
     static int set_geometry(lbm_ctx *c, const uint8_t *d_mask) {
-        build_links_kernel<L><<<grid_of(c), c->block_x, 0, c->stream>>>(c->g, d_mask, type(c), link(c));
+        unsigned *cnt = at<unsigned>(c, c->lay.counters);
+        if (cudaMemsetAsync(cnt, 0, sizeof(unsigned), c->stream) != cudaSuccess) return fail(c, LBM_ECUDA, "cudaMemsetAsync(counters)");
+        build_links_kernel<L><<<grid_of(c), c->block_x, 0, c->stream>>>(c->g, d_mask, type(c), link(c), cnt);
+        c->vec_pending = true;
         return check_launch(c, "build_links_kernel");
     }
 
@@ -265,10 +270,14 @@ int env_int(const char *name, int dflt, int lo, int hi) {
     return dflt;
 }
 
-// Nodes per thread: the widest pack (16 bytes) that divides nx; LBM_VEC overrides downwards.
-int pick_vec(const lbm_params *p) {
+// Nodes per thread of the step kernels, by measurement (profiles/): fp32 single-component runs
+// fastest with 4-node packs (16-byte accesses) unless many packs contain SOLID or BOUNDARY nodes
+// (their stores fall back to scalars); fp64 and the two-component kernel are register-bound and
+// run fastest with one node per thread.  LBM_VEC overrides (tuning knob, not part of the ABI).
+int pick_vec(const lbm_params *p, double nonbulk_fraction) {
     const int widest = p->precision == LBM_F32 ? 4 : 2;
-    int v = env_int("LBM_VEC", widest, 1, widest);
+    int v = (p->precision == LBM_F32 && p->model != LBM_SC2 && nonbulk_fraction < 0.2) ? 4 : 1;
+    v = env_int("LBM_VEC", v, 1, widest);
     if (v == 3) v = 2;
     while (v > 1 && p->nx % v) v /= 2;
     return v;
@@ -338,8 +347,9 @@ LBM_API int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, voi
     c->ws = static_cast<char *>(d_workspace);
     c->lay = lay;
     c->block_x = pick_block_x(p->nx);
-    c->vec = pick_vec(p);
-    c->block_threads = env_int("LBM_BLOCK_THREADS", 128, 32, 256);
+    c->vec = pick_vec(p, 0.0);
+    c->vec_pending = false;
+    c->block_threads = env_int("LBM_BLOCK_THREADS", 64, 32, 256);
     c->vt = select_impl(p);
     c->err[0] = 0;
     // geometry starts all-FLUID: type = BULK, link = 0
@@ -408,6 +418,14 @@ LBM_API int lbm_step(lbm_ctx *c, int n) {
     CHECK_CTX(c);
     if (n < 0) return fail(c, LBM_EINVAL, "n < 0");
     if (int rc = check_state(c)) return rc;
+    if (c->vec_pending && n > 0) {  // once per geometry: how many nodes are not BULK decides the pack width
+        unsigned nonbulk = 0;
+        cudaError_t e = cudaMemcpyAsync(&nonbulk, c->ws + c->lay.counters, sizeof nonbulk, cudaMemcpyDeviceToHost, c->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+        if (e != cudaSuccess) return fail(c, LBM_ECUDA, "reading the geometry counter: %s", cudaGetErrorString(e));
+        c->vec = pick_vec(&c->p, (double)nonbulk / (double)c->g.N);
+        c->vec_pending = false;
+    }
     return c->vt->step(c, n);
 }
 

@@ -91,17 +91,24 @@ __device__ __forceinline__ bool thread_node(const Geom &g, int &x, int &y, int &
 // ---- link encoding from the node-type mask (lbm_set_geometry) -------------------------------
 template <class L>
 __global__ void build_links_kernel(Geom g, const uint8_t *__restrict__ mask, uint8_t *__restrict__ type,
-                                   uint32_t *__restrict__ link) {
+                                   uint32_t *__restrict__ link, unsigned *__restrict__ nonbulk_count) {
     int x, y, z, n;
     if (!thread_node(g, x, y, z, n)) return;
-    if (mask[n]) { type[n] = NODE_SOLID; link[n] = LINK_SELF_SOLID; return; }
-    const Nbr o = neighbours(g, x, y, z);
-    uint32_t w = 0;
+    uint32_t w = LINK_SELF_SOLID;
+    uint8_t t = NODE_SOLID;
+    if (!mask[n]) {
+        const Nbr o = neighbours(g, x, y, z);
+        w = 0;
 #pragma unroll
-    for (int i = 1; i < L::Q; i++)
-        if (mask[n + shift<L>(i, -1, o)]) w |= 1u << i;
+        for (int i = 1; i < L::Q; i++)
+            if (mask[n + shift<L>(i, -1, o)]) w |= 1u << i;
+        t = w ? NODE_BOUNDARY : NODE_BULK;
+    }
     link[n] = w;
-    type[n] = w ? NODE_BOUNDARY : NODE_BULK;
+    type[n] = t;
+    // warp-aggregated count of nodes that are not BULK (picks the pack width of the step kernels)
+    const unsigned active = __activemask(), votes = __ballot_sync(active, t != NODE_BULK);
+    if (votes && (threadIdx.x & 31) == __ffs(active) - 1) atomicAdd(nonbulk_count, __popc(votes));
 }
 
 __global__ void get_geometry_kernel(Geom g, const uint8_t *__restrict__ type, uint8_t *__restrict__ mask) {
