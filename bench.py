@@ -106,6 +106,22 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def max_over_ranks(value: float, world: int, device) -> float:
+    """Slowest rank's time (the contract's max over ranks); identity for one rank."""
+    if world <= 1:
+        return float(value)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_mlups(sites: int, steps: int, world: int, seconds: float) -> float:
+    """Whole-job throughput of `world` independent replicas (replicas only)."""
+    return sites * steps * world / seconds / 1e6
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md)."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
@@ -181,10 +197,7 @@ def run_ours(args):
     clk = clocks.stop()
     launches = (sim.counters()[1] - l0) // args.repeats
     ms = float(np.median(reps))
-    t = torch.tensor([ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms = float(t.item())
+    ms = max_over_ranks(ms, world, dev)
     rho, _ = sim.macro()
     assert bool(torch.isfinite(rho).all()), "state went non-finite during the timed steps"
 
@@ -201,10 +214,7 @@ def run_ours(args):
     sim.run_host(h_mask, h_rho, h_u, K, o_rho, o_u)  # synchronises the stream before returning
     e2e_s = time.perf_counter() - t0
     barrier()
-    t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e_s = float(t.item())
+    e2e_s = max_over_ranks(e2e_s, world, dev)
     h2d = h_mask.numel() + sum(x.numel() * x.element_size() for x in h_rho + h_u)
     d2h = o_rho.numel() * o_rho.element_size() + o_u.numel() * o_u.element_size()
     assert bool(torch.isfinite(o_rho).all())
@@ -217,7 +227,7 @@ def run_ours(args):
         cb = None
         if world == 1 and not args.no_cpu_baseline:
             cb, _, _ = time_oracle(args.config, args.cpu_steps, 1)
-        line = {"metric": METRIC, "value": w.sites * K * world / (ms * 1e-3) / 1e6, "unit": UNIT,
+        line = {"metric": METRIC, "value": aggregate_mlups(w.sites, K, world, ms * 1e-3), "unit": UNIT,
                 "n_gpus": world, "steps": K, "warmup": Wm, "ms_per_step": ms / K, "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "f32" if w.precision == W.F32 else "f64",
                 "data": "synthetic",
@@ -226,7 +236,7 @@ def run_ours(args):
                     "timing": "median of %d repeats of K steps, CUDA events on the ctx stream" % args.repeats,
                     "repeats_ms": reps}),
                 "clocks": clk,
-                "e2e": {"value": w.sites * K * world / e2e_s / 1e6, "unit": UNIT,
+                "e2e": {"value": aggregate_mlups(w.sites, K, world, e2e_s), "unit": UNIT,
                         "h2d_bytes_per_step": h2d / K, "d2h_bytes_per_step": d2h / K,
                         "note": "one lbm_run_host call = H2D(mask, rho0, u0) + init + K steps + macro + D2H(rho, u); bytes amortised over K"},
                 "gpu_launches": int(launches),
