@@ -39,6 +39,7 @@ struct lbm_ctx {
     bool geometry_frozen;
     bool vec_pending;   // geometry changed: re-pick `vec` from the non-bulk node count at the next step
     int64_t steps, launches;
+    bool idx32;         // Q * N < 2^32: slot numbers fit 32 bits (cheaper address arithmetic)
     int block_x;        // one-node-per-thread kernels: 1-D block along x
     int vec;            // nodes per thread of the step kernels (1, 2 or 4 consecutive x)
     int block_threads;  // threads per block of the step kernels
@@ -166,25 +167,25 @@ template <class L, typename T> struct Impl {
 
     static int init_equilibrium(lbm_ctx *c, int s, const void *rho, const void *u) {
         init_equilibrium_kernel<L, T><<<grid_of(c), c->block_x, 0, c->stream>>>(
-            c->g, type(c), (const T *)rho, (const T *)u, at<T>(c, c->lay.store[s][c->cur]));
+            c->g, type(c), link(c), (const T *)rho, (const T *)u, at<T>(c, c->lay.store[s][c->cur]));
         return check_launch(c, "init_equilibrium_kernel");
     }
 
     static int set_distributions(lbm_ctx *c, int s, const void *f) {
         set_distributions_kernel<L, T><<<grid_of(c), c->block_x, 0, c->stream>>>(
-            c->g, type(c), (const T *)f, at<T>(c, c->lay.store[s][c->cur]));
+            c->g, type(c), link(c), (const T *)f, at<T>(c, c->lay.store[s][c->cur]));
         return check_launch(c, "set_distributions_kernel");
     }
 
     static int get_distributions(lbm_ctx *c, int s, void *f) {
-        get_distributions_kernel<L, T><<<grid_of(c), c->block_x, 0, c->stream>>>(c->g, type(c), src(c, s), (T *)f);
+        get_distributions_kernel<L, T><<<grid_of(c), c->block_x, 0, c->stream>>>(c->g, type(c), link(c), src(c, s), (T *)f);
         return check_launch(c, "get_distributions_kernel");
     }
 
     static int macro(lbm_ctx *c, int s, void *rho, void *u) {
         const bool sc = c->p.model == LBM_SC2;  // SC2: bare component velocity (lbm.h)
         macro_kernel<L, T><<<grid_of(c), c->block_x, 0, c->stream>>>(
-            c->g, type(c), src(c, s), (T *)rho, (T *)u, sc ? T(0) : T(0.5 * c->p.force[0]),
+            c->g, type(c), link(c), src(c, s), (T *)rho, (T *)u, sc ? T(0) : T(0.5 * c->p.force[0]),
             sc ? T(0) : T(0.5 * c->p.force[1]), sc ? T(0) : T(0.5 * c->p.force[2]));
         return check_launch(c, "macro_kernel");
     }
@@ -195,9 +196,13 @@ template <class L, typename T> struct Impl {
     }
 
     template <int V, bool MRT, bool FORCE> static int step_single_v(lbm_ctx *c, int n, const Relax<T> &rp) {
+        return c->idx32 ? step_single_vi<V, uint32_t, MRT, FORCE>(c, n, rp) : step_single_vi<V, int64_t, MRT, FORCE>(c, n, rp);
+    }
+
+    template <int V, typename I, bool MRT, bool FORCE> static int step_single_vi(lbm_ctx *c, int n, const Relax<T> &rp) {
         const Launch l = span_launch(c, V);
         for (int t = 0; t < n; t++) {
-            step_kernel<L, T, V, MRT, FORCE><<<l.grid, l.block, 0, c->stream>>>(c->g, type(c), link(c), src(c, 0), dst(c, 0), rp);
+            step_kernel<L, T, V, I, MRT, FORCE><<<l.grid, l.block, 0, c->stream>>>(c->g, type(c), link(c), src(c, 0), dst(c, 0), rp);
             if (int rc = check_launch(c, "step_kernel")) return rc;
             c->cur ^= 1;
             c->steps++;
@@ -214,13 +219,17 @@ template <class L, typename T> struct Impl {
     }
 
     template <int V, int PSI> static int step_sc_v(lbm_ctx *c, int n) {
+        return c->idx32 ? step_sc_vi<V, uint32_t, PSI>(c, n) : step_sc_vi<V, int64_t, PSI>(c, n);
+    }
+
+    template <int V, typename I, int PSI> static int step_sc_vi(lbm_ctx *c, int n) {
         const Launch l = span_launch(c, V);
         const Relax<T> rA = make_relax<T>(c, 0), rB = make_relax<T>(c, 1);
         T *pA = at<T>(c, c->lay.psi[0]), *pB = at<T>(c, c->lay.psi[1]);
         for (int t = 0; t < n; t++) {
-            sc_fields_kernel<L, T, V, PSI><<<l.grid, l.block, 0, c->stream>>>(c->g, type(c), src(c, 0), src(c, 1), pA, pB);
+            sc_fields_kernel<L, T, V, I, PSI><<<l.grid, l.block, 0, c->stream>>>(c->g, type(c), link(c), src(c, 0), src(c, 1), pA, pB);
             if (int rc = check_launch(c, "sc_fields_kernel")) return rc;
-            sc_step_kernel<L, T, V, PSI><<<l.grid, l.block, 0, c->stream>>>(
+            sc_step_kernel<L, T, V, I, PSI><<<l.grid, l.block, 0, c->stream>>>(
                 c->g, type(c), link(c), src(c, 0), src(c, 1), dst(c, 0), dst(c, 1), pA, pB, rA, rB, T(c->p.sc_G));
             if (int rc = check_launch(c, "sc_step_kernel")) return rc;
             c->cur ^= 1;
@@ -270,13 +279,16 @@ int env_int(const char *name, int dflt, int lo, int hi) {
     return dflt;
 }
 
-// Nodes per thread of the step kernels, by measurement (profiles/): fp32 single-component runs
-// fastest with 4-node packs (16-byte accesses) unless many packs contain SOLID or BOUNDARY nodes
-// (their stores fall back to scalars); fp64 and the two-component kernel are register-bound and
-// run fastest with one node per thread.  LBM_VEC overrides (tuning knob, not part of the ABI).
+// Nodes per thread of the step kernels, by measurement (profiles/):
+//   fp32 single component: 4-node packs (16-byte accesses) on mostly-bulk geometries (c2: 44.1 vs
+//   39.7 GLUPS at V = 1); 2-node packs when many nodes are BOUNDARY, where the reflected-link
+//   fix-up of 4 nodes costs too many registers (c3: V = 2 34.8, V = 4 29.5, V = 1 26.1 GLUPS);
+//   fp64: 2-node packs (c4: 22.4 vs 22.1); two-component kernel: register-bound, 1 node (c5: 12.0 vs 9.9).
+// LBM_VEC overrides (tuning knob, not part of the ABI).  Falls back to what divides nx.
 int pick_vec(const lbm_params *p, double nonbulk_fraction) {
     const int widest = p->precision == LBM_F32 ? 4 : 2;
-    int v = (p->precision == LBM_F32 && p->model != LBM_SC2 && nonbulk_fraction < 0.2) ? 4 : 1;
+    int v = 1;
+    if (p->model != LBM_SC2) v = p->precision == LBM_F64 ? 2 : (nonbulk_fraction < 0.2 ? 4 : 2);
     v = env_int("LBM_VEC", v, 1, widest);
     if (v == 3) v = 2;
     while (v > 1 && p->nx % v) v /= 2;
@@ -348,6 +360,7 @@ LBM_API int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, voi
     c->lay = lay;
     c->block_x = pick_block_x(p->nx);
     c->vec = pick_vec(p, 0.0);
+    c->idx32 = (double)Q * (double)c->g.N < 4294967296.0 && !env_int("LBM_IDX64", 0, 0, 1);
     c->vec_pending = false;
     c->block_threads = env_int("LBM_BLOCK_THREADS", 64, 32, 256);
     c->vt = select_impl(p);

@@ -2,12 +2,14 @@
 //
 // Store: structure of arrays real[Q][N], x fastest, holding
 // the DEVIATION h = f - w (reading A12) of the POST-collision populations (reading A9).
-//   * load side: f_i(x, t+1) is ALWAYS pulled from slot (i, x - e_i); no per-link selects.
-//   * store side: a node writes its post-collision h*_i(x) to (i, x) with aligned vector stores;
-//     for every link whose pull source x - e_i is SOLID (half-way bounce-back, reading
-//     A8) it also writes h*_ibar(x) into the otherwise unused slot (i, x - e_i) of that SOLID
-//     node, which is exactly what the pull of the next step must return.  SOLID nodes write
-//     nothing, so each slot has one writer and is read once and written once per step.
+//   * f_i(x, t+1) is pulled from slot (i, x - e_i) with aligned vector loads for every node;
+//     BOUNDARY nodes (>= 1 SOLID pull source) then replace each reflected population by their own
+//     h*_ibar(x) from slot (ibar, x) (half-way bounce-back, reading A8).  Only packs that
+//     contain a BOUNDARY node execute that fix-up.
+//   * a node writes its post-collision h*_i(x) to (i, x) of the other buffer with aligned vector
+//     stores.  Slots of SOLID nodes are never read (every pull from them is reflected), so packs
+//     that mix FLUID and SOLID nodes still store whole vectors.  Every FLUID slot is read once and
+//     written once per step: DRAM traffic is the algorithmic 2 Q sizeof(real) + mask bytes.
 #pragma once
 #include <cuda_runtime.h>
 #include "lbm_node.cuh"
@@ -59,24 +61,31 @@ template <class L> __device__ __forceinline__ int shift_yz(int i, int s, const N
     return d;
 }
 
-// THE streaming rule (reading A8), used by the step kernels' store side and by
-// lbm_get_stream_map alike: is population i of a node with link word `link` reflected?
+// THE streaming rule (reading A8), shared by the step kernels, the conversion kernels and
+// lbm_get_stream_map: population i of a node with link word `link` is reflected iff bit i is set;
+// then it comes from the node's own slot (ibar, x) instead of (i, x - e_i).
 __device__ __forceinline__ bool reflected(uint32_t link, int i) { return (link >> i) & 1u; }
 
-// Store-side half of the rule: after writing h*(x), feed every reflected link.
-template <class L, typename T>
-__device__ __forceinline__ void feed_reflected_links(T *__restrict__ dst, int n, int64_t N, const Nbr &o,
-                                                     uint32_t link, const T (&h)[L::Q]) {
-#pragma unroll
-    for (int i = 1; i < L::Q; i++)
-        if (reflected(link, i)) dst[(int64_t)i * N + (n + shift<L>(i, -1, o))] = h[L::opp(i)];
+// I = index type of slot numbers i * N + node: uint32_t when Q * N < 2^32 (one IMAD.WIDE per access
+// instead of a 64-bit add chain; the step kernels were issue-bound on address arithmetic), else int64_t.
+template <class L, typename I>
+__device__ __forceinline__ I source_slot(int i, int n, int64_t N, const Nbr &o, uint32_t link) {
+    return reflected(link, i) ? I(L::opp(i)) * I(N) + I(n) : I(i) * I(N) + I(n + shift<L>(i, -1, o));
 }
 
-// Load-side half: plain pull.
-template <class L, typename T>
-__device__ __forceinline__ void gather(const T *__restrict__ src, int n, int64_t N, const Nbr &o, T (&h)[L::Q]) {
+// Replace the reflected populations of one BOUNDARY node (after the plain pull).
+template <class L, typename T, typename I>
+__device__ __forceinline__ void pull_reflected(const T *__restrict__ src, int n, int64_t N, uint32_t link, T (&h)[L::Q]) {
 #pragma unroll
-    for (int i = 0; i < L::Q; i++) h[i] = __ldg(src + ((int64_t)i * N + (n + shift<L>(i, -1, o))));
+    for (int i = 1; i < L::Q; i++)
+        if (reflected(link, i)) h[i] = __ldg(src + (I(L::opp(i)) * I(N) + I(n)));
+}
+
+// One node, scalar (conversion kernels).
+template <class L, typename T>
+__device__ __forceinline__ void gather(const T *__restrict__ src, int n, int64_t N, const Nbr &o, uint32_t link, T (&h)[L::Q]) {
+#pragma unroll
+    for (int i = 0; i < L::Q; i++) h[i] = __ldg(src + source_slot<L, int64_t>(i, n, N, o, link));
 }
 
 // Thread -> node for the one-node-per-thread kernels: 1-D blocks along x.
@@ -127,8 +136,7 @@ __global__ void stream_map_kernel(Geom g, const uint8_t *__restrict__ type, cons
     const uint32_t w = (t == NODE_BOUNDARY) ? link[n] : 0u;
 #pragma unroll
     for (int i = 0; i < L::Q; i++) {
-        int64_t s = reflected(w, i) ? (int64_t)L::opp(i) * g.N + n : (int64_t)i * g.N + (n + shift<L>(i, -1, o));
-        map[(int64_t)i * g.N + n] = (t == NODE_SOLID) ? int64_t(-1) : s;
+        map[(int64_t)i * g.N + n] = (t == NODE_SOLID) ? int64_t(-1) : source_slot<L, int64_t>(i, n, g.N, o, w);
     }
 }
 
@@ -196,29 +204,30 @@ template <int V> __device__ __forceinline__ bool thread_span(const Geom &g, Span
 // Pull for V nodes (row a2): e_x = 0 planes with one aligned vector load; e_x = +-1 planes with
 // the aligned vector of the source row plus ONE scalar for the element that falls outside the
 // pack (an L1 hit: the neighbouring thread's vector load brings the same sector).
-template <class L, typename T, int V>
+template <class L, typename T, int V, typename I>
 __device__ __forceinline__ void gather_span(const T *__restrict__ src, int64_t N, const Span &s, T (&h)[V][L::Q]) {
 #pragma unroll
     for (int i = 0; i < L::Q; i++) {
-        const T *row = src + ((int64_t)i * N + (s.row + shift_yz<L>(i, -1, s.o)));
+        const int r = s.row + shift_yz<L>(i, -1, s.o);  // node index of x = 0 in the source row
+        const I plane = I(i) * I(N);
         if (L::ex(i) == 0) {
             T a[V];
-            Pack<T, V>::ld(row + s.x0, a);
+            Pack<T, V>::ld(src + (plane + I(r + s.x0)), a);
 #pragma unroll
             for (int k = 0; k < V; k++) h[k][i] = a[k];
         } else if (L::ex(i) == 1) {  // source x - 1
-            h[0][i] = __ldg(row + s.xm);
+            h[0][i] = __ldg(src + (plane + I(r + s.xm)));
             if (V > 1) {
                 T a[V];
-                Pack<T, V>::ld(row + s.x0, a);
+                Pack<T, V>::ld(src + (plane + I(r + s.x0)), a);
 #pragma unroll
                 for (int k = 1; k < V; k++) h[k][i] = a[k - 1];
             }
         } else {  // source x + 1
-            h[V - 1][i] = __ldg(row + s.xp);
+            h[V - 1][i] = __ldg(src + (plane + I(r + s.xp)));
             if (V > 1) {
                 T a[V];
-                Pack<T, V>::ld(row + s.x0, a);
+                Pack<T, V>::ld(src + (plane + I(r + s.x0)), a);
 #pragma unroll
                 for (int k = 0; k < V - 1; k++) h[k][i] = a[k + 1];
             }
@@ -236,43 +245,33 @@ template <int V> __device__ __forceinline__ bool all_solid(uint32_t t) {
     return t == (V == 4 ? 0x01010101u : V == 2 ? 0x0101u : 0x01u);
 }
 
-// Store for V nodes (row a8) + the reflected links of BOUNDARY nodes.
-template <class L, typename T, int V>
-__device__ __forceinline__ void store_span(T *__restrict__ dst, const Geom &g, const Span &s, uint32_t types,
-                                           const uint32_t *__restrict__ link, const T (&h)[V][L::Q]) {
-    const int n0 = s.row + s.x0;
-    if ((types & 0x01010101u) == 0) {  // no SOLID node in the pack: aligned vector stores
-#pragma unroll
-        for (int i = 0; i < L::Q; i++) {
-            T a[V];
-#pragma unroll
-            for (int k = 0; k < V; k++) a[k] = h[k][i];
-            Pack<T, V>::st(dst + ((int64_t)i * g.N + n0), a);
-        }
-    } else {  // SOLID slots belong to their neighbours' reflected links: do not touch them
-#pragma unroll
-        for (int k = 0; k < V; k++)
-            if (((types >> (8 * k)) & 0xffu) != NODE_SOLID) {
-#pragma unroll
-                for (int i = 0; i < L::Q; i++) dst[(int64_t)i * g.N + (n0 + k)] = h[k][i];
-            }
-    }
+// Fix-up of the pack's BOUNDARY nodes (row a2, reflected links).
+template <class L, typename T, int V, typename I>
+__device__ __forceinline__ void pull_reflected_span(const T *__restrict__ src, int64_t N, int n0, uint32_t types,
+                                                    const uint32_t *__restrict__ link, T (&h)[V][L::Q]) {
     if (types & 0x02020202u) {
 #pragma unroll
         for (int k = 0; k < V; k++)
-            if (((types >> (8 * k)) & 0xffu) == NODE_BOUNDARY) {
-                Nbr o = s.o;
-                const int x = s.x0 + k;
-                o.xm = (x == 0) ? (g.nx - 1) : -1;
-                o.xp = (x == g.nx - 1) ? -(g.nx - 1) : 1;
-                feed_reflected_links<L, T>(dst, n0 + k, g.N, o, __ldg(link + n0 + k), h[k]);
-            }
+            if (((types >> (8 * k)) & 0xffu) == NODE_BOUNDARY)
+                pull_reflected<L, T, I>(src, n0 + k, N, __ldg(link + n0 + k), h[k]);
+    }
+}
+
+// Store for V nodes (row a8): aligned vector, streaming.
+template <class L, typename T, int V, typename I>
+__device__ __forceinline__ void store_span(T *__restrict__ dst, int64_t N, int n0, const T (&h)[V][L::Q]) {
+#pragma unroll
+    for (int i = 0; i < L::Q; i++) {
+        T a[V];
+#pragma unroll
+        for (int k = 0; k < V; k++) a[k] = h[k][i];
+        Pack<T, V>::st(dst + (I(i) * I(N) + I(n0)), a);
     }
 }
 
 // ---- the fused step: pull-stream + moments + equilibrium + collision (+ Guo) + store ---------
 // Rows a1-a8 of DESIGN.md.  All loads of the pack are issued before first use (bytes in flight).
-template <class L, typename T, int V, bool MRT, bool FORCE>
+template <class L, typename T, int V, typename I, bool MRT, bool FORCE>
 __global__ void __launch_bounds__(256)
 step_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restrict__ link,
             const T *__restrict__ src, T *__restrict__ dst, Relax<T> rp) {
@@ -281,34 +280,39 @@ step_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restrict
     const uint32_t types = load_types<V>(type, s.row + s.x0);
     if (all_solid<V>(types)) return;
     T h[V][L::Q];
-    gather_span<L, T, V>(src, g.N, s, h);
+    gather_span<L, T, V, I>(src, g.N, s, h);
+    pull_reflected_span<L, T, V, I>(src, g.N, s.row + s.x0, types, link, h);
 #pragma unroll
     for (int k = 0; k < V; k++) update_node<L, T, MRT, FORCE>(h[k], rp);
-    store_span<L, T, V>(dst, g, s, types, link, h);
+    store_span<L, T, V, I>(dst, g.N, s.row + s.x0, h);
 }
 
 // ---- canonical <-> internal conversions (off the hot loop; reading A9) ----------------------
-// canonical f_i(x,t) -> store: S[(i, x - e_i)] = f_i(x) - w_i, the inverse of the pull.  Slot
-// (i, y) is written by x = y + e_i only, so every slot a FLUID node will pull is written once.
+// canonical f_i(x,t) -> store: S[source_slot(i, x)] = f_i(x) - w_i, the inverse of the pull.  The
+// pull is a permutation of FLUID slots (A8), so every FLUID slot is written exactly once.
 template <class L, typename T>
-__global__ void set_distributions_kernel(Geom g, const uint8_t *__restrict__ type, const T *__restrict__ f,
-                                         T *__restrict__ store) {
+__global__ void set_distributions_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restrict__ link,
+                                         const T *__restrict__ f, T *__restrict__ store) {
     int x, y, z, n;
     if (!thread_node(g, x, y, z, n)) return;
-    if (type[n] == NODE_SOLID) return;
+    const uint8_t t = type[n];
+    if (t == NODE_SOLID) return;
+    const uint32_t w = (t == NODE_BOUNDARY) ? link[n] : 0u;
     const Nbr o = neighbours(g, x, y, z);
 #pragma unroll
     for (int i = 0; i < L::Q; i++)
-        store[(int64_t)i * g.N + (n + shift<L>(i, -1, o))] = f[(int64_t)i * g.N + n] - L::template w<T>(i);
+        store[source_slot<L, int64_t>(i, n, g.N, o, w)] = f[(int64_t)i * g.N + n] - L::template w<T>(i);
 }
 
 // f_i(x,0) = f_i^eq(rho0, u0), eq. (3) (reading A15), scattered like above.
 template <class L, typename T>
-__global__ void init_equilibrium_kernel(Geom g, const uint8_t *__restrict__ type, const T *__restrict__ rho0,
-                                        const T *__restrict__ u0, T *__restrict__ store) {
+__global__ void init_equilibrium_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restrict__ link,
+                                        const T *__restrict__ rho0, const T *__restrict__ u0, T *__restrict__ store) {
     int x, y, z, n;
     if (!thread_node(g, x, y, z, n)) return;
-    if (type[n] == NODE_SOLID) return;
+    const uint8_t t = type[n];
+    if (t == NODE_SOLID) return;
+    const uint32_t w = (t == NODE_BOUNDARY) ? link[n] : 0u;
     const Nbr o = neighbours(g, x, y, z);
     const T rho = rho0[n];
     T v[3] = {T(0), T(0), T(0)};
@@ -317,37 +321,42 @@ __global__ void init_equilibrium_kernel(Geom g, const uint8_t *__restrict__ type
     T heq[L::Q];
     equilibrium_dev<L, T>(rho, rho - T(1), v, heq);
 #pragma unroll
-    for (int i = 0; i < L::Q; i++) store[(int64_t)i * g.N + (n + shift<L>(i, -1, o))] = heq[i];
+    for (int i = 0; i < L::Q; i++) store[source_slot<L, int64_t>(i, n, g.N, o, w)] = heq[i];
 }
 
 template <class L, typename T>
-__global__ void get_distributions_kernel(Geom g, const uint8_t *__restrict__ type, const T *__restrict__ store,
-                                         T *__restrict__ f) {
+__global__ void get_distributions_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restrict__ link,
+                                         const T *__restrict__ store, T *__restrict__ f) {
     int x, y, z, n;
     if (!thread_node(g, x, y, z, n)) return;
-    if (type[n] == NODE_SOLID) {
+    const uint8_t t = type[n];
+    if (t == NODE_SOLID) {
 #pragma unroll
         for (int i = 0; i < L::Q; i++) f[(int64_t)i * g.N + n] = T(0);
         return;
     }
+    const uint32_t w = (t == NODE_BOUNDARY) ? link[n] : 0u;
     const Nbr o = neighbours(g, x, y, z);
     T h[L::Q];
-    gather<L, T>(store, n, g.N, o, h);
+    gather<L, T>(store, n, g.N, o, w, h);
 #pragma unroll
     for (int i = 0; i < L::Q; i++) f[(int64_t)i * g.N + n] = h[i] + L::template w<T>(i);
 }
 
 // rho = sum f, v = (j + F/2)/rho (eq. 1, eq. 16).  hg = g/2 (0 for SC2).
 template <class L, typename T>
-__global__ void macro_kernel(Geom g, const uint8_t *__restrict__ type, const T *__restrict__ store,
-                             T *__restrict__ rho_out, T *__restrict__ u_out, T hgx, T hgy, T hgz) {
+__global__ void macro_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restrict__ link,
+                             const T *__restrict__ store, T *__restrict__ rho_out, T *__restrict__ u_out,
+                             T hgx, T hgy, T hgz) {
     int x, y, z, n;
     if (!thread_node(g, x, y, z, n)) return;
+    const uint8_t t = type[n];
     T rho = T(0), v[3] = {T(0), T(0), T(0)};
-    if (type[n] != NODE_SOLID) {
+    if (t != NODE_SOLID) {
+        const uint32_t w = (t == NODE_BOUNDARY) ? link[n] : 0u;
         const Nbr o = neighbours(g, x, y, z);
         T h[L::Q], drho, j[3];
-        gather<L, T>(store, n, g.N, o, h);
+        gather<L, T>(store, n, g.N, o, w, h);
         moments<L, T>(h, drho, j);
         rho = T(1) + drho;
         const T hg[3] = {hgx, hgy, hgz};
@@ -374,10 +383,11 @@ template <typename T, int PSI> __device__ __forceinline__ T psi_one() {
 }
 
 // Pass 1 (row a9): psi fields of both components from the time-t state.  SOLID: psi = 0 (A14).
-template <class L, typename T, int V, int PSI>
+template <class L, typename T, int V, typename I, int PSI>
 __global__ void __launch_bounds__(256)
-sc_fields_kernel(Geom g, const uint8_t *__restrict__ type, const T *__restrict__ srcA,
-                 const T *__restrict__ srcB, T *__restrict__ psiA, T *__restrict__ psiB) {
+sc_fields_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restrict__ link,
+                 const T *__restrict__ srcA, const T *__restrict__ srcB, T *__restrict__ psiA,
+                 T *__restrict__ psiB) {
     Span s;
     if (!thread_span<V>(g, s)) return;
     const int n0 = s.row + s.x0;
@@ -388,7 +398,8 @@ sc_fields_kernel(Geom g, const uint8_t *__restrict__ type, const T *__restrict__
         for (int k = 0; k < V; k++) pa[k] = pb[k] = -psi_one<T, PSI>();
     } else {
         T h[V][L::Q];
-        gather_span<L, T, V>(srcA, g.N, s, h);
+        gather_span<L, T, V, I>(srcA, g.N, s, h);
+        pull_reflected_span<L, T, V, I>(srcA, g.N, n0, types, link, h);
 #pragma unroll
         for (int k = 0; k < V; k++) {
             T sum = h[k][0];
@@ -396,7 +407,8 @@ sc_fields_kernel(Geom g, const uint8_t *__restrict__ type, const T *__restrict__
             for (int i = 1; i < L::Q; i++) sum += h[k][i];
             pa[k] = psi_dev<T, PSI>(sum);
         }
-        gather_span<L, T, V>(srcB, g.N, s, h);
+        gather_span<L, T, V, I>(srcB, g.N, s, h);
+        pull_reflected_span<L, T, V, I>(srcB, g.N, n0, types, link, h);
 #pragma unroll
         for (int k = 0; k < V; k++) {
             T sum = h[k][0];
@@ -432,7 +444,7 @@ __device__ __forceinline__ void psi_gradient(const T *__restrict__ psi, int n, c
 
 // Pass 2 (rows a10-a11): both components in one kernel: gather, moments, common velocity u'
 // (P:188), forces (eq. 10, sign A11) + body force, v_s = u' + F_s / (2 rho_s), LBGK + Guo (A13).
-template <class L, typename T, int V, int PSI>
+template <class L, typename T, int V, typename I, int PSI>
 __global__ void __launch_bounds__(256)
 sc_step_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restrict__ link,
                const T *__restrict__ srcA, const T *__restrict__ srcB, T *__restrict__ dstA,
@@ -444,8 +456,10 @@ sc_step_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restr
     const uint32_t types = load_types<V>(type, n0);
     if (all_solid<V>(types)) return;
     T hA[V][L::Q], hB[V][L::Q];
-    gather_span<L, T, V>(srcA, g.N, s, hA);
-    gather_span<L, T, V>(srcB, g.N, s, hB);
+    gather_span<L, T, V, I>(srcA, g.N, s, hA);
+    gather_span<L, T, V, I>(srcB, g.N, s, hB);
+    pull_reflected_span<L, T, V, I>(srcA, g.N, n0, types, link, hA);
+    pull_reflected_span<L, T, V, I>(srcB, g.N, n0, types, link, hB);
 #pragma unroll
     for (int k = 0; k < V; k++) {
         Nbr o = s.o;
@@ -474,8 +488,8 @@ sc_step_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restr
         collide<L, T, false, true>(hA[k], rA, dA, vA, FA, rpA);
         collide<L, T, false, true>(hB[k], rB, dB, vB, FB, rpB);
     }
-    store_span<L, T, V>(dstA, g, s, types, link, hA);
-    store_span<L, T, V>(dstB, g, s, types, link, hB);
+    store_span<L, T, V, I>(dstA, g.N, n0, hA);
+    store_span<L, T, V, I>(dstB, g.N, n0, hB);
 }
 
 }  // namespace lbm

@@ -69,6 +69,25 @@ LBM_HD void guo_bracket(const T (&v)[3], const T (&F)[3], T (&src)[L::Q]) {
 template <class L, typename T> struct Mrt;
 
 template <typename T> struct Mrt<D3Q19, T> {
+    static constexpr bool closed_form_meq = true;
+    // M (f^eq - w) in closed form (reading A6: m^eq = M f^eq with eq. (3)); the coefficients are
+    // sum_i M_ki w_i {1, 3 e_ia, 4.5 e_ia e_ib - 1.5 delta_ab}, which for this basis reduce to
+    // d'Humieres' equilibrium moments with w_eps = 3, w_epsj = -11/2, w_xx = -1/2.
+    LBM_HD static void meq_dev(T rho, T drho, const T (&v)[3], T (&q)[19]) {
+        const T xx = v[0] * v[0], yy = v[1] * v[1], zz = v[2] * v[2];
+        const T rvv = rho * (xx + yy + zz);
+        const T jx = rho * v[0], jy = rho * v[1], jz = rho * v[2];
+        q[0] = drho;
+        q[1] = T(19) * rvv - T(11) * drho;
+        q[2] = T(3) * drho - T(5.5) * rvv;
+        q[3] = jx; q[4] = T(-2.0 / 3.0) * jx;
+        q[5] = jy; q[6] = T(-2.0 / 3.0) * jy;
+        q[7] = jz; q[8] = T(-2.0 / 3.0) * jz;
+        q[9] = rho * (T(2) * xx - yy - zz); q[10] = T(-0.5) * q[9];
+        q[11] = rho * (yy - zz);            q[12] = T(-0.5) * q[11];
+        q[13] = jx * v[1]; q[14] = jy * v[2]; q[15] = jx * v[2];
+        q[16] = T(0); q[17] = T(0); q[18] = T(0);
+    }
     static constexpr double norm(int k) {
         constexpr double n[19] = {19, 2394, 252, 10, 40, 10, 40, 10, 40, 36, 72, 12, 24, 4, 4, 4, 8, 8, 8};
         return n[k];
@@ -136,6 +155,8 @@ template <typename T> struct Mrt<D3Q19, T> {
 // D2Q9 (reading A5): rows 1; -4+3n^2; 4-21n^2/2+9n^4/2; ex; (-5+3n^2)ex; ey; (-5+3n^2)ey;
 // ex^2-ey^2; ex ey.  9x9 is small enough to unroll as constants.
 template <typename T> struct Mrt<D2Q9, T> {
+    static constexpr bool closed_form_meq = false;  // not in the configs: m^eq through M f^eq
+    LBM_HD static void meq_dev(T, T, const T (&)[3], T (&)[9]) {}
     static constexpr double norm(int k) {
         constexpr double n[9] = {9, 36, 36, 6, 12, 6, 12, 4, 4};
         return n[k];
@@ -233,16 +254,47 @@ LBM_HD void collide(T (&h)[L::Q], T rho, T drho, const T (&v)[3], const T (&F)[3
 // Single-component node update: moments, F = rho g, v = j/rho + g/2 (eq. 16), collide.
 template <class L, typename T, bool MRT, bool FORCE>
 LBM_HD void update_node(T (&h)[L::Q], const Relax<T> &rp) {
-    T drho, j[3];
-    moments<L, T>(h, drho, j);
-    const T rho = T(1) + drho, inv_rho = T(1) / rho;
-    T v[3], F[3];
+    constexpr int Q = L::Q;
+    if constexpr (MRT && Mrt<L, T>::closed_form_meq) {
+        // eq. (4) in moment space: m = M h once (it also yields rho - 1 and j), relax towards the
+        // closed-form equilibrium moments, transform back the increment only.
+        T m[Q];
+        Mrt<L, T>::forward(h, m);
+        const T drho = m[0], rho = T(1) + drho, inv_rho = T(1) / rho;
+        T v[3], F[3];
 #pragma unroll
-    for (int a = 0; a < 3; a++) {
-        F[a] = FORCE ? rho * rp.g[a] : T(0);
-        v[a] = FORCE ? (j[a] + T(0.5) * F[a]) * inv_rho : j[a] * inv_rho;
+        for (int a = 0; a < 3; a++) {
+            const T ja = m[3 + 2 * a];
+            F[a] = FORCE ? rho * rp.g[a] : T(0);
+            v[a] = FORCE ? (ja + T(0.5) * F[a]) * inv_rho : ja * inv_rho;
+        }
+        T q[Q];
+        Mrt<L, T>::meq_dev(rho, drho, v, q);
+#pragma unroll
+        for (int k = 0; k < Q; k++) m[k] = rp.cr[k] * (q[k] - m[k]);
+        if constexpr (FORCE) {
+            T src[Q], ms[Q];
+            guo_bracket<L, T>(v, F, src);
+            Mrt<L, T>::forward(src, ms);
+#pragma unroll
+            for (int k = 0; k < Q; k++) m[k] += rp.cs[k] * ms[k];
+        }
+        T o[Q];
+        Mrt<L, T>::backward(m, o);
+#pragma unroll
+        for (int i = 0; i < Q; i++) h[i] += o[i];
+    } else {
+        T drho, j[3];
+        moments<L, T>(h, drho, j);
+        const T rho = T(1) + drho, inv_rho = T(1) / rho;
+        T v[3], F[3];
+#pragma unroll
+        for (int a = 0; a < 3; a++) {
+            F[a] = FORCE ? rho * rp.g[a] : T(0);
+            v[a] = FORCE ? (j[a] + T(0.5) * F[a]) * inv_rho : j[a] * inv_rho;
+        }
+        collide<L, T, MRT, FORCE>(h, rho, drho, v, F, rp);
     }
-    collide<L, T, MRT, FORCE>(h, rho, drho, v, F, rp);
 }
 
 }  // namespace lbm
