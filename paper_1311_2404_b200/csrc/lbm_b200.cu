@@ -44,6 +44,13 @@ struct lbm_ctx {
     int vec;            // nodes per thread of the step kernels (1, 2 or 4 consecutive x)
     int block_threads;  // threads per block of the step kernels
     const Vtbl *vt;
+    // small lattices are launch-bound: GRAPH_STEPS steps are captured once per buffer
+    // parity into a CUDA graph and replayed; capture happens on a private stream because the
+    // caller's stream may be the legacy default stream, which cannot be captured.
+    bool use_graph;
+    cudaStream_t capture_stream;
+    cudaGraphExec_t graph[2];
+    int64_t graph_launches;  // kernels inside one graph
     char err[256];
 };
 
@@ -63,6 +70,14 @@ int fail(lbm_ctx *c, int code, const char *fmt, const char *detail = "") {
     char *dst = c ? c->err : g_err;
     snprintf(dst, 256, fmt, detail);
     return code;
+}
+
+constexpr int GRAPH_STEPS = 50;           // steps per captured graph (even: the buffer parity is restored)
+constexpr int64_t GRAPH_MAX_SITES = 1 << 20;  // above this a step takes >> launch latency
+
+void drop_graphs(lbm_ctx *c) {
+    for (int k = 0; k < 2; k++)
+        if (c->graph[k]) { cudaGraphExecDestroy(c->graph[k]); c->graph[k] = nullptr; }
 }
 
 int check_launch(lbm_ctx *c, const char *what) {
@@ -114,7 +129,7 @@ void make_layout(const lbm_params *p, int Q, int D, Layout *L) {
     L->link = off; off += align_up(4 * N);
     L->counters = off; off += ALIGN;
     if (nc == 2)
-        for (int s = 0; s < 2; s++) { L->psi[s] = off; off += align_up(N * rs); }
+        { L->psi[0] = L->psi[1] = off; off += align_up(2 * N * rs); }  // (psi_A, psi_B) interleaved
     L->stage_mask = off; off += align_up(N);
     L->stage_rho = off; off += align_up(N * rs);
     L->stage_u = off; off += align_up(D * N * rs);
@@ -162,6 +177,7 @@ template <class L, typename T> struct Impl {
         if (cudaMemsetAsync(cnt, 0, sizeof(unsigned), c->stream) != cudaSuccess) return fail(c, LBM_ECUDA, "cudaMemsetAsync(counters)");
         build_links_kernel<L><<<grid_of(c), c->block_x, 0, c->stream>>>(c->g, d_mask, type(c), link(c), cnt);
         c->vec_pending = true;
+        drop_graphs(c);
         return check_launch(c, "build_links_kernel");
     }
 
@@ -225,12 +241,12 @@ template <class L, typename T> struct Impl {
     template <int V, typename I, int PSI> static int step_sc_vi(lbm_ctx *c, int n) {
         const Launch l = span_launch(c, V);
         const Relax<T> rA = make_relax<T>(c, 0), rB = make_relax<T>(c, 1);
-        T *pA = at<T>(c, c->lay.psi[0]), *pB = at<T>(c, c->lay.psi[1]);
+        auto *psi = at<typename Pair<T>::type>(c, c->lay.psi[0]);
         for (int t = 0; t < n; t++) {
-            sc_fields_kernel<L, T, V, I, PSI><<<l.grid, l.block, 0, c->stream>>>(c->g, type(c), link(c), src(c, 0), src(c, 1), pA, pB);
+            sc_fields_kernel<L, T, V, I, PSI><<<l.grid, l.block, 0, c->stream>>>(c->g, type(c), link(c), src(c, 0), src(c, 1), psi);
             if (int rc = check_launch(c, "sc_fields_kernel")) return rc;
             sc_step_kernel<L, T, V, I, PSI><<<l.grid, l.block, 0, c->stream>>>(
-                c->g, type(c), link(c), src(c, 0), src(c, 1), dst(c, 0), dst(c, 1), pA, pB, rA, rB, T(c->p.sc_G));
+                c->g, type(c), link(c), src(c, 0), src(c, 1), dst(c, 0), dst(c, 1), psi, rA, rB, T(c->p.sc_G));
             if (int rc = check_launch(c, "sc_step_kernel")) return rc;
             c->cur ^= 1;
             c->steps++;
@@ -365,11 +381,18 @@ LBM_API int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, voi
     c->block_threads = env_int("LBM_BLOCK_THREADS", 64, 32, 256);
     c->vt = select_impl(p);
     c->err[0] = 0;
+    c->use_graph = c->g.N <= GRAPH_MAX_SITES && !env_int("LBM_NO_GRAPH", 0, 0, 1);
+    if (c->use_graph && cudaStreamCreateWithFlags(&c->capture_stream, cudaStreamNonBlocking) != cudaSuccess) {
+        cudaGetLastError();
+        c->use_graph = false;
+        c->capture_stream = nullptr;
+    }
     // geometry starts all-FLUID: type = BULK, link = 0
     cudaError_t e = cudaMemsetAsync(c->ws + lay.type, 0, (size_t)c->g.N, c->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(c->ws + lay.link, 0, 4 * (size_t)c->g.N, c->stream);
     if (e != cudaSuccess) {
         fail(nullptr, LBM_ECUDA, "cudaMemsetAsync: %s", cudaGetErrorString(e));
+        if (c->capture_stream) cudaStreamDestroy(c->capture_stream);
         delete c;
         return LBM_ECUDA;
     }
@@ -379,6 +402,8 @@ LBM_API int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, voi
 
 LBM_API int lbm_destroy(lbm_ctx *c) {
     CHECK_CTX(c);
+    drop_graphs(c);
+    if (c->capture_stream) cudaStreamDestroy(c->capture_stream);
     delete c;
     return LBM_OK;
 }
@@ -438,6 +463,32 @@ LBM_API int lbm_step(lbm_ctx *c, int n) {
         if (e != cudaSuccess) return fail(c, LBM_ECUDA, "reading the geometry counter: %s", cudaGetErrorString(e));
         c->vec = pick_vec(&c->p, (double)nonbulk / (double)c->g.N);
         c->vec_pending = false;
+    }
+    while (c->use_graph && n >= GRAPH_STEPS) {
+        cudaGraphExec_t &exec = c->graph[c->cur];
+        if (!exec) {  // capture GRAPH_STEPS ordinary step launches; nothing executes during capture
+            const int64_t steps0 = c->steps, launches0 = c->launches;
+            const cudaStream_t user = c->stream;
+            cudaGraph_t g = nullptr;
+            cudaError_t e = cudaStreamBeginCapture(c->capture_stream, cudaStreamCaptureModeThreadLocal);
+            if (e != cudaSuccess) return fail(c, LBM_ECUDA, "cudaStreamBeginCapture: %s", cudaGetErrorString(e));
+            c->stream = c->capture_stream;
+            const int rc = c->vt->step(c, GRAPH_STEPS);
+            c->stream = user;
+            e = cudaStreamEndCapture(c->capture_stream, &g);
+            c->graph_launches = c->launches - launches0;
+            c->steps = steps0;
+            c->launches = launches0;
+            if (rc) { if (g) cudaGraphDestroy(g); return rc; }
+            if (e == cudaSuccess) e = cudaGraphInstantiate(&exec, g, 0);
+            if (g) cudaGraphDestroy(g);
+            if (e != cudaSuccess) { exec = nullptr; return fail(c, LBM_ECUDA, "graph capture/instantiate: %s", cudaGetErrorString(e)); }
+        }
+        cudaError_t e = cudaGraphLaunch(exec, c->stream);
+        if (e != cudaSuccess) return fail(c, LBM_ECUDA, "cudaGraphLaunch: %s", cudaGetErrorString(e));
+        c->steps += GRAPH_STEPS;
+        c->launches += c->graph_launches;
+        n -= GRAPH_STEPS;
     }
     return c->vt->step(c, n);
 }

@@ -382,12 +382,16 @@ template <typename T, int PSI> __device__ __forceinline__ T psi_one() {
     return PSI == 0 ? T(1) : T(0.63212055882855767840);
 }
 
+template <typename T> struct Pair;
+template <> struct Pair<float> { using type = float2; };
+template <> struct Pair<double> { using type = double2; };
+
 // Pass 1 (row a9): psi fields of both components from the time-t state.  SOLID: psi = 0 (A14).
 template <class L, typename T, int V, typename I, int PSI>
 __global__ void __launch_bounds__(256)
 sc_fields_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restrict__ link,
-                 const T *__restrict__ srcA, const T *__restrict__ srcB, T *__restrict__ psiA,
-                 T *__restrict__ psiB) {
+                 const T *__restrict__ srcA, const T *__restrict__ srcB,
+                 typename Pair<T>::type *__restrict__ psi) {
     Span s;
     if (!thread_span<V>(g, s)) return;
     const int n0 = s.row + s.x0;
@@ -418,28 +422,40 @@ sc_fields_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__res
             if (((types >> (8 * k)) & 0xffu) == NODE_SOLID) pa[k] = pb[k] = -psi_one<T, PSI>();
         }
     }
-    // plain stores: pass 2 re-reads the fields right away (L2-resident)
-    Pack<T, V>::stp(psiA + n0, pa);
-    Pack<T, V>::stp(psiB + n0, pb);
+    // (psi_A, psi_B) interleaved: pass 2 fetches both with one 8/16-byte load per neighbour.
+    // Plain stores: pass 2 re-reads the field right away (L2-resident).
+#pragma unroll
+    for (int k = 0; k < V; k++) {
+        typename Pair<T>::type p;
+        p.x = pa[k]; p.y = pb[k];
+        psi[n0 + k] = p;
+    }
 }
 
-// sum_i w_i psi(x + e_i) e_i over the neighbour field (18 L1/L2-served reads).
+// S_A = sum_i w_i psi_A(x + e_i) e_i and S_B likewise, over the interleaved neighbour field
+// (18 L1/L2-served reads of both components at once).
 template <class L, typename T>
-__device__ __forceinline__ void psi_gradient(const T *__restrict__ psi, int n, const Nbr &o, T (&S)[3]) {
-    T ax[3] = {T(0), T(0), T(0)}, dg[3] = {T(0), T(0), T(0)};
+__device__ __forceinline__ void psi_gradient(const typename Pair<T>::type *__restrict__ psi, int n, const Nbr &o,
+                                             T (&SA)[3], T (&SB)[3]) {
+    T axA[3] = {T(0), T(0), T(0)}, dgA[3] = {T(0), T(0), T(0)};
+    T axB[3] = {T(0), T(0), T(0)}, dgB[3] = {T(0), T(0), T(0)};
 #pragma unroll
     for (int i = 1; i < L::Q; i++) {
-        const T p = __ldg(psi + (n + shift<L>(i, +1, o)));
+        const typename Pair<T>::type p = __ldg(psi + (n + shift<L>(i, +1, o)));
         const bool axis = (L::ex(i) != 0) + (L::ey(i) != 0) + (L::ez(i) != 0) == 1;
-        T(&acc)[3] = axis ? ax : dg;
-        if (L::ex(i) == 1) acc[0] += p; else if (L::ex(i) == -1) acc[0] -= p;
-        if (L::ey(i) == 1) acc[1] += p; else if (L::ey(i) == -1) acc[1] -= p;
-        if (L::ez(i) == 1) acc[2] += p; else if (L::ez(i) == -1) acc[2] -= p;
+        T(&a)[3] = axis ? axA : dgA;
+        T(&b)[3] = axis ? axB : dgB;
+        if (L::ex(i) == 1) { a[0] += p.x; b[0] += p.y; } else if (L::ex(i) == -1) { a[0] -= p.x; b[0] -= p.y; }
+        if (L::ey(i) == 1) { a[1] += p.x; b[1] += p.y; } else if (L::ey(i) == -1) { a[1] -= p.x; b[1] -= p.y; }
+        if (L::ez(i) == 1) { a[2] += p.x; b[2] += p.y; } else if (L::ez(i) == -1) { a[2] -= p.x; b[2] -= p.y; }
     }
     // axis weight / diagonal weight = 4 (D2Q9: 1/9 vs 1/36) or 2 (D3Q19: 1/18 vs 1/36)
     const T ratio = L::template w<T>(1) / L::template w<T>(L::Q - 1), wd = L::template w<T>(L::Q - 1);
 #pragma unroll
-    for (int a = 0; a < 3; a++) S[a] = wd * (ratio * ax[a] + dg[a]);
+    for (int c = 0; c < 3; c++) {
+        SA[c] = wd * (ratio * axA[c] + dgA[c]);
+        SB[c] = wd * (ratio * axB[c] + dgB[c]);
+    }
 }
 
 // Pass 2 (rows a10-a11): both components in one kernel: gather, moments, common velocity u'
@@ -448,7 +464,7 @@ template <class L, typename T, int V, typename I, int PSI>
 __global__ void __launch_bounds__(256)
 sc_step_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restrict__ link,
                const T *__restrict__ srcA, const T *__restrict__ srcB, T *__restrict__ dstA,
-               T *__restrict__ dstB, const T *__restrict__ psiA, const T *__restrict__ psiB,
+               T *__restrict__ dstB, const typename Pair<T>::type *__restrict__ psi,
                Relax<T> rpA, Relax<T> rpB, T G) {
     Span s;
     if (!thread_span<V>(g, s)) return;
@@ -467,8 +483,7 @@ sc_step_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restr
         o.xm = (x == 0) ? (g.nx - 1) : -1;
         o.xp = (x == g.nx - 1) ? -(g.nx - 1) : 1;
         T SA[3], SB[3];
-        psi_gradient<L, T>(psiA, n0 + k, o, SA);
-        psi_gradient<L, T>(psiB, n0 + k, o, SB);
+        psi_gradient<L, T>(psi, n0 + k, o, SA, SB);
         T dA, dB, jA[3], jB[3];
         moments<L, T>(hA[k], dA, jA);
         moments<L, T>(hB[k], dB, jB);

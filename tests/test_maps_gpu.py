@@ -87,6 +87,29 @@ def test_set_get_distributions_round_trip_bit_exact(B):
     assert (back[:, fluid] - f[:, fluid]).abs().max() <= 2.3e-16
 
 
+@pytest.mark.parametrize("cfg", ["c1", "c5"])
+def test_graph_replay_is_bit_identical_to_single_launches(B, cfg):
+    """Small lattices replay 50-step CUDA graphs (launch-bound regime): step(120) must give
+    exactly the bits of 120 x step(1), which never reaches the graph threshold."""
+    w = W.c1_taylor_green(64) if cfg == "c1" else W.c5_shan_chen(24, 20, 16)
+    out = []
+    for chunks in ([120], [1] * 120, [50, 7, 63]):
+        sim = B.from_workload(w)
+        sim.set_geometry(w.mask)
+        for s in range(w.ncomp):
+            sim.init_equilibrium(w.rho[s], w.u[s], comp=s)
+        for n in chunks:
+            sim.step(n)
+        assert sim.counters()[0] == 120
+        out.append([sim.get_distributions(s).clone() for s in range(w.ncomp)])
+        assert sim.counters()[1] >= 120 * w.ncomp
+        sim.close()
+    import torch
+    for other in out[1:]:
+        for a, b in zip(out[0], other):
+            assert torch.equal(a, b)
+
+
 def test_run_host_matches_device_calls_and_oracle(B, orc):
     import torch
     w = W.c2_channel(40, 24, 12)
