@@ -80,12 +80,12 @@ def time_oracle(cfg: str, steps: int, warmup: int):
                 sample="%s, %d steps (%.1f s)" % (what, steps, dt)), dt, w
 
 
-def config_dict(w, cfg, extra=None):
+def config_dict(w, cfg, extra=None, store="ab"):
     d = {"workload": "%s: %s %s %s %dx%dx%d" % (cfg, "D2Q9" if w.lattice == W.D2Q9 else "D3Q19",
                                                  ["LBGK", "MRT", "Shan-Chen 2xLBGK"][w.model],
                                                  "fp32" if w.precision == W.F32 else "fp64", w.nx, w.ny, w.nz),
          "tau": list(w.tau)[: w.ncomp], "force": list(w.force), "seed": w.seed,
-         "solid_fraction": float(w.mask.mean()), "store": "AB, SoA real[Q][N]",
+         "solid_fraction": float(w.mask.mean()), "store": ("AA in place" if store == "aa" else "AB double buffer") + ", SoA real[Q][N]",
          "parallelism": "replicas only (path does not shard)"}
     d.update(extra or {})
     return d
@@ -172,7 +172,7 @@ def run_ours(args):
     w = W.CONFIGS[args.config]()
     if w.sites <= (1 << 20):
         Wm = max(Wm, 128)  # small lattices replay 50-step CUDA graphs: capture them before timing
-    sim = binding.from_workload(w, device=dev)
+    sim = binding.from_workload(w, device=dev, store=binding.LBM_STORE_AA if args.store == "aa" else binding.LBM_STORE_AB)
     sim.set_geometry(w.mask)
     for s in range(w.ncomp):
         sim.init_equilibrium(w.rho[s], w.u[s], comp=s)
@@ -236,7 +236,7 @@ def run_ours(args):
                 "config": config_dict(w, args.config, {
                     "l2": "working set %.2f GB per step >> 126 MB L2 (no flush needed)" % (bps * w.sites / 1e9),
                     "timing": "median of %d repeats of K steps, CUDA events on the ctx stream" % args.repeats,
-                    "repeats_ms": reps}),
+                    "repeats_ms": reps}, store=args.store),
                 "clocks": clk,
                 "e2e": {"value": aggregate_mlups(w.sites, K, world, e2e_s), "unit": UNIT,
                         "h2d_bytes_per_step": h2d / K, "d2h_bytes_per_step": d2h / K,
@@ -262,6 +262,7 @@ def main():
     ap.add_argument("--repeats", type=int, default=1)
     ap.add_argument("--cpu-steps", type=int, default=250, help="oracle steps on the bounded sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--store", default="ab", choices=["ab", "aa"], help="AB double buffer (default) or in-place AA")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -39,6 +39,7 @@ struct lbm_ctx {
     bool geometry_frozen;
     bool vec_pending;   // geometry changed: re-pick `vec` from the non-bulk node count at the next step
     int64_t steps, launches;
+    bool aa;            // LBM_STORE_AA: one buffer, `cur` is the step parity (0 even, 1 odd)
     bool idx32;         // Q * N < 2^32: slot numbers fit 32 bits (cheaper address arithmetic)
     int block_x;        // one-node-per-thread kernels: 1-D block along x
     int vec;            // nodes per thread of the step kernels (1, 2 or 4 consecutive x)
@@ -113,7 +114,8 @@ int validate(const lbm_params *p, int *Q, int *D) {
     if (p->model == LBM_SC2 && p->sc_psi != LBM_PSI_RHO && p->sc_psi != LBM_PSI_1MEXP)
         return fail(nullptr, LBM_EINVAL, "unknown sc_psi");
     if (p->lattice == LBM_D2Q9 && p->force[2] != 0.0) return fail(nullptr, LBM_EINVAL, "D2Q9 force has no z component");
-    if (p->store == LBM_STORE_AA) return fail(nullptr, LBM_EUNSUPPORTED, "AA store not built (AB only)");
+    if (p->store == LBM_STORE_AA && p->model == LBM_SC2)
+        return fail(nullptr, LBM_EUNSUPPORTED, "AA store is built for the single-component models only");
     if (p->ny > 65535 || p->nz > 65535) return fail(nullptr, LBM_EUNSUPPORTED, "ny and nz must be <= 65535");
     return LBM_OK;
 }
@@ -124,7 +126,10 @@ void make_layout(const lbm_params *p, int Q, int D, Layout *L) {
     size_t off = 0;
     memset(L, 0, sizeof *L);
     for (int s = 0; s < nc; s++)
-        for (int b = 0; b < 2; b++) { L->store[s][b] = off; off += align_up(Q * N * rs); }
+        for (int b = 0; b < 2; b++) {
+            if (b == 1 && p->store == LBM_STORE_AA) { L->store[s][1] = L->store[s][0]; continue; }  // in place
+            L->store[s][b] = off; off += align_up(Q * N * rs);
+        }
     L->type = off; off += align_up(N);
     L->link = off; off += align_up(4 * N);
     L->counters = off; off += ALIGN;
@@ -181,24 +186,35 @@ template <class L, typename T> struct Impl {
         return check_launch(c, "build_links_kernel");
     }
 
+    template <int MODE> static int aa_convert(lbm_ctx *c, const void *in0, const void *in1, void *out0, void *out1) {
+        aa_convert_kernel<L, T, MODE><<<grid_of(c), c->block_x, 0, c->stream>>>(
+            c->g, c->cur, type(c), link(c), at<T>(c, c->lay.store[0][0]), (const T *)in0, (const T *)in1, (T *)out0,
+            (T *)out1, T(0.5 * c->p.force[0]), T(0.5 * c->p.force[1]), T(0.5 * c->p.force[2]));
+        return check_launch(c, "aa_convert_kernel");
+    }
+
     static int init_equilibrium(lbm_ctx *c, int s, const void *rho, const void *u) {
+        if (c->aa) return aa_convert<2>(c, rho, u, nullptr, nullptr);
         init_equilibrium_kernel<L, T><<<grid_of(c), c->block_x, 0, c->stream>>>(
             c->g, type(c), link(c), (const T *)rho, (const T *)u, at<T>(c, c->lay.store[s][c->cur]));
         return check_launch(c, "init_equilibrium_kernel");
     }
 
     static int set_distributions(lbm_ctx *c, int s, const void *f) {
+        if (c->aa) return aa_convert<0>(c, f, nullptr, nullptr, nullptr);
         set_distributions_kernel<L, T><<<grid_of(c), c->block_x, 0, c->stream>>>(
             c->g, type(c), link(c), (const T *)f, at<T>(c, c->lay.store[s][c->cur]));
         return check_launch(c, "set_distributions_kernel");
     }
 
     static int get_distributions(lbm_ctx *c, int s, void *f) {
+        if (c->aa) return aa_convert<1>(c, nullptr, nullptr, f, nullptr);
         get_distributions_kernel<L, T><<<grid_of(c), c->block_x, 0, c->stream>>>(c->g, type(c), link(c), src(c, s), (T *)f);
         return check_launch(c, "get_distributions_kernel");
     }
 
     static int macro(lbm_ctx *c, int s, void *rho, void *u) {
+        if (c->aa) return aa_convert<3>(c, nullptr, nullptr, rho, u);
         const bool sc = c->p.model == LBM_SC2;  // SC2: bare component velocity (lbm.h)
         macro_kernel<L, T><<<grid_of(c), c->block_x, 0, c->stream>>>(
             c->g, type(c), link(c), src(c, s), (T *)rho, (T *)u, sc ? T(0) : T(0.5 * c->p.force[0]),
@@ -217,6 +233,18 @@ template <class L, typename T> struct Impl {
 
     template <int V, typename I, bool MRT, bool FORCE> static int step_single_vi(lbm_ctx *c, int n, const Relax<T> &rp) {
         const Launch l = span_launch(c, V);
+        if (c->aa) {  // in place: even steps are local (V-node packs), odd steps move data (one node per thread)
+            const Launch l1 = span_launch(c, 1);
+            T *f = at<T>(c, c->lay.store[0][0]);
+            for (int t = 0; t < n; t++) {
+                if (c->cur == 0) aa_even_kernel<L, T, V, I, MRT, FORCE><<<l.grid, l.block, 0, c->stream>>>(c->g, type(c), f, rp);
+                else aa_odd_kernel<L, T, I, MRT, FORCE><<<l1.grid, l1.block, 0, c->stream>>>(c->g, type(c), link(c), f, rp);
+                if (int rc = check_launch(c, "aa_step_kernel")) return rc;
+                c->cur ^= 1;
+                c->steps++;
+            }
+            return LBM_OK;
+        }
         for (int t = 0; t < n; t++) {
             step_kernel<L, T, V, I, MRT, FORCE><<<l.grid, l.block, 0, c->stream>>>(c->g, type(c), link(c), src(c, 0), dst(c, 0), rp);
             if (int rc = check_launch(c, "step_kernel")) return rc;
@@ -376,6 +404,7 @@ LBM_API int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, voi
     c->lay = lay;
     c->block_x = pick_block_x(p->nx);
     c->vec = pick_vec(p, 0.0);
+    c->aa = p->store == LBM_STORE_AA;
     c->idx32 = (double)Q * (double)c->g.N < 4294967296.0 && !env_int("LBM_IDX64", 0, 0, 1);
     c->vec_pending = false;
     c->block_threads = env_int("LBM_BLOCK_THREADS", 64, 32, 256);

@@ -146,6 +146,7 @@ template <typename T> struct Pack<T, 1> {
     static __device__ __forceinline__ void ld(const T *p, T (&a)[1]) { a[0] = __ldg(p); }
     static __device__ __forceinline__ void st(T *p, const T (&a)[1]) { __stcs(p, a[0]); }
     static __device__ __forceinline__ void stp(T *p, const T (&a)[1]) { *p = a[0]; }
+    static __device__ __forceinline__ void ldp(const T *p, T (&a)[1]) { a[0] = *p; }
 };
 template <> struct Pack<float, 2> {
     static __device__ __forceinline__ void ld(const float *p, float (&a)[2]) {
@@ -153,6 +154,9 @@ template <> struct Pack<float, 2> {
     }
     static __device__ __forceinline__ void st(float *p, const float (&a)[2]) {
         __stcs(reinterpret_cast<float2 *>(p), make_float2(a[0], a[1]));
+    }
+    static __device__ __forceinline__ void ldp(const float *p, float (&a)[2]) {
+        const float2 v = *reinterpret_cast<const float2 *>(p); a[0] = v.x; a[1] = v.y;
     }
     static __device__ __forceinline__ void stp(float *p, const float (&a)[2]) {
         *reinterpret_cast<float2 *>(p) = make_float2(a[0], a[1]);
@@ -165,6 +169,9 @@ template <> struct Pack<float, 4> {
     static __device__ __forceinline__ void st(float *p, const float (&a)[4]) {
         __stcs(reinterpret_cast<float4 *>(p), make_float4(a[0], a[1], a[2], a[3]));
     }
+    static __device__ __forceinline__ void ldp(const float *p, float (&a)[4]) {
+        const float4 v = *reinterpret_cast<const float4 *>(p); a[0] = v.x; a[1] = v.y; a[2] = v.z; a[3] = v.w;
+    }
     static __device__ __forceinline__ void stp(float *p, const float (&a)[4]) {
         *reinterpret_cast<float4 *>(p) = make_float4(a[0], a[1], a[2], a[3]);
     }
@@ -175,6 +182,9 @@ template <> struct Pack<double, 2> {
     }
     static __device__ __forceinline__ void st(double *p, const double (&a)[2]) {
         __stcs(reinterpret_cast<double2 *>(p), make_double2(a[0], a[1]));
+    }
+    static __device__ __forceinline__ void ldp(const double *p, double (&a)[2]) {
+        const double2 v = *reinterpret_cast<const double2 *>(p); a[0] = v.x; a[1] = v.y;
     }
     static __device__ __forceinline__ void stp(double *p, const double (&a)[2]) {
         *reinterpret_cast<double2 *>(p) = make_double2(a[0], a[1]);
@@ -367,6 +377,118 @@ __global__ void macro_kernel(Geom g, const uint8_t *__restrict__ type, const uin
     if (u_out) {
 #pragma unroll
         for (int a = 0; a < L::D; a++) u_out[(int64_t)a * g.N + n] = v[a];
+    }
+}
+
+// ---- in-place AA access pattern (row a12; Fig. 4) ---------------------------------
+// One buffer.  Before an EVEN step slot (i, x) holds the canonical f_i(x, t) - w_i.  The even step is
+// purely local: read (i, x), collide, write h*_i(x) to (ibar, x).  Before an ODD step the canonical
+// f_i(x, t) therefore sits in slot (ibar, x - e_i), or for a reflected link in the node's own slot
+// (i, x); the odd step reads those, collides, and writes h*_i(x) to the slot its read of ibar came
+// from, i.e. (i, x + e_i), or (ibar, x) when x + e_i is SOLID -- which is where the next even step
+// expects f(t+2).  Every thread reads and writes exactly the same set of slots.
+template <class L, typename I>
+__device__ __forceinline__ I aa_slot(int parity, int i, int n, int64_t N, const Nbr &o, uint32_t link) {
+    if (parity == 0) return I(i) * I(N) + I(n);
+    return reflected(link, i) ? I(i) * I(N) + I(n) : I(L::opp(i)) * I(N) + I(n + shift<L>(i, -1, o));
+}
+
+template <class L, typename T, int V, typename I, bool MRT, bool FORCE>
+__global__ void __launch_bounds__(256)
+aa_even_kernel(Geom g, const uint8_t *__restrict__ type, T *f, Relax<T> rp) {
+    Span s;
+    if (!thread_span<V>(g, s)) return;
+    const int n0 = s.row + s.x0;
+    const uint32_t types = load_types<V>(type, n0);
+    if (all_solid<V>(types)) return;
+    T h[V][L::Q];
+#pragma unroll
+    for (int i = 0; i < L::Q; i++) {
+        T a[V];
+        Pack<T, V>::ldp(f + (I(i) * I(g.N) + I(n0)), a);
+#pragma unroll
+        for (int k = 0; k < V; k++) h[k][i] = a[k];
+    }
+#pragma unroll
+    for (int k = 0; k < V; k++) update_node<L, T, MRT, FORCE>(h[k], rp);
+#pragma unroll
+    for (int i = 0; i < L::Q; i++) {
+        T a[V];
+#pragma unroll
+        for (int k = 0; k < V; k++) a[k] = h[k][i];
+        Pack<T, V>::stp(f + (I(L::opp(i)) * I(g.N) + I(n0)), a);
+    }
+}
+
+template <class L, typename T, typename I, bool MRT, bool FORCE>
+__global__ void __launch_bounds__(256)
+aa_odd_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restrict__ link, T *f, Relax<T> rp) {
+    Span s;
+    if (!thread_span<1>(g, s)) return;
+    const int n = s.row + s.x0;
+    const uint8_t t = type[n];
+    if (t == NODE_SOLID) return;
+    const uint32_t w = (t == NODE_BOUNDARY) ? __ldg(link + n) : 0u;
+    const Nbr o = neighbours(g, s.x0, s.y, s.z);
+    I slot[L::Q];
+    T h[L::Q];
+#pragma unroll
+    for (int i = 0; i < L::Q; i++) {
+        slot[i] = aa_slot<L, I>(1, i, n, g.N, o, w);
+        h[i] = f[slot[i]];
+    }
+    update_node<L, T, MRT, FORCE>(h, rp);
+#pragma unroll
+    for (int i = 0; i < L::Q; i++) f[slot[L::opp(i)]] = h[i];
+}
+
+// Conversions for the AA store (parity 0: before an even step, 1: before an odd step).
+template <class L, typename T, int MODE>  // MODE 0: set from canonical f, 1: get canonical f, 2: init f^eq, 3: macro
+__global__ void aa_convert_kernel(Geom g, int parity, const uint8_t *__restrict__ type,
+                                  const uint32_t *__restrict__ link, T *store, const T *in0, const T *in1,
+                                  T *out0, T *out1, T hgx, T hgy, T hgz) {
+    int x, y, z, n;
+    if (!thread_node(g, x, y, z, n)) return;
+    const uint8_t t = type[n];
+    const uint32_t w = (t == NODE_BOUNDARY) ? link[n] : 0u;
+    const Nbr o = neighbours(g, x, y, z);
+    if (MODE == 0 || MODE == 2) {
+        if (t == NODE_SOLID) return;
+        T h[L::Q];
+        if (MODE == 0) {
+#pragma unroll
+            for (int i = 0; i < L::Q; i++) h[i] = in0[(int64_t)i * g.N + n] - L::template w<T>(i);
+        } else {
+            T v[3] = {T(0), T(0), T(0)};
+#pragma unroll
+            for (int a = 0; a < L::D; a++) v[a] = in1[(int64_t)a * g.N + n];
+            equilibrium_dev<L, T>(in0[n], in0[n] - T(1), v, h);
+        }
+#pragma unroll
+        for (int i = 0; i < L::Q; i++) store[aa_slot<L, int64_t>(parity, i, n, g.N, o, w)] = h[i];
+    } else {
+        T h[L::Q];
+#pragma unroll
+        for (int i = 0; i < L::Q; i++) h[i] = (t == NODE_SOLID) ? T(0) : store[aa_slot<L, int64_t>(parity, i, n, g.N, o, w)];
+        if (MODE == 1) {
+#pragma unroll
+            for (int i = 0; i < L::Q; i++) out0[(int64_t)i * g.N + n] = (t == NODE_SOLID) ? T(0) : h[i] + L::template w<T>(i);
+        } else {
+            T rho = T(0), v[3] = {T(0), T(0), T(0)};
+            if (t != NODE_SOLID) {
+                T drho, j[3];
+                moments<L, T>(h, drho, j);
+                rho = T(1) + drho;
+                const T hg[3] = {hgx, hgy, hgz};
+#pragma unroll
+                for (int a = 0; a < 3; a++) v[a] = (j[a] + rho * hg[a]) / rho;
+            }
+            if (out0) out0[n] = rho;
+            if (out1) {
+#pragma unroll
+                for (int a = 0; a < L::D; a++) out1[(int64_t)a * g.N + n] = v[a];
+            }
+        }
     }
 }
 

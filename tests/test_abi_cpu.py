@@ -64,7 +64,8 @@ def test_lattice_info_table1(lib):
     (dict(nx=2048, ny=2048, nz=1024), binding.LBM_EINVAL),
     (dict(lattice=0, nz=4), binding.LBM_EINVAL),
     (dict(model=1, rates=[2.5] * 19), binding.LBM_EINVAL),
-    (dict(store=1), binding.LBM_EUNSUPPORTED),
+    (dict(store=1, model=2, tau=(1.0, 1.0)), binding.LBM_EUNSUPPORTED),
+    (dict(store=7), binding.LBM_EINVAL),
 ])
 def test_bad_params_rejected(lib, kw, code):
     args = dict(lattice=1, model=0, precision=0, nx=8, ny=8, nz=8, tau=0.8)

@@ -134,3 +134,70 @@ def test_all_solid_and_all_fluid(B, orc):
     rho, u = sim.macro()
     assert float(rho.abs().max()) == 0.0 and float(u.abs().max()) == 0.0
     assert (sim.get_stream_map().cpu().numpy() == -1).all()
+
+
+# ---- in-place AA store (row a12): same results from one buffer --------------------------
+def check_parity_aa(B, orc, w, steps):
+    sim = B.from_workload(w, store=B.LBM_STORE_AA)
+    ref = orc.Oracle(**w.params())
+    sim.set_geometry(w.mask)
+    ref.set_geometry(w.mask)
+    sim.init_equilibrium(w.rho[0], w.u[0])
+    ref.init_equilibrium(w.rho[0], w.u[0])
+    done = 0
+    for n in steps:  # odd chunk sizes: read-out happens at both parities
+        sim.step(n)
+        ref.step(n)
+        done += n
+        assert max_err(sim, ref, w) <= TOL[w.precision], done
+        rho_g, u_g = sim.macro()
+        rho_r, u_r = ref.macro()
+        assert np.abs(rho_g.cpu().numpy() - rho_r).max() <= TOL[w.precision]
+        assert np.abs(u_g.cpu().numpy() - u_r).max() <= TOL[w.precision]
+    sim.close()
+
+
+@pytest.mark.parametrize("shape", [(96, 40, 24), (50, 37, 29)])
+def test_aa_c2_channel(B, orc, shape):
+    check_parity_aa(B, orc, W.c2_channel(*shape), [1, 2, 37, 60])
+
+
+@pytest.mark.parametrize("precision", [W.F32, W.F64])
+def test_aa_c3_mrt_random_solids(B, orc, precision):
+    check_parity_aa(B, orc, W.c3_mrt_obstacles(64, 40, 23, precision=precision), [51, 49])
+
+
+def test_aa_c4_duct_fp64(B, orc):
+    check_parity_aa(B, orc, W.c4_duct(70, 21, 19), [33, 67])
+
+
+def test_aa_c1_taylor_green(B, orc):
+    check_parity_aa(B, orc, W.c1_taylor_green(), [101])
+
+
+def test_aa_degenerate_and_d2q9_mrt(B, orc):
+    check_parity_aa(B, orc, generic(W.D3Q19, W.BGK, W.F64, (2, 1, 3), 21, solid=0.0, force=(1e-5, 0, 0)), [7, 8])
+    check_parity_aa(B, orc, generic(W.D2Q9, W.MRT, W.F64, (37, 22, 1), 22, rates=W.mrt_rates_d2q9(0.7),
+                                    force=(2e-5, -1e-5, 0.0)), [15, 16])
+
+
+def test_aa_set_get_round_trip_at_both_parities(B):
+    import torch
+    mask, _, _ = W.random_state(W.D3Q19, 21, 13, 6, seed=5, solid_fraction=0.2)
+    fluid = torch.from_numpy(mask == 0)
+    f = torch.rand((19, 6, 13, 21), generator=torch.Generator().manual_seed(2), dtype=torch.float64)
+    for presteps in (0, 1):
+        sim = B.Lbm(W.D3Q19, W.BGK, W.F64, 21, 13, 6, tau=0.8, store=B.LBM_STORE_AA)
+        sim.set_geometry(mask)
+        sim.set_distributions(f)
+        sim.step(presteps)
+        sim.set_distributions(f)  # overwrite at the current parity
+        back = sim.get_distributions().cpu()
+        assert (back[:, ~fluid] == 0).all()
+        assert (back[:, fluid] - f[:, fluid]).abs().max() <= 2.3e-16
+
+
+def test_aa_uses_half_the_distribution_memory(B):
+    ab = B.lbm_workspace_bytes(B.make_params(W.D3Q19, W.BGK, W.F32, 64, 64, 64, tau=0.8))
+    aa = B.lbm_workspace_bytes(B.make_params(W.D3Q19, W.BGK, W.F32, 64, 64, 64, tau=0.8, store=B.LBM_STORE_AA))
+    assert ab - aa == 19 * 64 ** 3 * 4
