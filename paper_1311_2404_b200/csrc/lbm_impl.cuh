@@ -1,0 +1,271 @@
+// lbm_impl.cuh -- host-side context, workspace layout and the per-<lattice, real> kernel dispatch.
+// Included by lbm_b200.cu (the C ABI) and by one small translation unit per <lattice, real> pair
+// (lbm_impl_*.cu), so that the kernel instantiations compile in parallel.  Product code: shares
+// nothing with oracle/.
+#pragma once
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+#include "../../include/lbm.h"
+#include "lbm_kernels.cuh"
+
+using namespace lbm;
+
+namespace {
+
+thread_local char g_err[256] = "";
+
+constexpr size_t ALIGN = 256;
+inline size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
+
+struct Layout {
+    size_t store[2][2], type, link, counters, psi[2], stage_mask, stage_rho, stage_u, total;
+};
+
+struct Vtbl;
+
+}  // namespace
+
+struct lbm_ctx {
+    lbm_params p;
+    int Q, D, ncomp;
+    size_t rs;  // sizeof(real)
+    Geom g;
+    cudaStream_t stream;
+    char *ws;
+    Layout lay;
+    int cur;  // which of the two buffers holds the current state (AB)
+    bool inited[2];
+    bool geometry_frozen;
+    bool vec_pending;   // geometry changed: re-pick `vec` from the non-bulk node count at the next step
+    int64_t steps, launches;
+    bool aa;            // LBM_STORE_AA: one buffer, `cur` is the step parity (0 even, 1 odd)
+    bool idx32;         // Q * N < 2^32: slot numbers fit 32 bits (cheaper address arithmetic)
+    int block_x;        // one-node-per-thread kernels: 1-D block along x
+    int vec;            // nodes per thread of the step kernels (1, 2 or 4 consecutive x)
+    int block_threads;  // threads per block of the step kernels
+    const Vtbl *vt;
+    // small lattices are launch-bound: GRAPH_STEPS steps are captured once per buffer
+    // parity into a CUDA graph and replayed; capture happens on a private stream because the
+    // caller's stream may be the legacy default stream, which cannot be captured.
+    bool use_graph;
+    cudaStream_t capture_stream;
+    cudaGraphExec_t graph[2];
+    int64_t graph_launches;  // kernels inside one graph
+    char err[256];
+};
+
+namespace {
+
+struct Vtbl {
+    int (*set_geometry)(lbm_ctx *, const uint8_t *);
+    int (*init_equilibrium)(lbm_ctx *, int, const void *, const void *);
+    int (*step)(lbm_ctx *, int);
+    int (*macro)(lbm_ctx *, int, void *, void *);
+    int (*get_distributions)(lbm_ctx *, int, void *);
+    int (*set_distributions)(lbm_ctx *, int, const void *);
+    int (*get_stream_map)(lbm_ctx *, int64_t *);
+};
+
+int fail(lbm_ctx *c, int code, const char *fmt, const char *detail = "") {
+    char *dst = c ? c->err : g_err;
+    snprintf(dst, 256, fmt, detail);
+    return code;
+}
+
+constexpr int GRAPH_STEPS = 50;           // steps per captured graph (even: the buffer parity is restored)
+constexpr int64_t GRAPH_MAX_SITES = 1 << 20;  // above this a step takes >> launch latency
+
+void drop_graphs(lbm_ctx *c) {
+    for (int k = 0; k < 2; k++)
+        if (c->graph[k]) { cudaGraphExecDestroy(c->graph[k]); c->graph[k] = nullptr; }
+}
+
+int check_launch(lbm_ctx *c, const char *what) {
+    c->launches++;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) {
+        snprintf(c->err, sizeof c->err, "%s: %s", what, cudaGetErrorString(e));
+        return LBM_ECUDA;
+    }
+    return LBM_OK;
+}
+
+template <typename T> T *at(lbm_ctx *c, size_t off) { return reinterpret_cast<T *>(c->ws + off); }
+
+dim3 grid_of(const lbm_ctx *c) { return dim3((c->g.nx + c->block_x - 1) / c->block_x, c->g.ny, c->g.nz); }
+
+template <typename T> Relax<T> make_relax(const lbm_ctx *c, int comp) {
+    Relax<T> r;
+    const double tau = c->p.tau[comp];
+    r.inv_tau = T(1.0 / tau);
+    r.src_scale = T(1.0 - 0.5 / tau);
+    for (int a = 0; a < 3; a++) r.g[a] = T(c->p.force[a]);
+    for (int k = 0; k < 19; k++) r.cr[k] = r.cs[k] = T(0);
+    return r;
+}
+
+// ---- per <lattice, real> implementation -------------------------------------------------------
+struct Launch { dim3 grid, block; };
+
+// Step kernels: V nodes per thread along x, 2-D blocks (bx packs) x (by rows).
+Launch span_launch(const lbm_ctx *c, int V) {
+    const int nxv = c->g.nx / V;
+    const int bx = nxv > 32 ? 64 : 32;
+    int by = c->block_threads / bx;
+    if (by < 1) by = 1;
+    while (by > 1 && by / 2 >= c->g.ny) by /= 2;
+    Launch l;
+    l.block = dim3(bx, by, 1);
+    l.grid = dim3((nxv + bx - 1) / bx, (c->g.ny + by - 1) / by, c->g.nz);
+    return l;
+}
+
+template <class L, typename T> struct Impl {
+    static const T *src(lbm_ctx *c, int s) { return at<T>(c, c->lay.store[s][c->cur]); }
+    static T *dst(lbm_ctx *c, int s) { return at<T>(c, c->lay.store[s][c->cur ^ 1]); }
+    static uint8_t *type(lbm_ctx *c) { return at<uint8_t>(c, c->lay.type); }
+    static uint32_t *link(lbm_ctx *c) { return at<uint32_t>(c, c->lay.link); }
+
+    static int set_geometry(lbm_ctx *c, const uint8_t *d_mask) {
+        unsigned *cnt = at<unsigned>(c, c->lay.counters);
+        if (cudaMemsetAsync(cnt, 0, sizeof(unsigned), c->stream) != cudaSuccess) return fail(c, LBM_ECUDA, "cudaMemsetAsync(counters)");
+        build_links_kernel<L><<<grid_of(c), c->block_x, 0, c->stream>>>(c->g, d_mask, type(c), link(c), cnt);
+        c->vec_pending = true;
+        drop_graphs(c);
+        return check_launch(c, "build_links_kernel");
+    }
+
+    template <int MODE> static int aa_convert(lbm_ctx *c, const void *in0, const void *in1, void *out0, void *out1) {
+        aa_convert_kernel<L, T, MODE><<<grid_of(c), c->block_x, 0, c->stream>>>(
+            c->g, c->cur, type(c), link(c), at<T>(c, c->lay.store[0][0]), (const T *)in0, (const T *)in1, (T *)out0,
+            (T *)out1, T(0.5 * c->p.force[0]), T(0.5 * c->p.force[1]), T(0.5 * c->p.force[2]));
+        return check_launch(c, "aa_convert_kernel");
+    }
+
+    static int init_equilibrium(lbm_ctx *c, int s, const void *rho, const void *u) {
+        if (c->aa) return aa_convert<2>(c, rho, u, nullptr, nullptr);
+        init_equilibrium_kernel<L, T><<<grid_of(c), c->block_x, 0, c->stream>>>(
+            c->g, type(c), link(c), (const T *)rho, (const T *)u, at<T>(c, c->lay.store[s][c->cur]));
+        return check_launch(c, "init_equilibrium_kernel");
+    }
+
+    static int set_distributions(lbm_ctx *c, int s, const void *f) {
+        if (c->aa) return aa_convert<0>(c, f, nullptr, nullptr, nullptr);
+        set_distributions_kernel<L, T><<<grid_of(c), c->block_x, 0, c->stream>>>(
+            c->g, type(c), link(c), (const T *)f, at<T>(c, c->lay.store[s][c->cur]));
+        return check_launch(c, "set_distributions_kernel");
+    }
+
+    static int get_distributions(lbm_ctx *c, int s, void *f) {
+        if (c->aa) return aa_convert<1>(c, nullptr, nullptr, f, nullptr);
+        get_distributions_kernel<L, T><<<grid_of(c), c->block_x, 0, c->stream>>>(c->g, type(c), link(c), src(c, s), (T *)f);
+        return check_launch(c, "get_distributions_kernel");
+    }
+
+    static int macro(lbm_ctx *c, int s, void *rho, void *u) {
+        if (c->aa) return aa_convert<3>(c, nullptr, nullptr, rho, u);
+        const bool sc = c->p.model == LBM_SC2;  // SC2: bare component velocity (lbm.h)
+        macro_kernel<L, T><<<grid_of(c), c->block_x, 0, c->stream>>>(
+            c->g, type(c), link(c), src(c, s), (T *)rho, (T *)u, sc ? T(0) : T(0.5 * c->p.force[0]),
+            sc ? T(0) : T(0.5 * c->p.force[1]), sc ? T(0) : T(0.5 * c->p.force[2]));
+        return check_launch(c, "macro_kernel");
+    }
+
+    static int get_stream_map(lbm_ctx *c, int64_t *map) {
+        stream_map_kernel<L><<<grid_of(c), c->block_x, 0, c->stream>>>(c->g, type(c), link(c), map);
+        return check_launch(c, "stream_map_kernel");
+    }
+
+    template <int V, bool MRT, bool FORCE> static int step_single_v(lbm_ctx *c, int n, const Relax<T> &rp) {
+        return c->idx32 ? step_single_vi<V, uint32_t, MRT, FORCE>(c, n, rp) : step_single_vi<V, int64_t, MRT, FORCE>(c, n, rp);
+    }
+
+    template <int V, typename I, bool MRT, bool FORCE> static int step_single_vi(lbm_ctx *c, int n, const Relax<T> &rp) {
+        const Launch l = span_launch(c, V);
+        if (c->aa) {  // in place: even steps are local (V-node packs), odd steps move data (one node per thread)
+            const Launch l1 = span_launch(c, 1);
+            T *f = at<T>(c, c->lay.store[0][0]);
+            for (int t = 0; t < n; t++) {
+                if (c->cur == 0) aa_even_kernel<L, T, V, I, MRT, FORCE><<<l.grid, l.block, 0, c->stream>>>(c->g, type(c), f, rp);
+                else aa_odd_kernel<L, T, I, MRT, FORCE><<<l1.grid, l1.block, 0, c->stream>>>(c->g, type(c), link(c), f, rp);
+                if (int rc = check_launch(c, "aa_step_kernel")) return rc;
+                c->cur ^= 1;
+                c->steps++;
+            }
+            return LBM_OK;
+        }
+        for (int t = 0; t < n; t++) {
+            step_kernel<L, T, V, I, MRT, FORCE><<<l.grid, l.block, 0, c->stream>>>(c->g, type(c), link(c), src(c, 0), dst(c, 0), rp);
+            if (int rc = check_launch(c, "step_kernel")) return rc;
+            c->cur ^= 1;
+            c->steps++;
+        }
+        return LBM_OK;
+    }
+
+    template <bool MRT, bool FORCE> static int step_single(lbm_ctx *c, int n, const Relax<T> &rp) {
+        if constexpr (sizeof(T) == 4) {
+            if (c->vec == 4) return step_single_v<4, MRT, FORCE>(c, n, rp);
+        }
+        if (c->vec == 2) return step_single_v<2, MRT, FORCE>(c, n, rp);
+        return step_single_v<1, MRT, FORCE>(c, n, rp);
+    }
+
+    template <int V, int PSI> static int step_sc_v(lbm_ctx *c, int n) {
+        return c->idx32 ? step_sc_vi<V, uint32_t, PSI>(c, n) : step_sc_vi<V, int64_t, PSI>(c, n);
+    }
+
+    template <int V, typename I, int PSI> static int step_sc_vi(lbm_ctx *c, int n) {
+        const Launch l = span_launch(c, V);
+        const Relax<T> rA = make_relax<T>(c, 0), rB = make_relax<T>(c, 1);
+        auto *psi = at<typename Pair<T>::type>(c, c->lay.psi[0]);
+        for (int t = 0; t < n; t++) {
+            sc_fields_kernel<L, T, V, I, PSI><<<l.grid, l.block, 0, c->stream>>>(c->g, type(c), link(c), src(c, 0), src(c, 1), psi);
+            if (int rc = check_launch(c, "sc_fields_kernel")) return rc;
+            sc_step_kernel<L, T, V, I, PSI><<<l.grid, l.block, 0, c->stream>>>(
+                c->g, type(c), link(c), src(c, 0), src(c, 1), dst(c, 0), dst(c, 1), psi, rA, rB, T(c->p.sc_G));
+            if (int rc = check_launch(c, "sc_step_kernel")) return rc;
+            c->cur ^= 1;
+            c->steps++;
+        }
+        return LBM_OK;
+    }
+
+    template <int PSI> static int step_sc(lbm_ctx *c, int n) {
+        if constexpr (sizeof(T) == 4) {  // fp64 with two components and V = 2 would spill
+            if (c->vec >= 2) return step_sc_v<2, PSI>(c, n);
+        }
+        return step_sc_v<1, PSI>(c, n);
+    }
+
+    static int step(lbm_ctx *c, int n) {
+        if (c->p.model == LBM_SC2) return c->p.sc_psi == LBM_PSI_RHO ? step_sc<0>(c, n) : step_sc<1>(c, n);
+        Relax<T> rp = make_relax<T>(c, 0);
+        const bool force = c->p.force[0] != 0.0 || c->p.force[1] != 0.0 || c->p.force[2] != 0.0;
+        if (c->p.model == LBM_MRT) {
+            for (int k = 0; k < L::Q; k++) {  // M^-1 = M^T diag(1/|M_k|^2): rows are orthogonal (A5)
+                rp.cr[k] = T(c->p.rates[k] / Mrt<L, T>::norm(k));
+                rp.cs[k] = T((1.0 - 0.5 * c->p.rates[k]) / Mrt<L, T>::norm(k));
+            }
+            return force ? step_single<true, true>(c, n, rp) : step_single<true, false>(c, n, rp);
+        }
+        return force ? step_single<false, true>(c, n, rp) : step_single<false, false>(c, n, rp);
+    }
+
+    static const Vtbl *table() {
+        static const Vtbl vt = {&Impl::set_geometry, &Impl::init_equilibrium, &Impl::step, &Impl::macro,
+                                &Impl::get_distributions, &Impl::set_distributions, &Impl::get_stream_map};
+        return &vt;
+    }
+};
+
+}  // namespace
+
+// One factory per translation unit lbm_impl_*.cu.
+const void *lbm_impl_d2q9_f32();
+const void *lbm_impl_d2q9_f64();
+const void *lbm_impl_d3q19_f32();
+const void *lbm_impl_d3q19_f64();

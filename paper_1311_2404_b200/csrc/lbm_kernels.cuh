@@ -120,7 +120,7 @@ __global__ void build_links_kernel(Geom g, const uint8_t *__restrict__ mask, uin
     if (votes && (threadIdx.x & 31) == __ffs(active) - 1) atomicAdd(nonbulk_count, __popc(votes));
 }
 
-__global__ void get_geometry_kernel(Geom g, const uint8_t *__restrict__ type, uint8_t *__restrict__ mask) {
+static __global__ void get_geometry_kernel(Geom g, const uint8_t *__restrict__ type, uint8_t *__restrict__ mask) {
     int x, y, z, n;
     if (!thread_node(g, x, y, z, n)) return;
     mask[n] = type[n] == NODE_SOLID ? 1 : 0;
