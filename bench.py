@@ -54,6 +54,12 @@ def measured_peak():
         return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+def make_workload(args):
+    if args.precision is None:
+        return W.CONFIGS[args.config]()
+    return W.CONFIGS[args.config](precision=W.F32 if args.precision == "f32" else W.F64)
+
+
 def sample_workload(cfg: str):
     """Bounded sample of the config for the CPU oracle: same recipe, same nx*ny cross-section,
     a thin z-slab (the torus closes it), so one oracle step costs ~0.25 s per 2M sites."""
@@ -169,7 +175,7 @@ def run_ours(args):
     binding.load()  # no fallback: raises if the CUDA library is missing
 
     K, Wm = args.steps, max(args.warmup, 3)
-    w = W.CONFIGS[args.config]()
+    w = make_workload(args)
     if w.sites <= (1 << 20):
         Wm = max(Wm, 128)  # small lattices replay 50-step CUDA graphs: capture them before timing
     sim = binding.from_workload(w, device=dev, store=binding.LBM_STORE_AA if args.store == "aa" else binding.LBM_STORE_AB)
@@ -262,6 +268,7 @@ def main():
     ap.add_argument("--repeats", type=int, default=1)
     ap.add_argument("--cpu-steps", type=int, default=250, help="oracle steps on the bounded sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--precision", default=None, choices=["f32", "f64"], help="override the config's precision (c3 is quoted in both)")
     ap.add_argument("--store", default="ab", choices=["ab", "aa"], help="AB double buffer (default) or in-place AA")
     args = ap.parse_args()
     if args.impl == "reference":
