@@ -20,7 +20,7 @@ assert t == float(world), t
 assert bench.aggregate_mlups(1000, 10, world, 1e-3) == 1000 * 10 * world / 1e-3 / 1e6
 dist.barrier()
 dist.destroy_process_group()
-sys.stdout.write("rank%d-ok\n" % rank)
+sys.stdout.write("rank%%d-ok\n" %% rank)
 sys.stdout.flush()
 """
 
