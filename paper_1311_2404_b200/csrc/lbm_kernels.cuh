@@ -613,7 +613,7 @@ sc_step_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restr
         const T pA = psi_dev<T, PSI>(dA) + psi_one<T, PSI>(), pB = psi_dev<T, PSI>(dB) + psi_one<T, PSI>();
         const T inv_den = T(1) / (rA * rpA.inv_tau + rB * rpB.inv_tau);
         const T irA = T(0.5) / rA, irB = T(0.5) / rB;
-        T vA[3], vB[3], FA[3], FB[3];
+        T vA[3], vB[3], mA[3], mB[3], FA[3], FB[3];
 #pragma unroll
         for (int a = 0; a < 3; a++) {
             const T up = (jA[a] * rpA.inv_tau + jB[a] * rpB.inv_tau) * inv_den;
@@ -621,9 +621,11 @@ sc_step_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restr
             FB[a] = -G * pB * SA[a] + rB * rpB.g[a];
             vA[a] = up + FA[a] * irA;
             vB[a] = up + FB[a] * irB;
+            mA[a] = rA * vA[a];
+            mB[a] = rB * vB[a];
         }
-        collide<L, T, false, true>(hA[k], rA, dA, vA, FA, rpA);
-        collide<L, T, false, true>(hB[k], rB, dB, vB, FB, rpB);
+        collide<L, T, false, true>(hA[k], rA, dA, vA, mA, FA, rpA);
+        collide<L, T, false, true>(hB[k], rB, dB, vB, mB, FB, rpB);
     }
     store_span<L, T, V, I>(dstA, g.N, n0, hA);
     store_span<L, T, V, I>(dstB, g.N, n0, hB);

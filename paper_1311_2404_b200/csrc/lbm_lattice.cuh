@@ -23,6 +23,7 @@ struct D2Q9 {
     template <typename T> LBM_HD static constexpr T w(int i) {
         return i == 0 ? T(4) / T(9) : (i < 5 ? T(1) / T(9) : T(1) / T(36));
     }
+    LBM_HD static constexpr int w36(int i) { return i == 0 ? 16 : (i < 5 ? 4 : 1); }  // 36 w_i
 };
 
 struct D3Q19 {
@@ -48,6 +49,7 @@ struct D3Q19 {
     template <typename T> LBM_HD static constexpr T w(int i) {
         return i == 0 ? T(1) / T(3) : (i < 7 ? T(1) / T(18) : T(1) / T(36));
     }
+    LBM_HD static constexpr int w36(int i) { return i == 0 ? 12 : (i < 7 ? 2 : 1); }  // 36 w_i
 };
 
 // Bit 31 of a node's link word marks the node itself SOLID; bit i (< Q) marks the pull source

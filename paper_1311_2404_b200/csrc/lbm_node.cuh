@@ -13,12 +13,30 @@ namespace lbm {
 
 // Parameters of one component's collision, passed to kernels by value (constant bank).
 template <typename T> struct Relax {
-    T inv_tau;        // 1 / tau
-    T src_scale;      // 1 - 1/(2 tau), prefactor of eq. (17)
+    T inv_tau;        // omega = 1 / tau, rounded to T such that 1 - omega is also a T (set_bgk)
+    T keep;           // 1 - omega, exactly
+    T src_scale;      // 1 - omega / 2, prefactor of eq. (17)
+    // omega / 36 and (1 - omega / 2) / 36 as unevaluated sums hi + lo of two T (see collide()):
+    T om36_hi, om36_lo, sc36_hi, sc36_lo;
     T g[3];           // body acceleration
     T cr[19];         // MRT: rate_k / |M_k|^2                 (relaxation, eq. 4)
     T cs[19];         // MRT: (1 - rate_k / 2) / |M_k|^2       (source, reading A16)
 };
+
+// Fill the LBGK constants for relaxation time tau.  omega is rounded to T once and every other
+// constant is derived from that rounded value, so that the collision conserves mass and momentum
+// for the omega it actually uses.
+template <typename T> inline void set_bgk(Relax<T> &r, double tau) {
+    // pick the pair (omega, 1 - omega) so that both are representable: for omega in [1/2, 2] the
+    // difference 1 - fl(omega) is exact (Sterbenz); below 1/2 round 1 - omega first and take
+    // omega = 1 - fl(1 - omega), exact for the same reason.
+    if (1.0 / tau >= 0.5) { r.inv_tau = T(1.0 / tau); r.keep = T(1) - r.inv_tau; }
+    else { r.keep = T(1.0 - 1.0 / tau); r.inv_tau = T(1) - r.keep; }
+    const double om = double(r.inv_tau), c = om / 36.0, s = (1.0 - 0.5 * om) / 36.0;
+    r.src_scale = T(1.0 - 0.5 * om);
+    r.om36_hi = T(c); r.om36_lo = T(c - double(r.om36_hi));
+    r.sc36_hi = T(s); r.sc36_lo = T(s - double(r.sc36_hi));
+}
 
 template <class L, typename T> LBM_HD void moments(const T (&h)[L::Q], T &drho, T (&j)[3]) {
     T s = h[0], jx = T(0), jy = T(0), jz = T(0);
@@ -194,39 +212,58 @@ template <typename T> struct Mrt<D2Q9, T> {
 };
 
 // ---- collision: h (pre-collision deviations) -> h* (post-collision), in place ---------------
-// rho, drho = rho - 1, v = velocity entering f^eq and eq. (17) (reading A3), F = force density.
+// rho, drho = rho - 1, v = velocity entering f^eq and eq. (17) (reading A3), rv = rho v as formed
+// from the moments (j + F/2, eq. 16), F = force density.
 template <class L, typename T, bool MRT, bool FORCE>
-LBM_HD void collide(T (&h)[L::Q], T rho, T drho, const T (&v)[3], const T (&F)[3], const Relax<T> &rp) {
+LBM_HD void collide(T (&h)[L::Q], T rho, T drho, const T (&v)[3], const T (&rv)[3], const T (&F)[3], const Relax<T> &rp) {
     constexpr int Q = L::Q;
     if constexpr (!MRT) {
         // LBGK (Alg. 1 l.13) + eq. (17), evaluated per +/- pair of directions: with e_ibar = -e_i
         // the equilibrium and the source split into a part even in e_i (shared by the pair) and a
         // part odd in e_i (opposite signs), which halves the arithmetic per node.
-        const T om = rp.inv_tau, keep = T(1) - rp.inv_tau, sc = rp.src_scale;
-        const T base = drho - rho * (T(1.5) * (v[0] * v[0] + v[1] * v[1] + v[2] * v[2]));
-        const T r45 = T(4.5) * rho, r3 = T(3) * rho;
-        const T vF3 = FORCE ? T(3) * (v[0] * F[0] + v[1] * F[1] + v[2] * F[2]) : T(0);
-        {
-            T a = om * L::template w<T>(0) * base;
-            if constexpr (FORCE) a -= sc * L::template w<T>(0) * vF3;
-            h[0] = keep * h[0] + a;
+        //
+        // Round-off: a constant such as fl(omega w_i) carries the same rounding
+        // error at every node and step; in fp32 that made sum_i e_i f_i^eq differ from rho u by a
+        // fixed 6e-8 relative, i.e. a velocity drift of 7.6e-8 per step (1e-4 after 1300 steps on the
+        // Taylor-Green case).  Therefore: the weights enter as the exact integers 36 w_i (powers
+        // of two on all moving directions), omega / 36 multiplies the three per-node scalars as a
+        // two-term sum hi + lo (rounding then depends on the node's data, not on a constant), and
+        // the old value is scaled by keep = 1 - omega, which set_bgk makes exact for the omega in use.
+        const T keep = rp.keep;
+        const T vv = v[0] * v[0] + v[1] * v[1] + v[2] * v[2];
+        const T b0 = drho - rho * (T(1.5) * vv), q0 = T(4.5) * rho;
+        const T base = b0 * rp.om36_hi + b0 * rp.om36_lo;
+        const T r45 = q0 * rp.om36_hi + q0 * rp.om36_lo;
+        // odd part: omega w_i 3 rho (e_i . v) = 36 w_i e_i . m3 with m3 = (omega / 12) * (rho v),
+        // and rho v = j + F/2 is taken from the moments directly (no round trip through 1/rho),
+        // so that sum_i e_i f_i^eq reproduces it up to unbiased rounding.
+        T m3[3], Fs[3] = {T(0), T(0), T(0)}, vF3 = T(0);
+#pragma unroll
+        for (int a = 0; a < 3; a++) {
+            const T t = T(3) * rv[a];
+            m3[a] = t * rp.om36_hi + t * rp.om36_lo;
         }
+        if constexpr (FORCE) {
+#pragma unroll
+            for (int a = 0; a < 3; a++) Fs[a] = F[a] * rp.sc36_hi + F[a] * rp.sc36_lo;
+            vF3 = T(3) * (v[0] * Fs[0] + v[1] * Fs[1] + v[2] * Fs[2]);
+        }
+        h[0] = keep * h[0] + T(L::w36(0)) * (base - vF3);
 #pragma unroll
         for (int i = 1; i < Q; i++) {
             if (i < L::opp(i)) {
                 const int j = L::opp(i);
-                const T wo = om * L::template w<T>(i);
+                const T wi = T(L::w36(i));
                 const T ev = e_dot<L, T>(i, v);
-                T even = wo * (base + r45 * ev * ev);
-                T odd = wo * (r3 * ev);
+                T even = base + r45 * ev * ev;
+                T odd = e_dot<L, T>(i, m3);
                 if constexpr (FORCE) {
-                    const T ws = sc * L::template w<T>(i);
-                    const T eF = e_dot<L, T>(i, F);
-                    even += ws * (T(9) * ev * eF - vF3);
-                    odd += ws * (T(3) * eF);
+                    const T eF = e_dot<L, T>(i, Fs);
+                    even += T(9) * ev * eF - vF3;
+                    odd += T(3) * eF;
                 }
-                h[i] = keep * h[i] + (even + odd);
-                h[j] = keep * h[j] + (even - odd);
+                h[i] = keep * h[i] + wi * (even + odd);
+                h[j] = keep * h[j] + wi * (even - odd);
             }
         }
     } else {
@@ -287,13 +324,14 @@ LBM_HD void update_node(T (&h)[L::Q], const Relax<T> &rp) {
         T drho, j[3];
         moments<L, T>(h, drho, j);
         const T rho = T(1) + drho, inv_rho = T(1) / rho;
-        T v[3], F[3];
+        T v[3], rv[3], F[3];
 #pragma unroll
         for (int a = 0; a < 3; a++) {
             F[a] = FORCE ? rho * rp.g[a] : T(0);
-            v[a] = FORCE ? (j[a] + T(0.5) * F[a]) * inv_rho : j[a] * inv_rho;
+            rv[a] = FORCE ? j[a] + T(0.5) * F[a] : j[a];
+            v[a] = rv[a] * inv_rho;
         }
-        collide<L, T, MRT, FORCE>(h, rho, drho, v, F, rp);
+        collide<L, T, MRT, FORCE>(h, rho, drho, v, rv, F, rp);
     }
 }
 

@@ -9,8 +9,7 @@ using namespace lbm;
 template <class L, typename T, bool MRT, bool FORCE>
 static void run(const double *f, double tau, const double *rates, const double *g, double *out) {
     Relax<T> rp{};
-    rp.inv_tau = T(1.0 / tau);
-    rp.src_scale = T(1.0 - 0.5 / tau);
+    set_bgk(rp, tau);
     for (int a = 0; a < 3; a++) rp.g[a] = T(g[a]);
     for (int k = 0; k < L::Q; k++) {
         rp.cr[k] = T(rates[k] / Mrt<L, double>::norm(k));

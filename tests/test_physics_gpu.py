@@ -1,0 +1,128 @@
+"""Physics checks at the full length of the BASELINE.json configs, from lbm_macro output (tier T3 of
+SURVEY.md section 4): Taylor-Green decay (c1, 1000 steps), Shan-Chen component mass and total
+momentum (c5, 1000 steps at 256^3), uniform-force closed form, Poiseuille profile."""
+import numpy as np
+import pytest
+
+from paper_1311_2404_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    assert torch.cuda.is_available()
+    from paper_1311_2404_b200 import binding
+    binding.load()
+    return binding
+
+
+def start(B, w, **kw):
+    sim = B.from_workload(w, **kw)
+    sim.set_geometry(w.mask)
+    for s in range(w.ncomp):
+        sim.init_equilibrium(w.rho[s], w.u[s], comp=s)
+    return sim
+
+
+def energy(rho, u):
+    return 0.5 * float((u.double() ** 2).sum())
+
+
+@pytest.mark.parametrize("store", ["ab", "aa"])
+def test_c1_taylor_green_energy_decay_1000_steps(B, orc, store):
+    """c1: sqrt(E(t)/E(0)) follows exp(-2 nu k^2 t), nu = (tau - 1/2)/3 (eq. 19, P:472-474;
+    reading A10), within 1e-3 relative at t = 1000; and the fp32 GPU energy equals the fp64
+    oracle's within 1e-5 relative."""
+    w = W.c1_taylor_green()
+    sim = start(B, w, store=B.LBM_STORE_AA if store == "aa" else B.LBM_STORE_AB)
+    ref = orc.Oracle(**w.params())
+    ref.init_equilibrium(w.rho[0], w.u[0])
+    e0 = energy(*sim.macro())
+    sim.step(1000)
+    ref.step(1000)
+    e1 = energy(*sim.macro())
+    nu, k = (0.8 - 0.5) / 3.0, 2.0 * np.pi / 128
+    assert abs(np.sqrt(e1 / e0) / np.exp(-2.0 * nu * k * k * 1000) - 1.0) < 1e-3
+    rho_r, u_r = ref.macro()
+    e_ref = 0.5 * float((u_r ** 2).sum())
+    assert abs(e1 / e_ref - 1.0) < 1e-5
+
+
+def test_c5_full_size_mass_and_momentum_conserved_1000_steps(B):
+    """c5 as configured (256^3, 1000 steps): mass of each component is conserved (reading A8
+    permutation + sum of source = 0) and total momentum stays zero (A13), up to fp32 round-off."""
+    import torch
+    w = W.c5_shan_chen()
+    sim = start(B, w)
+    N = w.sites
+
+    def totals():
+        out = []
+        for s in range(2):
+            rho, u = sim.macro(s)
+            out.append((float(rho.double().sum()), (rho.double() * u.double()).sum(dim=(1, 2, 3)).cpu().numpy()))
+        return out
+
+    (ma0, ja0), (mb0, jb0) = totals()
+    sim.step(1000)
+    (ma1, ja1), (mb1, jb1) = totals()
+    assert abs(ma1 / ma0 - 1.0) < 5e-6 and abs(mb1 / mb0 - 1.0) < 5e-6
+    # bare component momenta differ from the physical one by the half-force term, which sums to zero
+    assert np.abs(ja1 + jb1).max() / N < 1e-7
+    rho_a, _ = sim.macro(0)
+    assert bool(torch.isfinite(rho_a).all())
+    # spinodal decomposition under the repulsive sign of reading A11: the contrast grows
+    assert float(rho_a.std()) > 0.01 * 3 ** -0.5 * 2
+
+
+@pytest.mark.parametrize("lattice,model,precision", [(W.D2Q9, W.BGK, W.F32), (W.D3Q19, W.BGK, W.F64),
+                                                     (W.D3Q19, W.MRT, W.F64)])
+def test_uniform_force_closed_form(B, lattice, model, precision):
+    """Uniform state on a torus, body acceleration g: lbm_macro velocity after n steps is
+    u0 + (n + 1/2) g exactly (eq. 16; readings A13, A15)."""
+    shape = (12, 10, 1) if lattice == W.D2Q9 else (8, 6, 5)
+    nx, ny, nz = shape
+    D = 2 if lattice == W.D2Q9 else 3
+    g = (1e-5, -2e-5, 0.0) if D == 2 else (1e-5, -2e-5, 3e-5)
+    u0 = (0.01, 0.02, -0.015)[:D]
+    rates = (W.mrt_rates_d3q19(0.8) if lattice == W.D3Q19 else W.mrt_rates_d2q9(0.8)) if model == W.MRT else None
+    sim = B.Lbm(lattice, model, precision, nx, ny, nz, tau=0.8, force=g, rates=rates)
+    rho = np.ones((nz, ny, nx))
+    u = np.zeros((D, nz, ny, nx))
+    for a in range(D):
+        u[a] = u0[a]
+    sim.init_equilibrium(rho, u)
+    n = 37
+    sim.step(n)
+    _, v = sim.macro()
+    tol = 2e-7 if precision == W.F32 else 1e-14
+    for a in range(D):
+        assert abs(float(v[a].double().mean()) - (u0[a] + (n + 0.5) * g[a])) < tol
+        assert float((v[a].double() - v[a].double().mean()).abs().max()) < tol
+
+
+def test_poiseuille_profile_parabola_plus_constant(B):
+    """Steady force-driven channel with half-way bounce-back walls (A8): the profile is the
+    parabola g/(2 nu) (y - 1/2)(ny - 3/2 - y) plus a constant slip; checked through second
+    differences (which remove the constant) and the wall position (symmetry)."""
+    nx, ny, nz, tau, g = 4, 34, 1, 0.8, 1e-6
+    nu = (tau - 0.5) / 3.0
+    mask = np.zeros((1, ny, nx), np.uint8)
+    mask[:, 0, :] = 1
+    mask[:, ny - 1, :] = 1
+    sim = B.Lbm(W.D2Q9, W.BGK, W.F64, nx, ny, nz, tau=tau, force=(g, 0.0, 0.0))
+    sim.set_geometry(mask)
+    sim.init_equilibrium(np.ones((1, ny, nx)), np.zeros((2, 1, ny, nx)))
+    sim.step(40000)  # diffusion time H^2 / nu ~ 1e4 steps
+    _, u = sim.macro()
+    ux = u[0, 0, 1:ny - 1, 0].double().cpu().numpy()
+    second = ux[2:] - 2 * ux[1:-1] + ux[:-2]
+    assert np.abs(second / (-g / nu) - 1.0).max() < 1e-6
+    assert np.abs(ux - ux[::-1]).max() < 1e-12 * ux.max() + 1e-18
+    y = np.arange(1, ny - 1)
+    parab = g / (2 * nu) * (y - 0.5) * (ny - 1.5 - y)
+    slip = ux - parab
+    assert np.ptp(slip) < 1e-6 * ux.max()
+    assert abs(slip.mean() - g * (48 * nu * nu - 1) / (8 * nu)) < 1e-6 * ux.max()
