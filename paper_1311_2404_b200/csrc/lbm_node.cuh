@@ -237,31 +237,36 @@ LBM_HD void collide(T (&h)[L::Q], T rho, T drho, const T (&v)[3], const T (&rv)[
         // odd part: omega w_i 3 rho (e_i . v) = 36 w_i e_i . m3 with m3 = (omega / 12) * (rho v),
         // and rho v = j + F/2 is taken from the moments directly (no round trip through 1/rho),
         // so that sum_i e_i f_i^eq reproduces it up to unbiased rounding.
-        T m3[3], Fs[3] = {T(0), T(0), T(0)}, vF3 = T(0);
+        // With a force the source of eq. (17) folds into the same two sums: the odd part gains
+        // 3 e_i.F' and the even part 9 (e_i.v)(e_i.F') - 3 v.F', F' = (1 - omega/2) F / 36.
+        T mo[3], F9[3] = {T(0), T(0), T(0)}, base_f = base;
 #pragma unroll
         for (int a = 0; a < 3; a++) {
             const T t = T(3) * rv[a];
-            m3[a] = t * rp.om36_hi + t * rp.om36_lo;
+            mo[a] = t * rp.om36_hi + t * rp.om36_lo;
         }
         if constexpr (FORCE) {
+            T vF = T(0);
 #pragma unroll
-            for (int a = 0; a < 3; a++) Fs[a] = F[a] * rp.sc36_hi + F[a] * rp.sc36_lo;
-            vF3 = T(3) * (v[0] * Fs[0] + v[1] * Fs[1] + v[2] * Fs[2]);
+            for (int a = 0; a < 3; a++) {
+                const T Fs = F[a] * rp.sc36_hi + F[a] * rp.sc36_lo;
+                mo[a] += T(3) * Fs;
+                F9[a] = T(9) * Fs;
+                vF += v[a] * Fs;
+            }
+            base_f = base - T(3) * vF;
         }
-        h[0] = keep * h[0] + T(L::w36(0)) * (base - vF3);
+        h[0] = keep * h[0] + T(L::w36(0)) * base_f;
 #pragma unroll
         for (int i = 1; i < Q; i++) {
             if (i < L::opp(i)) {
                 const int j = L::opp(i);
                 const T wi = T(L::w36(i));
                 const T ev = e_dot<L, T>(i, v);
-                T even = base + r45 * ev * ev;
-                T odd = e_dot<L, T>(i, m3);
-                if constexpr (FORCE) {
-                    const T eF = e_dot<L, T>(i, Fs);
-                    even += T(9) * ev * eF - vF3;
-                    odd += T(3) * eF;
-                }
+                const T odd = e_dot<L, T>(i, mo);
+                T even;
+                if constexpr (FORCE) even = base_f + ev * (r45 * ev + e_dot<L, T>(i, F9));
+                else even = base_f + r45 * ev * ev;
                 h[i] = keep * h[i] + wi * (even + odd);
                 h[j] = keep * h[j] + wi * (even - odd);
             }
