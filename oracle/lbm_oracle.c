@@ -58,6 +58,8 @@ enum { ORC_D2Q9 = 0, ORC_D3Q19 = 1 };
 enum { ORC_BGK = 0, ORC_MRT = 1, ORC_SC2 = 2 };
 enum { ORC_PSI_RHO = 0, ORC_PSI_1MEXP = 1 };
 #define ORC_QMAX 19
+/* node types (P:446 reduced; readings A8, A20, A21) */
+enum { ORC_FLUID = 0, ORC_SOLID = 1, ORC_WALL_FULLWAY = 2, ORC_VELOCITY = 3 };
 
 typedef struct {
     int32_t lattice, model;
@@ -67,6 +69,7 @@ typedef struct {
     double force[3]; /* body acceleration g; F = rho g */
     double sc_G;
     int32_t sc_psi;
+    double bc_velocity[3]; /* velocity imposed on ORC_VELOCITY nodes (reading A21) */
 } orc_params;
 
 /* ---- velocity sets (reading A2; weights from Table 1) ------------- */
@@ -193,7 +196,7 @@ typedef struct {
     lattice_t L;
     int64_t N;
     int ncomp;
-    uint8_t *mask;        /* N, 0 FLUID / 1 SOLID */
+    uint8_t *mask;        /* N, node type ORC_FLUID / SOLID / WALL_FULLWAY / VELOCITY */
     double *f[2];         /* per component: Q*N, canonical pre-collision state */
     double *fs[2];        /* per component: Q*N, post-collision f*            */
     double *rho[2];       /* Shan-Chen: per-component density field           */
@@ -292,7 +295,9 @@ orc_ctx *orc_create(const orc_params *p)
 
 int orc_set_geometry(orc_ctx *c, const uint8_t *mask)
 {
-    for (int64_t n = 0; n < c->N; n++) c->mask[n] = mask[n] ? 1 : 0;
+    /* 0, 2, 3 as named; every other value is a dry SOLID node */
+    for (int64_t n = 0; n < c->N; n++)
+        c->mask[n] = (mask[n] == ORC_FLUID || mask[n] == ORC_WALL_FULLWAY || mask[n] == ORC_VELOCITY) ? mask[n] : ORC_SOLID;
     return 0;
 }
 
@@ -334,10 +339,10 @@ int orc_stream_map(const orc_ctx *c, int64_t *map)
             for (int x = 0; x < nx; x++) {
                 int64_t n = node_index(c, x, y, z);
                 for (int i = 0; i < Q; i++) {
-                    if (c->mask[n]) { map[i * c->N + n] = -1; continue; }
+                    if (c->mask[n] == ORC_SOLID) { map[i * c->N + n] = -1; continue; }
                     int64_t m = node_index(c, wrap(x - c->L.e[i][0], nx), wrap(y - c->L.e[i][1], ny),
                                            wrap(z - c->L.e[i][2], nz));
-                    map[i * c->N + n] = c->mask[m] ? (int64_t)c->L.opp[i] * c->N + n : (int64_t)i * c->N + m;
+                    map[i * c->N + n] = c->mask[m] == ORC_SOLID ? (int64_t)c->L.opp[i] * c->N + n : (int64_t)i * c->N + m;
                 }
             }
     return 0;
@@ -386,6 +391,27 @@ static void collide_node(const orc_ctx *c, const double *f, double rho, const do
     }
 }
 
+/* ---- boundary nodes that replace the collision (readings A20, A21) -------------------------
+ * WALL_FULLWAY (Fig. 2 (1)): a dry node that only stores the populations streamed into it
+ *   and scatters them back: f*_i = f_ibar, no relaxation; they return to the fluid one step later.
+ * VELOCITY (equilibrium velocity boundary): the node is wet; its incoming populations are
+ *   the streamed ones, the missing ones (from SOLID neighbours) equal their opposites, which is
+ *   exactly the half-way rule of stream(); rho is computed from them and the post-collision
+ *   state is f^eq(rho, u_bc).
+ * Returns 1 if the node type was handled here. */
+static int special_node(const orc_ctx *c, int type, const double *f, double rho, double *fstar)
+{
+    if (type == ORC_WALL_FULLWAY) {
+        for (int i = 0; i < c->L.Q; i++) fstar[i] = f[c->L.opp[i]];
+        return 1;
+    }
+    if (type == ORC_VELOCITY) {
+        feq(&c->L, rho, c->p.bc_velocity, fstar);
+        return 1;
+    }
+    return 0;
+}
+
 /* ---- streaming with half-way bounce-back: f <- stream(f*) (step 5 of DESIGN.md) ---------- */
 static void stream(orc_ctx *c, int comp)
 {
@@ -397,11 +423,11 @@ static void stream(orc_ctx *c, int comp)
         for (int y = 0; y < ny; y++)
             for (int x = 0; x < nx; x++) {
                 int64_t n = node_index(c, x, y, z);
-                if (c->mask[n]) continue;
+                if (c->mask[n] == ORC_SOLID) continue;
                 for (int i = 0; i < Q; i++) {
                     int64_t m = node_index(c, wrap(x - c->L.e[i][0], nx), wrap(y - c->L.e[i][1], ny),
                                            wrap(z - c->L.e[i][2], nz));
-                    f[i * c->N + n] = c->mask[m] ? fs[c->L.opp[i] * c->N + n] : fs[i * c->N + m];
+                    f[i * c->N + n] = c->mask[m] == ORC_SOLID ? fs[c->L.opp[i] * c->N + n] : fs[i * c->N + m];
                 }
             }
 }
@@ -412,13 +438,17 @@ static void step_single(orc_ctx *c)
     const int64_t N = c->N;
 #pragma omp parallel for schedule(static)
     for (int64_t n = 0; n < N; n++) {
-        if (c->mask[n]) continue;
+        if (c->mask[n] == ORC_SOLID) continue;
         double f[ORC_QMAX], fstar[ORC_QMAX];
         double rho = 0, j[3] = {0, 0, 0}, F[3], v[3];
         for (int i = 0; i < Q; i++) {
             f[i] = c->f[0][i * N + n];
             rho += f[i];                                               /* eq. (1) */
             for (int a = 0; a < 3; a++) j[a] += f[i] * c->L.e[i][a];
+        }
+        if (special_node(c, c->mask[n], f, rho, fstar)) {
+            for (int i = 0; i < Q; i++) c->fs[0][i * N + n] = fstar[i];
+            continue;
         }
         for (int a = 0; a < 3; a++) {
             F[a] = rho * c->p.force[a];                                /* F = rho g (A4) */
@@ -441,7 +471,8 @@ static void sc_force_node(const orc_ctx *c, int s, int x, int y, int z, double F
     for (int i = 0; i < c->L.Q; i++) {
         int64_t m = node_index(c, wrap(x + c->L.e[i][0], nx), wrap(y + c->L.e[i][1], ny),
                                wrap(z + c->L.e[i][2], nz));
-        double ps = c->mask[m] ? 0.0 : psi_of(c->p.sc_psi, c->rho[o][m]);
+        int dry = c->mask[m] == ORC_SOLID || c->mask[m] == ORC_WALL_FULLWAY; /* A14 */
+        double ps = dry ? 0.0 : psi_of(c->p.sc_psi, c->rho[o][m]);
         for (int a = 0; a < 3; a++) acc[a] += c->L.w[i] * ps * c->L.e[i][a];
     }
     double p0 = psi_of(c->p.sc_psi, c->rho[s][n]);
@@ -456,7 +487,7 @@ static void sc_macro_fields(orc_ctx *c)
 #pragma omp parallel for schedule(static)
         for (int64_t n = 0; n < N; n++) {
             double rho = 0, j[3] = {0, 0, 0};
-            if (!c->mask[n])
+            if (c->mask[n] != ORC_SOLID)
                 for (int i = 0; i < Q; i++) {
                     double fi = c->f[s][i * N + n];
                     rho += fi;
@@ -478,7 +509,16 @@ static void step_sc2(orc_ctx *c)
         for (int y = 0; y < ny; y++)
             for (int x = 0; x < nx; x++) {
                 int64_t n = node_index(c, x, y, z);
-                if (c->mask[n]) continue;
+                if (c->mask[n] == ORC_SOLID) continue;
+                if (c->mask[n] != ORC_FLUID) {
+                    for (int s = 0; s < 2; s++) {
+                        double f[ORC_QMAX], fstar[ORC_QMAX];
+                        for (int i = 0; i < Q; i++) f[i] = c->f[s][i * N + n];
+                        special_node(c, c->mask[n], f, c->rho[s][n], fstar);
+                        for (int i = 0; i < Q; i++) c->fs[s][i * N + n] = fstar[i];
+                    }
+                    continue;
+                }
                 const double tA = c->p.tau[0], tB = c->p.tau[1];
                 double den = c->rho[0][n] / tA + c->rho[1][n] / tB, up[3];
                 for (int a = 0; a < 3; a++)                            /* (ii) */
@@ -518,7 +558,7 @@ int orc_macro(const orc_ctx *c, int comp, double *rho_out, double *u_out)
     const int64_t N = c->N;
     for (int64_t n = 0; n < N; n++) {
         double rho = 0, j[3] = {0, 0, 0};
-        if (c->mask[n]) {
+        if (c->mask[n] == ORC_SOLID || c->mask[n] == ORC_WALL_FULLWAY) { /* dry nodes */
             rho_out[n] = 0.0;
             for (int a = 0; a < D; a++) u_out[a * N + n] = 0.0;
             continue;
@@ -547,7 +587,7 @@ int orc_sc_force(orc_ctx *c, int comp, double *F_out)
             for (int x = 0; x < c->p.nx; x++) {
                 int64_t n = node_index(c, x, y, z);
                 double F[3] = {0, 0, 0};
-                if (!c->mask[n]) sc_force_node(c, comp, x, y, z, F);
+                if (c->mask[n] == ORC_FLUID) sc_force_node(c, comp, x, y, z, F);
                 for (int a = 0; a < 3; a++) F_out[a * c->N + n] = F[a];
             }
     return 0;

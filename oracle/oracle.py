@@ -18,6 +18,7 @@ _SRC = os.path.join(_HERE, "lbm_oracle.c")
 _LIB = os.path.join(_HERE, "liblbm_oracle.so")
 
 D2Q9, D3Q19 = 0, 1
+FLUID, SOLID, WALL_FULLWAY, VELOCITY = 0, 1, 2, 3
 BGK, MRT, SC2 = 0, 1, 2
 PSI_RHO, PSI_1MEXP = 0, 1
 QMAX = 19
@@ -32,6 +33,7 @@ class _Params(C.Structure):
         ("force", C.c_double * 3),
         ("sc_G", C.c_double),
         ("sc_psi", C.c_int32),
+        ("bc_velocity", C.c_double * 3),
     ]
 
 
@@ -109,7 +111,7 @@ class Oracle:
     """One oracle simulation.  Arrays are C-order [z][y][x]; u is [D][z][y][x]; f is [Q][z][y][x]."""
 
     def __init__(self, lattice, model, nx, ny, nz=1, tau=(1.0, 1.0), rates=None,
-                 force=(0.0, 0.0, 0.0), sc_G=0.0, sc_psi=PSI_RHO):
+                 force=(0.0, 0.0, 0.0), sc_G=0.0, sc_psi=PSI_RHO, bc_velocity=(0.0, 0.0, 0.0)):
         p = _Params()
         p.lattice, p.model = lattice, model
         p.nx, p.ny, p.nz = nx, ny, nz
@@ -121,6 +123,8 @@ class Oracle:
         for a in range(3):
             p.force[a] = float(force[a]) if a < len(force) else 0.0
         p.sc_G, p.sc_psi = float(sc_G), int(sc_psi)
+        for a in range(3):
+            p.bc_velocity[a] = float(bc_velocity[a]) if a < len(bc_velocity) else 0.0
         self._h = lib().orc_create(C.byref(p))
         if not self._h:
             raise ValueError("orc_create rejected the parameters")

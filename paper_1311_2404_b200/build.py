@@ -43,7 +43,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     """Compile the library if it is missing or older than its sources; return its path."""
     if force or stale():
         os.makedirs(OBJDIR, exist_ok=True)
-        extra = ["-Xptxas", "-v"] if verbose else []
+        extra = (["-Xptxas", "-v"] if verbose else []) + os.environ.get("LBM_NVCC_EXTRA", "").split()
         objs, procs = [], []
         for src in SOURCES:  # the translation units are independent: compile them side by side
             obj = os.path.join(OBJDIR, os.path.basename(src)[:-3] + ".o")

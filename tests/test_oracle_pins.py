@@ -508,3 +508,165 @@ def test_shan_chen_repulsive_sign_demixes(orc):
     d1 = np.std(o.macro(0)[0] - o.macro(1)[0])
     assert d1 > 5 * d0
     assert np.isfinite(o.get_distributions(0)).all()
+
+
+# ---------------------------------------------------------------- NEXT-2: full-way bounce-back walls and the
+# equilibrium-velocity boundary (Fig. 2 (1); readings A20, A21)
+def test_fullway_wall_returns_populations_two_steps_later(orc):
+    """Fig. 2 (1): a population streamed into a full-way wall node at t+1 is reversed there
+    (no relaxation) and is back at the originating node at t+2, opposite direction.  tau = 1 in a
+    uniform rest state makes the fluid collision a no-op on the marked population's neighbours
+    except for relaxing towards equilibrium, so track total mass instead of one arrow: mass inside
+    the wall layer after one step equals what streamed in, and total mass is conserved for ever."""
+    nx, ny = 6, 7
+    o = orc.Oracle(0, 0, nx, ny, 1, tau=0.8)
+    mask = np.zeros((1, ny, nx), np.uint8)
+    mask[:, 0, :] = orc.WALL_FULLWAY
+    mask[:, ny - 1, :] = orc.WALL_FULLWAY
+    o.set_geometry(mask)
+    rng = np.random.default_rng(3)
+    rho = 1 + rng.uniform(-0.01, 0.01, (1, ny, nx))
+    u = rng.uniform(-0.02, 0.02, (2, 1, ny, nx))
+    u[:, mask == orc.WALL_FULLWAY] = 0
+    o.init_equilibrium(rho, u)
+    f0 = o.get_distributions()
+    m0 = f0.sum()
+    for _ in range(50):
+        o.step(1)
+        assert abs(o.get_distributions().sum() - m0) < 1e-12 * m0
+    # one hand-tracked arrow: direction 2 (+y) leaving the top fluid row enters the wall row at
+    # t+1, is stored there as direction 2, reversed by the wall "collision", and arrives back in
+    # the top fluid row as direction 4 (-y) at t+2 with exactly the same value.
+    o2 = orc.Oracle(0, 0, nx, ny, 1, tau=1.0)
+    o2.set_geometry(mask)
+    o2.init_equilibrium(np.ones((1, ny, nx)), np.zeros((2, 1, ny, nx)))
+    f = o2.get_distributions()
+    f[2, 0, ny - 2, 3] += 1e-3                     # pre-collision bump at the top fluid row
+    o2.set_distributions(f)
+    ref = orc.Oracle(0, 0, nx, ny, 1, tau=1.0)     # same without the bump
+    ref.set_geometry(mask)
+    ref.init_equilibrium(np.ones((1, ny, nx)), np.zeros((2, 1, ny, nx)))
+    o2.step(1); ref.step(1)
+    d1 = o2.get_distributions() - ref.get_distributions()
+    in_wall = d1[:, 0, ny - 1, :].sum()
+    assert in_wall > 0                               # part of the bump now sits in the dry wall row
+    o2.step(1); ref.step(1)
+    d2 = o2.get_distributions() - ref.get_distributions()
+    # after the reversal step nothing of the perturbation remains in the wall row except what
+    # streamed in during this step; what was there is back in the fluid, travelling downwards
+    assert abs(d2[:, 0, :ny - 1, :].sum() + d2[:, 0, ny - 1, :].sum() - 1e-3) < 1e-15
+    back = d2[[4, 7, 8], 0, ny - 2, :].sum()       # -y directions in the top fluid row
+    assert abs(back - in_wall) < 1e-15
+
+
+@pytest.mark.parametrize("lat", [0, 1])
+def test_fullway_walls_steady_poiseuille_equals_halfway(orc, lat):
+    """In steady state the one-step delay of the full-way wall is invisible: the profile equals the
+    half-way bounce-back profile with the wall nodes at the same places ("the physical wall is
+    effectively located between the last fluid node and the wall node")."""
+    g, tau, H = 1e-6, 0.8, 12
+    ny = H + 2
+    shp = (3, ny, 1) if lat == 0 else (3, ny, 3)
+    prof = []
+    for wall in (orc.SOLID, orc.WALL_FULLWAY):
+        o = orc.Oracle(lat, 0, *shp, tau=tau, force=(g, 0, 0))
+        mask = np.zeros(o.shape, np.uint8)
+        mask[:, 0, :] = wall
+        mask[:, ny - 1, :] = wall
+        o.set_geometry(mask)
+        o.init_equilibrium(*_uniform(o, 1.0, (0, 0, 0)))
+        o.step(30000)
+        r, v = o.macro()
+        assert np.all(r[:, 0, :] == 0) and np.all(v[:, :, 0, :] == 0)      # dry nodes report nothing
+        prof.append(v[0][0, 1:ny - 1, 1])
+    assert np.max(np.abs(prof[0] - prof[1])) < 1e-9 * prof[0].max()
+
+
+def test_velocity_node_uniform_flow_is_a_fixed_point(orc):
+    """Equilibrium-velocity node: post-collision state f^eq(rho, u_bc) with rho from the
+    node's own populations.  In a uniform flow at u_bc it changes nothing."""
+    ubc = (0.03, -0.01, 0.02)
+    o = orc.Oracle(1, 0, 5, 4, 3, tau=0.7, bc_velocity=ubc)
+    mask = np.zeros(o.shape, np.uint8)
+    mask[1, 2, :] = orc.VELOCITY
+    mask[0, 1, 3] = orc.VELOCITY
+    o.set_geometry(mask)
+    o.init_equilibrium(*_uniform(o, 1.1, ubc))
+    f0 = o.get_distributions().copy()
+    o.step(25)
+    assert np.max(np.abs(o.get_distributions() - f0)) < 1e-15
+
+
+def test_velocity_lid_drives_couette_flow(orc):
+    """Channel: half-way wall at the bottom, equilibrium-velocity lid (backed by a SOLID row, so its
+    missing populations are bounce-back copies) moving at U.  Steady state: the lid row
+    moves at U; every interior row obeys the discrete Laplace equation, i.e. the profile is exactly
+    linear between the first and the last interior row; its slope is U / H to first order."""
+    U, tau, ny = 0.02, 0.8, 20
+    o = orc.Oracle(0, 0, 3, ny, 1, tau=tau, bc_velocity=(U, 0, 0))
+    mask = np.zeros(o.shape, np.uint8)
+    mask[:, 0, :] = orc.SOLID
+    mask[:, ny - 2, :] = orc.VELOCITY
+    mask[:, ny - 1, :] = orc.SOLID
+    o.set_geometry(mask)
+    o.init_equilibrium(*_uniform(o, 1.0, (0, 0, 0)))
+    o.step(20000)
+    r, v = o.macro()
+    ux = v[0][0, 1:ny - 1, 1]                      # rows 1 .. ny-2 (the last one is the lid)
+    interior = ux[:-1]
+    second = interior[2:] - 2 * interior[1:-1] + interior[:-2]
+    assert np.max(np.abs(second)) < 1e-12
+    assert np.max(np.abs(v[1])) < 1e-12            # no wall-normal flow
+    slope = interior[1] - interior[0]
+    H = (ny - 2) - 0.5                             # bottom wall plane at y = 1/2, lid node at y = ny-2
+    assert abs(slope / (U / H) - 1.0) < 0.05
+    assert abs(interior[0] / (0.5 * slope) - 1.0) < 0.02   # no-slip plane half a link below row 1
+    # the lid row itself reports the velocity of its INCOMING populations (lbm_macro is pre-collision),
+    # which is below U; the interior line extrapolated to the lid row recovers U to first order
+    assert abs((interior[-1] + slope) / U - 1.0) < 0.05 and 0 < ux[-1] < U
+
+
+@pytest.mark.parametrize("lat,shp", [(0, (7, 6, 1)), (1, (5, 6, 4))])
+def test_step_with_all_node_types_against_numpy_roll_reference(orc, lat, shp):
+    """Independent whole-array numpy re-implementation with all four node types."""
+    from paper_1311_2404_b200 import workloads as W
+    nx, ny, nz = shp
+    e, w, opp = orc.lattice_tables(lat)
+    Q, D = len(e), (2 if lat == 0 else 3)
+    _, rho, u = W.random_state(lat, nx, ny, nz, seed=31)
+    rng = np.random.default_rng(32)
+    mask = rng.choice(np.array([0, 0, 0, 1, 2, 3], np.uint8), size=(nz, ny, nx))
+    tau, g = 0.9, np.array([1e-4, -2e-4, 3e-4 if D == 3 else 0.0])
+    ubc = np.array([0.02, -0.01, 0.015 if D == 3 else 0.0])
+    o = orc.Oracle(lat, 0, nx, ny, nz, tau=tau, force=g, bc_velocity=ubc)
+    o.set_geometry(mask)
+    o.init_equilibrium(rho[0], u[0])
+    f = o.get_distributions().copy()
+    ef = e.astype(float)
+    live = mask != 1
+    for _ in range(10):
+        r = f.sum(0)
+        j = np.einsum("qzyx,qa->azyx", f, ef)
+        v = j / r + 0.5 * g[:, None, None, None]
+        ev = np.einsum("qa,azyx->qzyx", ef, v)
+        fe = r * w[:, None, None, None] * (1 + 3 * ev + 4.5 * ev ** 2 - 1.5 * (v ** 2).sum(0))
+        eg = ef @ g
+        vg = np.einsum("a,azyx->zyx", g, v)
+        src = w[:, None, None, None] * r * (3 * (eg[:, None, None, None] - vg) + 9 * ev * eg[:, None, None, None])
+        fs = f + (fe - f) / tau + (1 - 0.5 / tau) * src
+        eb = ef @ ubc
+        fbc = r * w[:, None, None, None] * (1 + 3 * eb[:, None, None, None] + 4.5 * eb[:, None, None, None] ** 2
+                                             - 1.5 * (ubc ** 2).sum())
+        fs = np.where(mask == 2, f[opp], fs)        # full-way wall: reverse, no relaxation
+        fs = np.where(mask == 3, fbc, fs)           # equilibrium-velocity node
+        new = f.copy()
+        for i in range(Q):
+            sh = (e[i][2], e[i][1], e[i][0])
+            moved = np.roll(fs[i], shift=sh, axis=(0, 1, 2))
+            from_solid = np.roll(mask, shift=sh, axis=(0, 1, 2)) == 1
+            new[i] = np.where(live, np.where(from_solid, fs[opp[i]], moved), f[i])
+        f = new
+    o.step(10)
+    got = o.get_distributions()
+    assert np.max(np.abs(got - f)[:, live]) < 1e-14
+    assert np.array_equal(got[:, ~live], f[:, ~live])
