@@ -38,6 +38,18 @@ enum { LBM_BGK = 0, LBM_MRT = 1, LBM_SC2 = 2 };  /* model: SC2 = two LBGK compon
 enum { LBM_F32 = 0, LBM_F64 = 1 };               /* precision of storage and arithmetic      */
 enum { LBM_PSI_RHO = 0, LBM_PSI_1MEXP = 1 };     /* psi(rho) = rho | 1 - exp(-rho)   */
 enum { LBM_STORE_AB = 0, LBM_STORE_AA = 1 };     /* two copies | in-place AA */
+/* node types of the lbm_set_geometry mask (P:446 reduced to what the path needs):
+ *   FLUID         wet, collides
+ *   SOLID         dry; a pull from it returns the puller's own opposite post-collision population
+ *                 in the same step (half-way bounce-back, reading A8)
+ *   WALL_FULLWAY  dry; stores the populations streamed into it and scatters them back reversed,
+ *                 without relaxation, so they return one step later (full-way bounce-back,
+ *                 Fig. 2 (1), reading A20)
+ *   VELOCITY      wet; post-collision state f^eq(rho, bc_velocity) with rho from its own incoming
+ *                 populations, missing ones = bounce-back copies, i.e. put a SOLID node behind it
+ *                 (equilibrium velocity boundary, reading A21)
+ * Any other byte value is SOLID. */
+enum { LBM_NODE_FLUID = 0, LBM_NODE_SOLID = 1, LBM_NODE_WALL_FULLWAY = 2, LBM_NODE_VELOCITY = 3 };
 
 #define LBM_QMAX 19
 
@@ -56,6 +68,8 @@ typedef struct {
     double sc_G;              /* Shan-Chen coupling G of eq. (10), sign per reading A11    */
     int32_t sc_psi;           /* LBM_PSI_*                                                         */
     int32_t store;            /* LBM_STORE_AB (default 0) | LBM_STORE_AA                           */
+    double bc_velocity[3];    /* velocity imposed on LBM_NODE_VELOCITY nodes (reading A21);
+                                 callers built against the 240-byte struct (no such field) get 0   */
 } lbm_params;
 
 /* Static description of a lattice (Table 1; ordering = reading A2).
@@ -75,12 +89,11 @@ int lbm_workspace_bytes(const lbm_params *p, size_t *bytes);
 int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, void *cuda_stream, lbm_ctx **out);
 int lbm_destroy(lbm_ctx *ctx);
 
-/* Node types (reduced to FLUID/SOLID, reading A8).  d_mask: uint8[nz][ny][nx], 0 = FLUID,
- * non-zero = SOLID.  Builds the internal link encoding (which of the Q pull sources are
+/* Node types.  d_mask: uint8[nz][ny][nx] of LBM_NODE_* values.  Builds the internal link encoding (which of the Q pull sources are
  * reflected).  Must be called before lbm_init_equilibrium / lbm_set_distributions if the
  * geometry is not all-FLUID; calling it afterwards returns LBM_ESTATE. */
 int lbm_set_geometry(lbm_ctx *ctx, const uint8_t *d_mask);
-int lbm_get_geometry(lbm_ctx *ctx, uint8_t *d_mask);          /* writes 0/1 per node */
+int lbm_get_geometry(lbm_ctx *ctx, uint8_t *d_mask);          /* writes LBM_NODE_* per node */
 
 /* f_i(x, 0) = f_i^eq(rho0(x), u0(x)), eq. (3), velocity used as given (A15).
  * d_rho: real[N], d_u: real[D][N].  SOLID nodes are ignored. */
@@ -95,7 +108,7 @@ int lbm_init_equilibrium(lbm_ctx *ctx, int comp, const void *d_rho, const void *
 int lbm_step(lbm_ctx *ctx, int n);
 
 /* rho = sum_i f_i, velocity v of eq. (16) (includes g/2) from the current state.
- * SC2: rho_s and the bare component velocity j_s / rho_s.  SOLID nodes: rho = 0, u = 0.
+ * SC2: rho_s and the bare component velocity j_s / rho_s.  Dry nodes (SOLID, WALL_FULLWAY): rho = 0, u = 0.
  * d_rho: real[N] or NULL, d_u: real[D][N] or NULL. */
 int lbm_macro(lbm_ctx *ctx, int comp, void *d_rho, void *d_u);
 

@@ -19,6 +19,7 @@ LBM_BGK, LBM_MRT, LBM_SC2 = 0, 1, 2
 LBM_F32, LBM_F64 = 0, 1
 LBM_PSI_RHO, LBM_PSI_1MEXP = 0, 1
 LBM_STORE_AB, LBM_STORE_AA = 0, 1
+LBM_NODE_FLUID, LBM_NODE_SOLID, LBM_NODE_WALL_FULLWAY, LBM_NODE_VELOCITY = 0, 1, 2, 3
 LBM_QMAX = 19
 
 EXPORTS = ("lbm_lattice_info", "lbm_workspace_bytes", "lbm_create", "lbm_destroy", "lbm_set_geometry",
@@ -38,6 +39,7 @@ class lbm_params(C.Structure):
         ("sc_G", C.c_double),
         ("sc_psi", C.c_int32),
         ("store", C.c_int32),
+        ("bc_velocity", C.c_double * 3),
     ]
 
 
@@ -84,7 +86,8 @@ def load():
 
 
 def make_params(lattice, model, precision, nx, ny, nz=1, tau=(1.0, 1.0), rates=None,
-                force=(0.0, 0.0, 0.0), sc_G=0.0, sc_psi=LBM_PSI_RHO, store=LBM_STORE_AB) -> lbm_params:
+                force=(0.0, 0.0, 0.0), sc_G=0.0, sc_psi=LBM_PSI_RHO, store=LBM_STORE_AB,
+                bc_velocity=(0.0, 0.0, 0.0)) -> lbm_params:
     p = lbm_params()
     p.struct_size = C.sizeof(lbm_params)
     p.lattice, p.model, p.precision = int(lattice), int(model), int(precision)
@@ -97,6 +100,8 @@ def make_params(lattice, model, precision, nx, ny, nz=1, tau=(1.0, 1.0), rates=N
     for a in range(3):
         p.force[a] = float(force[a]) if a < len(force) else 0.0
     p.sc_G, p.sc_psi, p.store = float(sc_G), int(sc_psi), int(store)
+    for a in range(3):
+        p.bc_velocity[a] = float(bc_velocity[a]) if a < len(bc_velocity) else 0.0
     return p
 
 
@@ -252,4 +257,4 @@ class Lbm:
 def from_workload(w, device="cuda:0", **kw) -> "Lbm":
     """Context for a workloads.Workload (parameters only; arrays are passed separately)."""
     return Lbm(w.lattice, w.model, w.precision, w.nx, w.ny, w.nz, device=device, tau=w.tau, rates=w.rates,
-               force=w.force, sc_G=w.sc_G, sc_psi=w.sc_psi, **kw)
+               force=w.force, sc_G=w.sc_G, sc_psi=w.sc_psi, bc_velocity=w.bc_velocity, **kw)

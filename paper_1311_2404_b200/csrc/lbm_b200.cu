@@ -5,9 +5,13 @@
 
 namespace {
 
+// sizeof(lbm_params) before bc_velocity was appended; such callers get bc_velocity = 0
+constexpr uint32_t LBM_PARAMS_SIZE_V1 = 240;
+
 int validate(const lbm_params *p, int *Q, int *D) {
     if (!p) return fail(nullptr, LBM_EINVAL, "params is NULL");
-    if (p->struct_size != sizeof(lbm_params)) return fail(nullptr, LBM_EINVAL, "struct_size != sizeof(lbm_params)");
+    if (p->struct_size != sizeof(lbm_params) && p->struct_size != LBM_PARAMS_SIZE_V1)
+        return fail(nullptr, LBM_EINVAL, "struct_size is not a known sizeof(lbm_params)");
     if (p->lattice != LBM_D2Q9 && p->lattice != LBM_D3Q19) return fail(nullptr, LBM_EINVAL, "unknown lattice");
     if (p->model < LBM_BGK || p->model > LBM_SC2) return fail(nullptr, LBM_EINVAL, "unknown model");
     if (p->precision != LBM_F32 && p->precision != LBM_F64) return fail(nullptr, LBM_EINVAL, "unknown precision");
@@ -25,6 +29,9 @@ int validate(const lbm_params *p, int *Q, int *D) {
             if (!(p->rates[k] >= 0.0 && p->rates[k] <= 2.0)) return fail(nullptr, LBM_EINVAL, "MRT rates must be in [0, 2]");
     for (int a = 0; a < 3; a++)
         if (!(p->force[a] == p->force[a])) return fail(nullptr, LBM_EINVAL, "force is NaN");
+    if (p->struct_size == sizeof(lbm_params))
+        for (int a = 0; a < 3; a++)
+            if (!(p->bc_velocity[a] > -1.0 && p->bc_velocity[a] < 1.0)) return fail(nullptr, LBM_EINVAL, "bc_velocity must be within (-1, 1)");
     if (p->model == LBM_SC2 && p->sc_psi != LBM_PSI_RHO && p->sc_psi != LBM_PSI_1MEXP)
         return fail(nullptr, LBM_EINVAL, "unknown sc_psi");
     if (p->lattice == LBM_D2Q9 && p->force[2] != 0.0) return fail(nullptr, LBM_EINVAL, "D2Q9 force has no z component");
@@ -141,7 +148,8 @@ LBM_API int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, voi
     if (reinterpret_cast<uintptr_t>(d_workspace) % ALIGN) return fail(nullptr, LBM_EINVAL, "workspace must be 256-byte aligned");
     lbm_ctx *c = new (std::nothrow) lbm_ctx();
     if (!c) return fail(nullptr, LBM_ENOMEM, "host allocation failed");
-    c->p = *p;
+    memset(&c->p, 0, sizeof c->p);
+    memcpy(&c->p, p, p->struct_size);  // a shorter (older) struct leaves the newer fields zero
     c->Q = Q; c->D = D; c->ncomp = p->model == LBM_SC2 ? 2 : 1;
     c->rs = p->precision == LBM_F32 ? 4 : 8;
     c->g.nx = p->nx; c->g.ny = p->ny; c->g.nz = p->nz; c->g.N = (int64_t)p->nx * p->ny * p->nz;

@@ -100,7 +100,7 @@ dim3 grid_of(const lbm_ctx *c) { return dim3((c->g.nx + c->block_x - 1) / c->blo
 template <typename T> Relax<T> make_relax(const lbm_ctx *c, int comp) {
     Relax<T> r;
     set_bgk(r, c->p.tau[comp]);
-    for (int a = 0; a < 3; a++) r.g[a] = T(c->p.force[a]);
+    for (int a = 0; a < 3; a++) { r.g[a] = T(c->p.force[a]); r.ubc[a] = T(c->p.bc_velocity[a]); }
     for (int k = 0; k < 19; k++) r.cr[k] = r.cs[k] = T(0);
     return r;
 }

@@ -16,9 +16,15 @@
 
 namespace lbm {
 
-// Node classes of the uint8 type array (1 B/node of mask traffic, BASELINE.json's byte count).
-// Only BOUNDARY nodes read their 4-byte link word.
-constexpr uint8_t NODE_BULK = 0, NODE_SOLID = 1, NODE_BOUNDARY = 2;
+// Node classes of the uint8 type array (1 B/node of mask traffic, BASELINE.json's byte count),
+// as bit flags: SOLID (dry, reflects by half-way bounce-back), LINKS (>= 1 SOLID pull source: the
+// node reads its 4-byte link word), FULLWAY (dry full-way bounce-back wall node, A20),
+// VELOCITY (equilibrium-velocity node, A21).  0 = BULK fluid.
+constexpr uint8_t NODE_BULK = 0, NODE_SOLID = 1, NODE_LINKS = 2, NODE_FULLWAY = 4, NODE_VELOCITY = 8;
+constexpr uint32_t PACK_SOLID = 0x01010101u, PACK_LINKS = 0x02020202u, PACK_SPECIAL = 0x0C0C0C0Cu;
+// lbm_set_geometry mask values (include/lbm.h)
+constexpr uint8_t MASK_FLUID = 0, MASK_SOLID = 1, MASK_FULLWAY = 2, MASK_VELOCITY = 3;
+__device__ __forceinline__ bool mask_is_solid(uint8_t m) { return m != MASK_FLUID && m != MASK_FULLWAY && m != MASK_VELOCITY; }
 
 struct Geom {
     int nx, ny, nz;
@@ -105,13 +111,14 @@ __global__ void build_links_kernel(Geom g, const uint8_t *__restrict__ mask, uin
     if (!thread_node(g, x, y, z, n)) return;
     uint32_t w = LINK_SELF_SOLID;
     uint8_t t = NODE_SOLID;
-    if (!mask[n]) {
+    const uint8_t m = mask[n];
+    if (!mask_is_solid(m)) {
         const Nbr o = neighbours(g, x, y, z);
         w = 0;
 #pragma unroll
         for (int i = 1; i < L::Q; i++)
-            if (mask[n + shift<L>(i, -1, o)]) w |= 1u << i;
-        t = w ? NODE_BOUNDARY : NODE_BULK;
+            if (mask_is_solid(mask[n + shift<L>(i, -1, o)])) w |= 1u << i;
+        t = (w ? NODE_LINKS : NODE_BULK) | (m == MASK_FULLWAY ? NODE_FULLWAY : 0) | (m == MASK_VELOCITY ? NODE_VELOCITY : 0);
     }
     link[n] = w;
     type[n] = t;
@@ -123,7 +130,8 @@ __global__ void build_links_kernel(Geom g, const uint8_t *__restrict__ mask, uin
 static __global__ void get_geometry_kernel(Geom g, const uint8_t *__restrict__ type, uint8_t *__restrict__ mask) {
     int x, y, z, n;
     if (!thread_node(g, x, y, z, n)) return;
-    mask[n] = type[n] == NODE_SOLID ? 1 : 0;
+    const uint8_t t = type[n];
+    mask[n] = (t & NODE_SOLID) ? MASK_SOLID : (t & NODE_FULLWAY) ? MASK_FULLWAY : (t & NODE_VELOCITY) ? MASK_VELOCITY : MASK_FLUID;
 }
 
 template <class L>
@@ -133,10 +141,10 @@ __global__ void stream_map_kernel(Geom g, const uint8_t *__restrict__ type, cons
     if (!thread_node(g, x, y, z, n)) return;
     const uint8_t t = type[n];
     const Nbr o = neighbours(g, x, y, z);
-    const uint32_t w = (t == NODE_BOUNDARY) ? link[n] : 0u;
+    const uint32_t w = (t & NODE_LINKS) ? link[n] : 0u;
 #pragma unroll
     for (int i = 0; i < L::Q; i++) {
-        map[(int64_t)i * g.N + n] = (t == NODE_SOLID) ? int64_t(-1) : source_slot<L, int64_t>(i, n, g.N, o, w);
+        map[(int64_t)i * g.N + n] = (t & NODE_SOLID) ? int64_t(-1) : source_slot<L, int64_t>(i, n, g.N, o, w);
     }
 }
 
@@ -259,10 +267,10 @@ template <int V> __device__ __forceinline__ bool all_solid(uint32_t t) {
 template <class L, typename T, int V, typename I>
 __device__ __forceinline__ void pull_reflected_span(const T *__restrict__ src, int64_t N, int n0, uint32_t types,
                                                     const uint32_t *__restrict__ link, T (&h)[V][L::Q]) {
-    if (types & 0x02020202u) {
+    if (types & PACK_LINKS) {
 #pragma unroll
         for (int k = 0; k < V; k++)
-            if (((types >> (8 * k)) & 0xffu) == NODE_BOUNDARY)
+            if (((types >> (8 * k)) & 0xffu) & NODE_LINKS)
                 pull_reflected<L, T, I>(src, n0 + k, N, __ldg(link + n0 + k), h[k]);
     }
 }
@@ -279,6 +287,26 @@ __device__ __forceinline__ void store_span(T *__restrict__ dst, int64_t N, int n
     }
 }
 
+// Collision by node type (t = the node's type byte).
+template <class L, typename T, bool MRT, bool FORCE>
+__device__ __forceinline__ void update_typed(T (&h)[L::Q], uint32_t t, const Relax<T> &rp) {
+    if (t & NODE_FULLWAY) fullway_reverse<L, T>(h);
+    else if (t & NODE_VELOCITY) velocity_node<L, T>(h, rp.ubc);
+    else update_node<L, T, MRT, FORCE>(h, rp);
+}
+
+// All nodes of a pack; packs without FULLWAY / VELOCITY nodes take the branch-free path.
+template <class L, typename T, int V, bool MRT, bool FORCE>
+__device__ __forceinline__ void update_span(T (&h)[V][L::Q], uint32_t types, const Relax<T> &rp) {
+    if ((types & PACK_SPECIAL) == 0) {
+#pragma unroll
+        for (int k = 0; k < V; k++) update_node<L, T, MRT, FORCE>(h[k], rp);
+    } else {
+#pragma unroll
+        for (int k = 0; k < V; k++) update_typed<L, T, MRT, FORCE>(h[k], (types >> (8 * k)) & 0xffu, rp);
+    }
+}
+
 // ---- the fused step: pull-stream + moments + equilibrium + collision (+ Guo) + store ---------
 // Rows a1-a8 of DESIGN.md.  All loads of the pack are issued before first use (bytes in flight).
 template <class L, typename T, int V, typename I, bool MRT, bool FORCE>
@@ -292,8 +320,7 @@ step_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restrict
     T h[V][L::Q];
     gather_span<L, T, V, I>(src, g.N, s, h);
     pull_reflected_span<L, T, V, I>(src, g.N, s.row + s.x0, types, link, h);
-#pragma unroll
-    for (int k = 0; k < V; k++) update_node<L, T, MRT, FORCE>(h[k], rp);
+    update_span<L, T, V, MRT, FORCE>(h, types, rp);
     store_span<L, T, V, I>(dst, g.N, s.row + s.x0, h);
 }
 
@@ -306,8 +333,8 @@ __global__ void set_distributions_kernel(Geom g, const uint8_t *__restrict__ typ
     int x, y, z, n;
     if (!thread_node(g, x, y, z, n)) return;
     const uint8_t t = type[n];
-    if (t == NODE_SOLID) return;
-    const uint32_t w = (t == NODE_BOUNDARY) ? link[n] : 0u;
+    if (t & NODE_SOLID) return;
+    const uint32_t w = (t & NODE_LINKS) ? link[n] : 0u;
     const Nbr o = neighbours(g, x, y, z);
 #pragma unroll
     for (int i = 0; i < L::Q; i++)
@@ -321,8 +348,8 @@ __global__ void init_equilibrium_kernel(Geom g, const uint8_t *__restrict__ type
     int x, y, z, n;
     if (!thread_node(g, x, y, z, n)) return;
     const uint8_t t = type[n];
-    if (t == NODE_SOLID) return;
-    const uint32_t w = (t == NODE_BOUNDARY) ? link[n] : 0u;
+    if (t & NODE_SOLID) return;
+    const uint32_t w = (t & NODE_LINKS) ? link[n] : 0u;
     const Nbr o = neighbours(g, x, y, z);
     const T rho = rho0[n];
     T v[3] = {T(0), T(0), T(0)};
@@ -340,12 +367,12 @@ __global__ void get_distributions_kernel(Geom g, const uint8_t *__restrict__ typ
     int x, y, z, n;
     if (!thread_node(g, x, y, z, n)) return;
     const uint8_t t = type[n];
-    if (t == NODE_SOLID) {
+    if (t & NODE_SOLID) {
 #pragma unroll
         for (int i = 0; i < L::Q; i++) f[(int64_t)i * g.N + n] = T(0);
         return;
     }
-    const uint32_t w = (t == NODE_BOUNDARY) ? link[n] : 0u;
+    const uint32_t w = (t & NODE_LINKS) ? link[n] : 0u;
     const Nbr o = neighbours(g, x, y, z);
     T h[L::Q];
     gather<L, T>(store, n, g.N, o, w, h);
@@ -362,8 +389,8 @@ __global__ void macro_kernel(Geom g, const uint8_t *__restrict__ type, const uin
     if (!thread_node(g, x, y, z, n)) return;
     const uint8_t t = type[n];
     T rho = T(0), v[3] = {T(0), T(0), T(0)};
-    if (t != NODE_SOLID) {
-        const uint32_t w = (t == NODE_BOUNDARY) ? link[n] : 0u;
+    if (!(t & (NODE_SOLID | NODE_FULLWAY))) {  // dry nodes report rho = 0, u = 0
+        const uint32_t w = (t & NODE_LINKS) ? link[n] : 0u;
         const Nbr o = neighbours(g, x, y, z);
         T h[L::Q], drho, j[3];
         gather<L, T>(store, n, g.N, o, w, h);
@@ -409,8 +436,7 @@ aa_even_kernel(Geom g, const uint8_t *__restrict__ type, T *f, Relax<T> rp) {
 #pragma unroll
         for (int k = 0; k < V; k++) h[k][i] = a[k];
     }
-#pragma unroll
-    for (int k = 0; k < V; k++) update_node<L, T, MRT, FORCE>(h[k], rp);
+    update_span<L, T, V, MRT, FORCE>(h, types, rp);
 #pragma unroll
     for (int i = 0; i < L::Q; i++) {
         T a[V];
@@ -427,8 +453,8 @@ aa_odd_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restri
     if (!thread_span<1>(g, s)) return;
     const int n = s.row + s.x0;
     const uint8_t t = type[n];
-    if (t == NODE_SOLID) return;
-    const uint32_t w = (t == NODE_BOUNDARY) ? __ldg(link + n) : 0u;
+    if (t & NODE_SOLID) return;
+    const uint32_t w = (t & NODE_LINKS) ? __ldg(link + n) : 0u;
     const Nbr o = neighbours(g, s.x0, s.y, s.z);
     I slot[L::Q];
     T h[L::Q];
@@ -437,7 +463,7 @@ aa_odd_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restri
         slot[i] = aa_slot<L, I>(1, i, n, g.N, o, w);
         h[i] = f[slot[i]];
     }
-    update_node<L, T, MRT, FORCE>(h, rp);
+    update_typed<L, T, MRT, FORCE>(h, t, rp);
 #pragma unroll
     for (int i = 0; i < L::Q; i++) f[slot[L::opp(i)]] = h[i];
 }
@@ -450,10 +476,10 @@ __global__ void aa_convert_kernel(Geom g, int parity, const uint8_t *__restrict_
     int x, y, z, n;
     if (!thread_node(g, x, y, z, n)) return;
     const uint8_t t = type[n];
-    const uint32_t w = (t == NODE_BOUNDARY) ? link[n] : 0u;
+    const uint32_t w = (t & NODE_LINKS) ? link[n] : 0u;
     const Nbr o = neighbours(g, x, y, z);
     if (MODE == 0 || MODE == 2) {
-        if (t == NODE_SOLID) return;
+        if (t & NODE_SOLID) return;
         T h[L::Q];
         if (MODE == 0) {
 #pragma unroll
@@ -469,13 +495,13 @@ __global__ void aa_convert_kernel(Geom g, int parity, const uint8_t *__restrict_
     } else {
         T h[L::Q];
 #pragma unroll
-        for (int i = 0; i < L::Q; i++) h[i] = (t == NODE_SOLID) ? T(0) : store[aa_slot<L, int64_t>(parity, i, n, g.N, o, w)];
+        for (int i = 0; i < L::Q; i++) h[i] = (t & NODE_SOLID) ? T(0) : store[aa_slot<L, int64_t>(parity, i, n, g.N, o, w)];
         if (MODE == 1) {
 #pragma unroll
-            for (int i = 0; i < L::Q; i++) out0[(int64_t)i * g.N + n] = (t == NODE_SOLID) ? T(0) : h[i] + L::template w<T>(i);
+            for (int i = 0; i < L::Q; i++) out0[(int64_t)i * g.N + n] = (t & NODE_SOLID) ? T(0) : h[i] + L::template w<T>(i);
         } else {
             T rho = T(0), v[3] = {T(0), T(0), T(0)};
-            if (t != NODE_SOLID) {
+            if (!(t & (NODE_SOLID | NODE_FULLWAY))) {
                 T drho, j[3];
                 moments<L, T>(h, drho, j);
                 rho = T(1) + drho;
@@ -541,7 +567,7 @@ sc_fields_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__res
 #pragma unroll
             for (int i = 1; i < L::Q; i++) sum += h[k][i];
             pb[k] = psi_dev<T, PSI>(sum);
-            if (((types >> (8 * k)) & 0xffu) == NODE_SOLID) pa[k] = pb[k] = -psi_one<T, PSI>();
+            if ((types >> (8 * k)) & (NODE_SOLID | NODE_FULLWAY)) pa[k] = pb[k] = -psi_one<T, PSI>();  // dry: psi = 0 (A14)
         }
     }
     // (psi_A, psi_B) interleaved: pass 2 fetches both with one 8/16-byte load per neighbour.
@@ -600,6 +626,12 @@ sc_step_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restr
     pull_reflected_span<L, T, V, I>(srcB, g.N, n0, types, link, hB);
 #pragma unroll
     for (int k = 0; k < V; k++) {
+        const uint32_t t = (types >> (8 * k)) & 0xffu;
+        if (t & (NODE_FULLWAY | NODE_VELOCITY)) {  // these replace the collision of both components
+            if (t & NODE_FULLWAY) { fullway_reverse<L, T>(hA[k]); fullway_reverse<L, T>(hB[k]); }
+            else { velocity_node<L, T>(hA[k], rpA.ubc); velocity_node<L, T>(hB[k], rpB.ubc); }
+            continue;
+        }
         Nbr o = s.o;
         const int x = s.x0 + k;
         o.xm = (x == 0) ? (g.nx - 1) : -1;

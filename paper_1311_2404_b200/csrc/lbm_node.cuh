@@ -19,6 +19,7 @@ template <typename T> struct Relax {
     // omega / 36 and (1 - omega / 2) / 36 as unevaluated sums hi + lo of two T (see collide()):
     T om36_hi, om36_lo, sc36_hi, sc36_lo;
     T g[3];           // body acceleration
+    T ubc[3];         // velocity imposed on equilibrium-velocity nodes (reading A21)
     T cr[19];         // MRT: rate_k / |M_k|^2                 (relaxation, eq. 4)
     T cs[19];         // MRT: (1 - rate_k / 2) / |M_k|^2       (source, reading A16)
 };
@@ -338,6 +339,24 @@ LBM_HD void update_node(T (&h)[L::Q], const Relax<T> &rp) {
         }
         collide<L, T, MRT, FORCE>(h, rho, drho, v, rv, F, rp);
     }
+}
+
+// ---- node types that replace the collision (readings A20, A21) --------------------
+// Full-way bounce-back wall node (Fig. 2 (1)): dry; the populations streamed into it are
+// scattered back, h*_i = h_ibar, without relaxation.
+template <class L, typename T> LBM_HD void fullway_reverse(T (&h)[L::Q]) {
+#pragma unroll
+    for (int i = 1; i < L::Q; i++)
+        if (i < L::opp(i)) { const T t = h[i]; h[i] = h[L::opp(i)]; h[L::opp(i)] = t; }
+}
+
+// Equilibrium-velocity node: rho from the node's own incoming populations (the missing ones
+// are bounce-back copies, supplied by the reflected-link rule), post-collision state f^eq(rho, u_bc).
+template <class L, typename T> LBM_HD void velocity_node(T (&h)[L::Q], const T (&ubc)[3]) {
+    T drho = h[0];
+#pragma unroll
+    for (int i = 1; i < L::Q; i++) drho += h[i];
+    equilibrium_dev<L, T>(T(1) + drho, drho, ubc, h);
 }
 
 }  // namespace lbm

@@ -23,6 +23,7 @@ import numpy as np
 D2Q9, D3Q19 = 0, 1
 BGK, MRT, SC2 = 0, 1, 2
 F32, F64 = 0, 1
+FLUID, SOLID, WALL_FULLWAY, VELOCITY = 0, 1, 2, 3   # node types of the geometry mask
 
 
 def mrt_rates_d3q19(tau: float) -> list:
@@ -51,6 +52,7 @@ class Workload:
     rates: list | None = None
     sc_G: float = 0.0
     sc_psi: int = 0
+    bc_velocity: tuple = (0.0, 0.0, 0.0)
     seed: int | None = None
     mask: np.ndarray | None = None                 # uint8 [nz][ny][nx], 0 FLUID 1 SOLID
     rho: list = field(default_factory=list)        # per component, fp64 [nz][ny][nx]
@@ -74,7 +76,8 @@ class Workload:
 
     def params(self) -> dict:
         return dict(lattice=self.lattice, model=self.model, nx=self.nx, ny=self.ny, nz=self.nz,
-                    tau=self.tau, rates=self.rates, force=self.force, sc_G=self.sc_G, sc_psi=self.sc_psi)
+                    tau=self.tau, rates=self.rates, force=self.force, sc_G=self.sc_G, sc_psi=self.sc_psi,
+                    bc_velocity=self.bc_velocity)
 
 
 def c1_taylor_green(n: int = 128, steps: int = 1000, u0: float = 0.01, tau: float = 0.8,
@@ -142,6 +145,36 @@ def c5_shan_chen(nx: int = 256, ny: int = 256, nz: int = 256, steps: int = 1000,
     return w
 
 
+def ldc_cavity(nx: int = 256, ny: int = 256, nz: int = 256, steps: int = 1000, Re: float = 1000.0,
+               U: float = 0.05, precision: int = F32, model: int = BGK) -> Workload:
+    """Lid-driven cavity, the paper's single-fluid benchmark case (254^3 interior, Re = 1000,
+    full bounce-back walls, equilibrium-velocity lid).  Box = interior + one node of wall all round:
+    x, z faces and the floor y = 0 are full-way walls, the lid row y = ny-2 moves at (U, 0, 0) and is
+    backed by a SOLID row y = ny-1 (which also separates it from the floor on the torus)."""
+    nu = U * (nx - 2) / Re
+    tau = 3.0 * nu + 0.5
+    w = Workload("ldc_cavity_d3q19", D3Q19, model, precision, nx, ny, nz, (tau, tau), steps,
+                 rates=mrt_rates_d3q19(tau) if model == MRT else None, bc_velocity=(U, 0.0, 0.0))
+    mask = np.zeros((nz, ny, nx), np.uint8)
+    mask[:, ny - 2, :] = VELOCITY
+    mask[:, 0, :] = WALL_FULLWAY
+    mask[:, :, 0] = WALL_FULLWAY
+    mask[:, :, nx - 1] = WALL_FULLWAY
+    mask[0, :, :] = WALL_FULLWAY
+    mask[nz - 1, :, :] = WALL_FULLWAY
+    mask[:, ny - 1, :] = SOLID
+    w.mask, w.rho, w.u = mask, [np.ones((nz, ny, nx))], [np.zeros((3, nz, ny, nx))]
+    return w
+
+
+def random_types(lattice: int, nx: int, ny: int, nz: int, seed: int, ncomp: int = 1):
+    """Seeded state with all four node types mixed at random (parity tests of the boundary nodes)."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    _, rho, u = random_state(lattice, nx, ny, nz, seed + 1, ncomp=ncomp)
+    mask = rng.choice(np.array([FLUID] * 7 + [SOLID, WALL_FULLWAY, VELOCITY], np.uint8), size=(nz, ny, nx))
+    return mask, rho, u
+
+
 def random_state(lattice: int, nx: int, ny: int, nz: int, seed: int, solid_fraction: float = 0.0,
                  du: float = 0.02, drho: float = 0.02, ncomp: int = 1):
     """Generic seeded (mask, rho[], u[]) for parity tests at arbitrary (ragged) sizes."""
@@ -163,4 +196,5 @@ CONFIGS = {
     "c3": c3_mrt_obstacles,
     "c4": c4_duct,
     "c5": c5_shan_chen,
+    "ldc": ldc_cavity,
 }

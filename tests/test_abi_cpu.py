@@ -33,10 +33,14 @@ def test_header_symbols_exported(lib):
 
 
 def test_params_struct_matches_header(lib):
-    # uint32 + 6 int32 (28) -> pad to 32; 2 + 19 + 3 + 1 doubles (200); 2 int32 (8)  => 240
-    assert C.sizeof(binding.lbm_params) == 240
+    # uint32 + 6 int32 (28) -> pad to 32; 2 + 19 + 3 + 1 doubles (200); 2 int32 (8) => 240 (v1);
+    # + bc_velocity[3] => 264
+    assert C.sizeof(binding.lbm_params) == 264
     p = binding.make_params(1, 0, 0, 8, 8, 8, tau=0.6)
-    assert binding.lbm_workspace_bytes(p) > 0
+    n = binding.lbm_workspace_bytes(p)
+    assert n > 0
+    p.struct_size = 240  # a caller built against the first layout: accepted, bc_velocity = 0
+    assert binding.lbm_workspace_bytes(p) == n
     p.struct_size = 16
     with pytest.raises(binding.LbmError) as e:
         binding.lbm_workspace_bytes(p)
@@ -66,6 +70,7 @@ def test_lattice_info_table1(lib):
     (dict(model=1, rates=[2.5] * 19), binding.LBM_EINVAL),
     (dict(store=1, model=2, tau=(1.0, 1.0)), binding.LBM_EUNSUPPORTED),
     (dict(store=7), binding.LBM_EINVAL),
+    (dict(bc_velocity=(1.5, 0.0, 0.0)), binding.LBM_EINVAL),
 ])
 def test_bad_params_rejected(lib, kw, code):
     args = dict(lattice=1, model=0, precision=0, nx=8, ny=8, nz=8, tau=0.8)

@@ -201,3 +201,58 @@ def test_aa_uses_half_the_distribution_memory(B):
     ab = B.lbm_workspace_bytes(B.make_params(W.D3Q19, W.BGK, W.F32, 64, 64, 64, tau=0.8))
     aa = B.lbm_workspace_bytes(B.make_params(W.D3Q19, W.BGK, W.F32, 64, 64, 64, tau=0.8, store=B.LBM_STORE_AA))
     assert ab - aa == 19 * 64 ** 3 * 4
+
+
+# ---- NEXT-2: full-way bounce-back walls and equilibrium-velocity nodes (A20, A21) ---------
+def check_parity_live(B, orc, w, steps=100, **kw):
+    """Like check_parity but compares every node that is not SOLID (wall nodes hold populations)."""
+    sim = B.from_workload(w, **kw)
+    ref = orc.Oracle(**w.params())
+    sim.set_geometry(w.mask)
+    ref.set_geometry(w.mask)
+    for s in range(w.ncomp):
+        sim.init_equilibrium(w.rho[s], w.u[s], comp=s)
+        ref.init_equilibrium(w.rho[s], w.u[s], comp=s)
+    assert np.array_equal(sim.get_geometry().cpu().numpy(), w.mask)
+    assert np.array_equal(sim.get_stream_map().cpu().numpy(), ref.stream_map())
+    live = w.mask != W.SOLID
+    for chunk in (steps // 2 + 1, steps - steps // 2 - 1):
+        sim.step(chunk)
+        ref.step(chunk)
+        for s in range(w.ncomp):
+            d = np.abs(sim.get_distributions(s).cpu().numpy().astype(np.float64) - ref.get_distributions(s))
+            assert d[:, live].max() <= TOL[w.precision]
+            rho_g, u_g = sim.macro(s)
+            rho_r, u_r = ref.macro(s)
+            assert np.abs(rho_g.cpu().numpy() - rho_r).max() <= TOL[w.precision]
+            assert np.abs(u_g.cpu().numpy() - u_r).max() <= TOL[w.precision]
+    sim.close()
+
+
+@pytest.mark.parametrize("store", ["ab", "aa"])
+@pytest.mark.parametrize("lattice,model,precision,shape", [
+    (W.D3Q19, W.BGK, W.F32, (48, 21, 10)), (W.D3Q19, W.BGK, W.F64, (37, 14, 9)),
+    (W.D3Q19, W.MRT, W.F32, (40, 12, 11)), (W.D2Q9, W.BGK, W.F64, (66, 31, 1)), (W.D2Q9, W.MRT, W.F32, (52, 30, 1))])
+def test_all_node_types_mixed_at_random(B, orc, lattice, model, precision, shape, store):
+    nx, ny, nz = shape
+    mask, rho, u = W.random_types(lattice, nx, ny, nz, seed=41)
+    D = 2 if lattice == W.D2Q9 else 3
+    rates = (W.mrt_rates_d3q19(0.7) if lattice == W.D3Q19 else W.mrt_rates_d2q9(0.7)) if model == W.MRT else None
+    w = W.Workload("types", lattice, model, precision, nx, ny, nz, (0.7, 0.7), 100, rates=rates,
+                   force=(1e-5, -2e-5, 3e-5 if D == 3 else 0.0), bc_velocity=(0.02, -0.01, 0.015 if D == 3 else 0.0))
+    w.mask, w.rho, w.u = mask, rho, u
+    check_parity_live(B, orc, w, store=B.LBM_STORE_AA if store == "aa" else B.LBM_STORE_AB)
+
+
+def test_all_node_types_shan_chen(B, orc):
+    mask, rho, u = W.random_types(W.D3Q19, 30, 16, 9, seed=43, ncomp=2)
+    w = W.Workload("types_sc", W.D3Q19, W.SC2, W.F64, 30, 16, 9, (0.8, 1.1), 100, sc_G=0.6,
+                   bc_velocity=(0.01, 0.0, -0.01))
+    w.mask, w.rho, w.u = mask, rho, u
+    check_parity_live(B, orc, w, steps=60)
+
+
+@pytest.mark.parametrize("precision", [W.F32, W.F64])
+def test_lid_driven_cavity_reduced(B, orc, precision):
+    """The paper's benchmark box at 40 x 36 x 32: full-way walls, equilibrium-velocity lid."""
+    check_parity_live(B, orc, W.ldc_cavity(40, 36, 32, precision=precision))
