@@ -34,6 +34,9 @@
  *              u' = (j_A/tau_A + j_B/tau_B)/(rho_A/tau_A + rho_B/tau_B)    P:188;
  *              v_s = u' + F_s/(2 rho_s), then f^eq / LBGK / Guo per component (A13);
  *              macro fields are computed for all nodes first
+ *   full-way BB  wall node (dry): f* = f reversed, no relaxation; back in the fluid at t+2     P:237 Fig. 2 (1), A20
+ *   velocity BC  f* = f^eq(rho, u_bc), rho from the node's own populations, missing ones
+ *              are bounce-back copies (the half-way rule behind a SOLID node)              P:239, A21
  *   init       f_i(x,0) = f^eq_i(rho0(x), u0(x))
  *   macro      rho = sum f_i, velocity v of eq. (16)
  *
@@ -42,7 +45,9 @@
  * Poiseuille parabola + second-order convergence, Taylor-Green decay rate, MRT == LBGK for
  * equal rates, MRT matrix orthogonality and d'Humieres' closed-form equilibrium moments,
  * MRT shear-wave viscosity, brute-force stream map on tiny lattices, Shan-Chen conservation
- * laws / G = 0 / linear-gradient force.
+ * laws / G = 0 / linear-gradient force, full-way wall (hand-tracked arrow, steady Poiseuille equals
+ * the half-way profile), velocity node (uniform-flow fixed point, Couette flow), and one step with
+ * all four node types against an independent whole-array numpy implementation.
  * PARITY UNPINNED (no printed value in the paper): the physical sign of the
  * Shan-Chen coupling (reading A11) and the c3 rate s_m = 1.98 (a parameter, not arithmetic).
  */
