@@ -64,6 +64,7 @@ enum { ORC_BGK = 0, ORC_MRT = 1, ORC_SC2 = 2 };
 enum { ORC_PSI_RHO = 0, ORC_PSI_1MEXP = 1 };
 #define ORC_QMAX 19
 /* node types (P:446 reduced; readings A8, A20, A21) */
+enum { ORC_FORCE_GUO = 0, ORC_FORCE_EDM = 1 };
 enum { ORC_FLUID = 0, ORC_SOLID = 1, ORC_WALL_FULLWAY = 2, ORC_VELOCITY = 3 };
 
 typedef struct {
@@ -75,6 +76,7 @@ typedef struct {
     double sc_G;
     int32_t sc_psi;
     double bc_velocity[3]; /* velocity imposed on ORC_VELOCITY nodes (reading A21) */
+    int32_t force_scheme;  /* ORC_FORCE_GUO (eq. 17) | ORC_FORCE_EDM (eq. 18) */
 } orc_params;
 
 /* ---- velocity sets (reading A2; weights from Table 1) ------------- */
@@ -357,11 +359,37 @@ int orc_stream_map(const orc_ctx *c, int64_t *map)
  * in:  f (Q values), rho, v (velocity entering f^eq and the source), F (force density), tau
  * out: fstar */
 static void collide_node(const orc_ctx *c, const double *f, double rho, const double v[3],
-                         const double F[3], double tau, double *fstar)
+                         const double ub[3], const double F[3], double tau, double *fstar)
 {
     const lattice_t *L = &c->L;
     const int Q = L->Q;
     double fe[ORC_QMAX], src[ORC_QMAX];
+    if (c->p.force_scheme == ORC_FORCE_EDM) {
+        /* Exact Difference Method, eq. (18) P:253-258 (reading A22): relax towards f^eq(rho, u) at
+         * the bare velocity u = ub (sum e f / rho; the common velocity u' for Shan-Chen) and add
+         * F_i = f^eq(rho, u + F/rho) - f^eq(rho, u), unscaled, for any collision operator. */
+        double u2[3], fe2[ORC_QMAX];
+        for (int a = 0; a < 3; a++) u2[a] = ub[a] + F[a] / rho;
+        feq(L, rho, ub, fe);
+        feq(L, rho, u2, fe2);
+        if (c->p.model == ORC_MRT) {
+            double m[ORC_QMAX], me[ORC_QMAX], d[ORC_QMAX];
+            for (int k = 0; k < Q; k++) {
+                double a = 0, b = 0;
+                for (int i = 0; i < Q; i++) { a += c->M[k * Q + i] * f[i]; b += c->M[k * Q + i] * fe[i]; }
+                m[k] = a; me[k] = b;
+            }
+            for (int k = 0; k < Q; k++) d[k] = c->p.rates[k] * (me[k] - m[k]);
+            for (int i = 0; i < Q; i++) {
+                double a = 0;
+                for (int k = 0; k < Q; k++) a += c->Minv[i * Q + k] * d[k];
+                fstar[i] = f[i] + a + (fe2[i] - fe[i]);
+            }
+        } else {
+            for (int i = 0; i < Q; i++) fstar[i] = f[i] + (fe[i] - f[i]) / tau + (fe2[i] - fe[i]);
+        }
+        return;
+    }
     feq(L, rho, v, fe); /* eq. (3) */
     /* bracket of eq. (17): w_i [3 (e_i - v) + 9 (e_i.v) e_i] . F */
     for (int i = 0; i < Q; i++) {
@@ -445,7 +473,7 @@ static void step_single(orc_ctx *c)
     for (int64_t n = 0; n < N; n++) {
         if (c->mask[n] == ORC_SOLID) continue;
         double f[ORC_QMAX], fstar[ORC_QMAX];
-        double rho = 0, j[3] = {0, 0, 0}, F[3], v[3];
+        double rho = 0, j[3] = {0, 0, 0}, F[3], v[3], ub[3];
         for (int i = 0; i < Q; i++) {
             f[i] = c->f[0][i * N + n];
             rho += f[i];                                               /* eq. (1) */
@@ -458,8 +486,9 @@ static void step_single(orc_ctx *c)
         for (int a = 0; a < 3; a++) {
             F[a] = rho * c->p.force[a];                                /* F = rho g (A4) */
             v[a] = (j[a] + 0.5 * F[a]) / rho;                          /* eq. (16)       */
+            ub[a] = j[a] / rho;                                        /* eq. (1)        */
         }
-        collide_node(c, f, rho, v, F, c->p.tau[0], fstar);
+        collide_node(c, f, rho, v, ub, F, c->p.tau[0], fstar);
         for (int i = 0; i < Q; i++) c->fs[0][i * N + n] = fstar[i];
     }
     stream(c, 0);
@@ -537,7 +566,7 @@ static void step_sc2(orc_ctx *c)
                         v[a] = up[a] + F[a] / (2.0 * rs);              /* (iv)  */
                     }
                     for (int i = 0; i < Q; i++) f[i] = c->f[s][i * N + n];
-                    collide_node(c, f, rs, v, F, c->p.tau[s], fstar);  /* (v)   */
+                    collide_node(c, f, rs, v, up, F, c->p.tau[s], fstar); /* (v) */
                     for (int i = 0; i < Q; i++) c->fs[s][i * N + n] = fstar[i];
                 }
             }

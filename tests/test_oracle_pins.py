@@ -670,3 +670,98 @@ def test_step_with_all_node_types_against_numpy_roll_reference(orc, lat, shp):
     got = o.get_distributions()
     assert np.max(np.abs(got - f)[:, live]) < 1e-14
     assert np.array_equal(got[:, ~live], f[:, ~live])
+
+
+# ---------------------------------------------------------------- NEXT-3: Exact Difference Method (eq. 18,
+# P:253-258; reading A22)
+@pytest.mark.parametrize("lat,model", [(0, 0), (0, 1), (1, 0), (1, 1)])
+def test_edm_uniform_force_closed_form(orc, lat, model):
+    """sum_i e_i [f^eq(rho, u + F/rho) - f^eq(rho, u)] = F: every step adds exactly g to the
+    velocity, for any collision operator, and eq. (16) holds: v(n) = u0 + (n + 1/2) g."""
+    from paper_1311_2404_b200 import workloads as W
+    shp = (4, 5, 1) if lat == 0 else (4, 5, 6)
+    g = (1e-5, -2e-5, 0.0 if lat == 0 else 3e-5)
+    u0 = (0.01, 0.02, 0.0 if lat == 0 else -0.015)
+    rates = (W.mrt_rates_d3q19(0.8) if lat else W.mrt_rates_d2q9(0.8)) if model else None
+    o = orc.Oracle(lat, model, *shp, tau=0.8, force=g, rates=rates, force_scheme=orc.FORCE_EDM)
+    o.init_equilibrium(*_uniform(o, 1.1, u0))
+    o.step(37)
+    r, v = o.macro()
+    assert np.max(np.abs(r - 1.1)) < 1e-14
+    for a in range(o.D):
+        assert np.max(np.abs(v[a] - (u0[a] + 37.5 * g[a]))) < 1e-15
+
+
+def test_edm_steady_poiseuille_curvature_and_wall_symmetry(orc):
+    """Steady channel driven through the EDM: the momentum balance fixes the curvature of the
+    profile to -g / nu at every interior row, whatever the force scheme."""
+    g, tau, ny = 1e-6, 0.8, 18
+    nu = (tau - 0.5) / 3.0
+    o = orc.Oracle(0, 0, 3, ny, 1, tau=tau, force=(g, 0, 0), force_scheme=orc.FORCE_EDM)
+    mask = np.zeros(o.shape, np.uint8)
+    mask[:, 0, :] = 1
+    mask[:, ny - 1, :] = 1
+    o.set_geometry(mask)
+    o.init_equilibrium(*_uniform(o, 1.0, (0, 0, 0)))
+    o.step(40000)
+    ux = o.macro()[1][0][0, 1:ny - 1, 1]
+    second = ux[2:] - 2 * ux[1:-1] + ux[:-2]
+    assert np.max(np.abs(second / (-g / nu) - 1.0)) < 1e-9
+    assert np.max(np.abs(ux - ux[::-1])) < 1e-14
+    y = np.arange(1, ny - 1, dtype=float)
+    parab = g / (2 * nu) * (y - 0.5) * (ny - 1.5 - y)
+    assert np.ptp(ux - parab) < 1e-9 * ux.max()            # parabola + constant slip
+
+
+def test_edm_shan_chen_conserves_mass_and_total_momentum(orc):
+    o = orc.Oracle(1, 2, 6, 5, 4, tau=(0.8, 1.3), sc_G=0.9, force_scheme=orc.FORCE_EDM)
+    rng = np.random.default_rng(8)
+    ra, rb = 1 + rng.uniform(-0.05, 0.05, o.shape), 0.7 + rng.uniform(-0.05, 0.05, o.shape)
+    u = rng.uniform(-0.01, 0.01, (3,) + o.shape)
+    o.init_equilibrium(ra, u, 0)
+    o.init_equilibrium(rb, u, 1)
+    def totals():
+        fa, fb = o.get_distributions(0), o.get_distributions(1)
+        e = orc.lattice_tables(1)[0].astype(float)
+        return fa.sum(), fb.sum(), np.einsum("qzyx,qa->a", fa + fb, e)
+    ma0, mb0, p0 = totals()
+    o.step(40)
+    ma1, mb1, p1 = totals()
+    assert abs(ma1 - ma0) < 1e-12 * ma0 and abs(mb1 - mb0) < 1e-12 * mb0
+    assert np.max(np.abs(p1 - p0)) < 1e-12                  # sum of F_A + F_B vanishes on a torus (psi = rho)
+
+
+@pytest.mark.parametrize("lat,shp", [(0, (7, 6, 1)), (1, (5, 6, 4))])
+def test_edm_step_against_numpy_roll_reference(orc, lat, shp):
+    """Independent whole-array numpy implementation of LBGK + EDM + half-way bounce-back."""
+    from paper_1311_2404_b200 import workloads as W
+    nx, ny, nz = shp
+    e, w, opp = orc.lattice_tables(lat)
+    Q, D = len(e), (2 if lat == 0 else 3)
+    mask, rho, u = W.random_state(lat, nx, ny, nz, seed=51, solid_fraction=0.2)
+    tau, g = 0.9, np.array([1e-4, -2e-4, 3e-4 if D == 3 else 0.0])
+    o = orc.Oracle(lat, 0, nx, ny, nz, tau=tau, force=g, force_scheme=orc.FORCE_EDM)
+    o.set_geometry(mask)
+    o.init_equilibrium(rho[0], u[0])
+    f = o.get_distributions().copy()
+    ef, fluid = e.astype(float), mask == 0
+    wq = w[:, None, None, None]
+
+    def feq(r, v):
+        ev = np.einsum("qa,azyx->qzyx", ef, v)
+        return r * wq * (1 + 3 * ev + 4.5 * ev ** 2 - 1.5 * (v ** 2).sum(0))
+
+    for _ in range(12):
+        r = f.sum(0)
+        ub = np.einsum("qzyx,qa->azyx", f, ef) / r
+        fe = feq(r, ub)
+        fs = f + (fe - f) / tau + feq(r, ub + g[:, None, None, None]) - fe      # F = rho g, du = F / rho = g
+        new = f.copy()
+        for i in range(Q):
+            sh = (e[i][2], e[i][1], e[i][0])
+            moved = np.roll(fs[i], shift=sh, axis=(0, 1, 2))
+            from_solid = np.roll(mask, shift=sh, axis=(0, 1, 2)) == 1
+            new[i] = np.where(fluid, np.where(from_solid, fs[opp[i]], moved), f[i])
+        f = new
+    o.step(12)
+    assert np.max(np.abs(o.get_distributions() - f)[:, fluid]) < 1e-14
