@@ -38,6 +38,8 @@ enum { LBM_BGK = 0, LBM_MRT = 1, LBM_SC2 = 2 };  /* model: SC2 = two LBGK compon
 enum { LBM_F32 = 0, LBM_F64 = 1 };               /* precision of storage and arithmetic      */
 enum { LBM_PSI_RHO = 0, LBM_PSI_1MEXP = 1 };     /* psi(rho) = rho | 1 - exp(-rho)   */
 enum { LBM_STORE_AB = 0, LBM_STORE_AA = 1 };     /* two copies | in-place AA */
+enum { LBM_FORCE_GUO = 0, LBM_FORCE_EDM = 1 };   /* Guo, eq. (17) P:251 | Exact Difference Method,
+                                                    eq. (18), reading A22            */
 /* node types of the lbm_set_geometry mask (P:446 reduced to what the path needs):
  *   FLUID         wet, collides
  *   SOLID         dry; a pull from it returns the puller's own opposite post-collision population
@@ -70,6 +72,9 @@ typedef struct {
     int32_t store;            /* LBM_STORE_AB (default 0) | LBM_STORE_AA                           */
     double bc_velocity[3];    /* velocity imposed on LBM_NODE_VELOCITY nodes (reading A21);
                                  callers built against the 240-byte struct (no such field) get 0   */
+    int32_t force_scheme;     /* LBM_FORCE_GUO (default 0, eq. 17) | LBM_FORCE_EDM (eq. 18); applies to
+                                 the body force and to the Shan-Chen coupling force alike          */
+    int32_t reserved_;        /* keeps sizeof a multiple of 8; set to 0                            */
 } lbm_params;
 
 /* Static description of a lattice (Table 1; ordering = reading A2).

@@ -19,6 +19,7 @@ LBM_BGK, LBM_MRT, LBM_SC2 = 0, 1, 2
 LBM_F32, LBM_F64 = 0, 1
 LBM_PSI_RHO, LBM_PSI_1MEXP = 0, 1
 LBM_STORE_AB, LBM_STORE_AA = 0, 1
+LBM_FORCE_GUO, LBM_FORCE_EDM = 0, 1
 LBM_NODE_FLUID, LBM_NODE_SOLID, LBM_NODE_WALL_FULLWAY, LBM_NODE_VELOCITY = 0, 1, 2, 3
 LBM_QMAX = 19
 
@@ -40,6 +41,8 @@ class lbm_params(C.Structure):
         ("sc_psi", C.c_int32),
         ("store", C.c_int32),
         ("bc_velocity", C.c_double * 3),
+        ("force_scheme", C.c_int32),
+        ("reserved_", C.c_int32),
     ]
 
 
@@ -87,7 +90,7 @@ def load():
 
 def make_params(lattice, model, precision, nx, ny, nz=1, tau=(1.0, 1.0), rates=None,
                 force=(0.0, 0.0, 0.0), sc_G=0.0, sc_psi=LBM_PSI_RHO, store=LBM_STORE_AB,
-                bc_velocity=(0.0, 0.0, 0.0)) -> lbm_params:
+                bc_velocity=(0.0, 0.0, 0.0), force_scheme=0) -> lbm_params:
     p = lbm_params()
     p.struct_size = C.sizeof(lbm_params)
     p.lattice, p.model, p.precision = int(lattice), int(model), int(precision)
@@ -100,6 +103,7 @@ def make_params(lattice, model, precision, nx, ny, nz=1, tau=(1.0, 1.0), rates=N
     for a in range(3):
         p.force[a] = float(force[a]) if a < len(force) else 0.0
     p.sc_G, p.sc_psi, p.store = float(sc_G), int(sc_psi), int(store)
+    p.force_scheme = int(force_scheme)
     for a in range(3):
         p.bc_velocity[a] = float(bc_velocity[a]) if a < len(bc_velocity) else 0.0
     return p
@@ -257,4 +261,4 @@ class Lbm:
 def from_workload(w, device="cuda:0", **kw) -> "Lbm":
     """Context for a workloads.Workload (parameters only; arrays are passed separately)."""
     return Lbm(w.lattice, w.model, w.precision, w.nx, w.ny, w.nz, device=device, tau=w.tau, rates=w.rates,
-               force=w.force, sc_G=w.sc_G, sc_psi=w.sc_psi, bc_velocity=w.bc_velocity, **kw)
+               force=w.force, sc_G=w.sc_G, sc_psi=w.sc_psi, bc_velocity=w.bc_velocity, force_scheme=w.force_scheme, **kw)

@@ -7,10 +7,12 @@ namespace {
 
 // sizeof(lbm_params) before bc_velocity was appended; such callers get bc_velocity = 0
 constexpr uint32_t LBM_PARAMS_SIZE_V1 = 240;
+// ... and before force_scheme was appended; such callers get the Guo scheme
+constexpr uint32_t LBM_PARAMS_SIZE_V2 = 264;
 
 int validate(const lbm_params *p, int *Q, int *D) {
     if (!p) return fail(nullptr, LBM_EINVAL, "params is NULL");
-    if (p->struct_size != sizeof(lbm_params) && p->struct_size != LBM_PARAMS_SIZE_V1)
+    if (p->struct_size != sizeof(lbm_params) && p->struct_size != LBM_PARAMS_SIZE_V1 && p->struct_size != LBM_PARAMS_SIZE_V2)
         return fail(nullptr, LBM_EINVAL, "struct_size is not a known sizeof(lbm_params)");
     if (p->lattice != LBM_D2Q9 && p->lattice != LBM_D3Q19) return fail(nullptr, LBM_EINVAL, "unknown lattice");
     if (p->model < LBM_BGK || p->model > LBM_SC2) return fail(nullptr, LBM_EINVAL, "unknown model");
@@ -29,7 +31,9 @@ int validate(const lbm_params *p, int *Q, int *D) {
             if (!(p->rates[k] >= 0.0 && p->rates[k] <= 2.0)) return fail(nullptr, LBM_EINVAL, "MRT rates must be in [0, 2]");
     for (int a = 0; a < 3; a++)
         if (!(p->force[a] == p->force[a])) return fail(nullptr, LBM_EINVAL, "force is NaN");
-    if (p->struct_size == sizeof(lbm_params))
+    if (p->struct_size == sizeof(lbm_params) && p->force_scheme != LBM_FORCE_GUO && p->force_scheme != LBM_FORCE_EDM)
+        return fail(nullptr, LBM_EINVAL, "unknown force_scheme");
+    if (p->struct_size >= LBM_PARAMS_SIZE_V2)
         for (int a = 0; a < 3; a++)
             if (!(p->bc_velocity[a] > -1.0 && p->bc_velocity[a] < 1.0)) return fail(nullptr, LBM_EINVAL, "bc_velocity must be within (-1, 1)");
     if (p->model == LBM_SC2 && p->sc_psi != LBM_PSI_RHO && p->sc_psi != LBM_PSI_1MEXP)

@@ -101,7 +101,7 @@ template <typename T> Relax<T> make_relax(const lbm_ctx *c, int comp) {
     Relax<T> r;
     set_bgk(r, c->p.tau[comp]);
     for (int a = 0; a < 3; a++) { r.g[a] = T(c->p.force[a]); r.ubc[a] = T(c->p.bc_velocity[a]); }
-    for (int k = 0; k < 19; k++) r.cr[k] = r.cs[k] = T(0);
+    for (int k = 0; k < 19; k++) r.cr[k] = r.cs[k] = r.in[k] = T(0);
     return r;
 }
 
@@ -177,11 +177,11 @@ template <class L, typename T> struct Impl {
         return check_launch(c, "stream_map_kernel");
     }
 
-    template <int V, bool MRT, bool FORCE> static int step_single_v(lbm_ctx *c, int n, const Relax<T> &rp) {
+    template <int V, bool MRT, int FORCE> static int step_single_v(lbm_ctx *c, int n, const Relax<T> &rp) {
         return c->idx32 ? step_single_vi<V, uint32_t, MRT, FORCE>(c, n, rp) : step_single_vi<V, int64_t, MRT, FORCE>(c, n, rp);
     }
 
-    template <int V, typename I, bool MRT, bool FORCE> static int step_single_vi(lbm_ctx *c, int n, const Relax<T> &rp) {
+    template <int V, typename I, bool MRT, int FORCE> static int step_single_vi(lbm_ctx *c, int n, const Relax<T> &rp) {
         const Launch l = span_launch(c, V);
         if (c->aa) {  // in place: even steps are local (V-node packs), odd steps move data (one node per thread)
             const Launch l1 = span_launch(c, 1);
@@ -204,7 +204,7 @@ template <class L, typename T> struct Impl {
         return LBM_OK;
     }
 
-    template <bool MRT, bool FORCE> static int step_single(lbm_ctx *c, int n, const Relax<T> &rp) {
+    template <bool MRT, int FORCE> static int step_single(lbm_ctx *c, int n, const Relax<T> &rp) {
         if constexpr (sizeof(T) == 4) {
             if (c->vec == 4) return step_single_v<4, MRT, FORCE>(c, n, rp);
         }
@@ -213,17 +213,19 @@ template <class L, typename T> struct Impl {
     }
 
     template <int V, int PSI> static int step_sc_v(lbm_ctx *c, int n) {
-        return c->idx32 ? step_sc_vi<V, uint32_t, PSI>(c, n) : step_sc_vi<V, int64_t, PSI>(c, n);
+        if (c->p.force_scheme == LBM_FORCE_EDM)
+            return c->idx32 ? step_sc_vi<V, uint32_t, PSI, FORCE_EDM>(c, n) : step_sc_vi<V, int64_t, PSI, FORCE_EDM>(c, n);
+        return c->idx32 ? step_sc_vi<V, uint32_t, PSI, FORCE_GUO>(c, n) : step_sc_vi<V, int64_t, PSI, FORCE_GUO>(c, n);
     }
 
-    template <int V, typename I, int PSI> static int step_sc_vi(lbm_ctx *c, int n) {
+    template <int V, typename I, int PSI, int FS> static int step_sc_vi(lbm_ctx *c, int n) {
         const Launch l = span_launch(c, V);
         const Relax<T> rA = make_relax<T>(c, 0), rB = make_relax<T>(c, 1);
         auto *psi = at<typename Pair<T>::type>(c, c->lay.psi[0]);
         for (int t = 0; t < n; t++) {
             sc_fields_kernel<L, T, V, I, PSI><<<l.grid, l.block, 0, c->stream>>>(c->g, type(c), link(c), src(c, 0), src(c, 1), psi);
             if (int rc = check_launch(c, "sc_fields_kernel")) return rc;
-            sc_step_kernel<L, T, V, I, PSI><<<l.grid, l.block, 0, c->stream>>>(
+            sc_step_kernel<L, T, V, I, PSI, FS><<<l.grid, l.block, 0, c->stream>>>(
                 c->g, type(c), link(c), src(c, 0), src(c, 1), dst(c, 0), dst(c, 1), psi, rA, rB, T(c->p.sc_G));
             if (int rc = check_launch(c, "sc_step_kernel")) return rc;
             c->cur ^= 1;
@@ -243,14 +245,18 @@ template <class L, typename T> struct Impl {
         if (c->p.model == LBM_SC2) return c->p.sc_psi == LBM_PSI_RHO ? step_sc<0>(c, n) : step_sc<1>(c, n);
         Relax<T> rp = make_relax<T>(c, 0);
         const bool force = c->p.force[0] != 0.0 || c->p.force[1] != 0.0 || c->p.force[2] != 0.0;
+        const bool edm = c->p.force_scheme == LBM_FORCE_EDM;
         if (c->p.model == LBM_MRT) {
             for (int k = 0; k < L::Q; k++) {  // M^-1 = M^T diag(1/|M_k|^2): rows are orthogonal (A5)
                 rp.cr[k] = T(c->p.rates[k] / Mrt<L, T>::norm(k));
                 rp.cs[k] = T((1.0 - 0.5 * c->p.rates[k]) / Mrt<L, T>::norm(k));
+                rp.in[k] = T(1.0 / Mrt<L, T>::norm(k));
             }
-            return force ? step_single<true, true>(c, n, rp) : step_single<true, false>(c, n, rp);
+            if (!force) return step_single<true, FORCE_NONE>(c, n, rp);
+            return edm ? step_single<true, FORCE_EDM>(c, n, rp) : step_single<true, FORCE_GUO>(c, n, rp);
         }
-        return force ? step_single<false, true>(c, n, rp) : step_single<false, false>(c, n, rp);
+        if (!force) return step_single<false, FORCE_NONE>(c, n, rp);
+        return edm ? step_single<false, FORCE_EDM>(c, n, rp) : step_single<false, FORCE_GUO>(c, n, rp);
     }
 
     static const Vtbl *table() {

@@ -288,7 +288,7 @@ __device__ __forceinline__ void store_span(T *__restrict__ dst, int64_t N, int n
 }
 
 // Collision by node type (t = the node's type byte).
-template <class L, typename T, bool MRT, bool FORCE>
+template <class L, typename T, bool MRT, int FORCE>
 __device__ __forceinline__ void update_typed(T (&h)[L::Q], uint32_t t, const Relax<T> &rp) {
     if (t & NODE_FULLWAY) fullway_reverse<L, T>(h);
     else if (t & NODE_VELOCITY) velocity_node<L, T>(h, rp.ubc);
@@ -296,7 +296,7 @@ __device__ __forceinline__ void update_typed(T (&h)[L::Q], uint32_t t, const Rel
 }
 
 // All nodes of a pack; packs without FULLWAY / VELOCITY nodes take the branch-free path.
-template <class L, typename T, int V, bool MRT, bool FORCE>
+template <class L, typename T, int V, bool MRT, int FORCE>
 __device__ __forceinline__ void update_span(T (&h)[V][L::Q], uint32_t types, const Relax<T> &rp) {
     if ((types & PACK_SPECIAL) == 0) {
 #pragma unroll
@@ -309,7 +309,7 @@ __device__ __forceinline__ void update_span(T (&h)[V][L::Q], uint32_t types, con
 
 // ---- the fused step: pull-stream + moments + equilibrium + collision (+ Guo) + store ---------
 // Rows a1-a8 of DESIGN.md.  All loads of the pack are issued before first use (bytes in flight).
-template <class L, typename T, int V, typename I, bool MRT, bool FORCE>
+template <class L, typename T, int V, typename I, bool MRT, int FORCE>
 __global__ void __launch_bounds__(256)
 step_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restrict__ link,
             const T *__restrict__ src, T *__restrict__ dst, Relax<T> rp) {
@@ -420,7 +420,7 @@ __device__ __forceinline__ I aa_slot(int parity, int i, int n, int64_t N, const 
     return reflected(link, i) ? I(i) * I(N) + I(n) : I(L::opp(i)) * I(N) + I(n + shift<L>(i, -1, o));
 }
 
-template <class L, typename T, int V, typename I, bool MRT, bool FORCE>
+template <class L, typename T, int V, typename I, bool MRT, int FORCE>
 __global__ void __launch_bounds__(256)
 aa_even_kernel(Geom g, const uint8_t *__restrict__ type, T *f, Relax<T> rp) {
     Span s;
@@ -446,7 +446,7 @@ aa_even_kernel(Geom g, const uint8_t *__restrict__ type, T *f, Relax<T> rp) {
     }
 }
 
-template <class L, typename T, typename I, bool MRT, bool FORCE>
+template <class L, typename T, typename I, bool MRT, int FORCE>
 __global__ void __launch_bounds__(256)
 aa_odd_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restrict__ link, T *f, Relax<T> rp) {
     Span s;
@@ -608,7 +608,7 @@ __device__ __forceinline__ void psi_gradient(const typename Pair<T>::type *__res
 
 // Pass 2 (rows a10-a11): both components in one kernel: gather, moments, common velocity u'
 // (P:188), forces (eq. 10, sign A11) + body force, v_s = u' + F_s / (2 rho_s), LBGK + Guo (A13).
-template <class L, typename T, int V, typename I, int PSI>
+template <class L, typename T, int V, typename I, int PSI, int FS>
 __global__ void __launch_bounds__(256)
 sc_step_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restrict__ link,
                const T *__restrict__ srcA, const T *__restrict__ srcB, T *__restrict__ dstA,
@@ -651,13 +651,14 @@ sc_step_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restr
             const T up = (jA[a] * rpA.inv_tau + jB[a] * rpB.inv_tau) * inv_den;
             FA[a] = -G * pA * SB[a] + rA * rpA.g[a];
             FB[a] = -G * pB * SA[a] + rB * rpB.g[a];
-            vA[a] = up + FA[a] * irA;
-            vB[a] = up + FB[a] * irB;
+            // Guo: v_s = u' + F_s / (2 rho_s) (A13); EDM: the bare common velocity u' (A22)
+            vA[a] = FS == FORCE_EDM ? up : up + FA[a] * irA;
+            vB[a] = FS == FORCE_EDM ? up : up + FB[a] * irB;
             mA[a] = rA * vA[a];
             mB[a] = rB * vB[a];
         }
-        collide<L, T, false, true>(hA[k], rA, dA, vA, mA, FA, rpA);
-        collide<L, T, false, true>(hB[k], rB, dB, vB, mB, FB, rpB);
+        collide<L, T, false, FS>(hA[k], rA, dA, vA, mA, FA, rpA);
+        collide<L, T, false, FS>(hB[k], rB, dB, vB, mB, FB, rpB);
     }
     store_span<L, T, V, I>(dstA, g.N, n0, hA);
     store_span<L, T, V, I>(dstB, g.N, n0, hB);

@@ -18,6 +18,8 @@ template <typename T> struct Relax {
     T src_scale;      // 1 - omega / 2, prefactor of eq. (17)
     // omega / 36 and (1 - omega / 2) / 36 as unevaluated sums hi + lo of two T (see collide()):
     T om36_hi, om36_lo, sc36_hi, sc36_lo;
+    T i36_hi, i36_lo; // 1 / 36 likewise (Exact Difference Method)
+    T in[19];         // MRT: 1 / |M_k|^2 (Exact Difference Method increment)
     T g[3];           // body acceleration
     T ubc[3];         // velocity imposed on equilibrium-velocity nodes (reading A21)
     T cr[19];         // MRT: rate_k / |M_k|^2                 (relaxation, eq. 4)
@@ -37,6 +39,7 @@ template <typename T> inline void set_bgk(Relax<T> &r, double tau) {
     r.src_scale = T(1.0 - 0.5 * om);
     r.om36_hi = T(c); r.om36_lo = T(c - double(r.om36_hi));
     r.sc36_hi = T(s); r.sc36_lo = T(s - double(r.sc36_hi));
+    r.i36_hi = T(1.0 / 36.0); r.i36_lo = T(1.0 / 36.0 - double(r.i36_hi));
 }
 
 template <class L, typename T> LBM_HD void moments(const T (&h)[L::Q], T &drho, T (&j)[3]) {
@@ -212,10 +215,14 @@ template <typename T> struct Mrt<D2Q9, T> {
     }
 };
 
+// FORCE: 0 no body force, 1 Guo (eq. 17), 2 Exact Difference Method (eq. 18).
+constexpr int FORCE_NONE = 0, FORCE_GUO = 1, FORCE_EDM = 2;
+
 // ---- collision: h (pre-collision deviations) -> h* (post-collision), in place ---------------
 // rho, drho = rho - 1, v = velocity entering f^eq and eq. (17) (reading A3), rv = rho v as formed
-// from the moments (j + F/2, eq. 16), F = force density.
-template <class L, typename T, bool MRT, bool FORCE>
+// from the moments (j + F/2, eq. 16), F = force density.  With FORCE_EDM v is the bare velocity u
+// (reading A22), rv = rho u, and the routine adds f^eq(rho, u + F/rho) - f^eq(rho, u).
+template <class L, typename T, bool MRT, int FORCE>
 LBM_HD void collide(T (&h)[L::Q], T rho, T drho, const T (&v)[3], const T (&rv)[3], const T (&F)[3], const Relax<T> &rp) {
     constexpr int Q = L::Q;
     if constexpr (!MRT) {
@@ -231,6 +238,38 @@ LBM_HD void collide(T (&h)[L::Q], T rho, T drho, const T (&v)[3], const T (&rv)[
         // two-term sum hi + lo (rounding then depends on the node's data, not on a constant), and
         // the old value is scaled by keep = 1 - omega, which set_bgk makes exact for the omega in use.
         const T keep = rp.keep;
+        if constexpr (FORCE == FORCE_EDM) {
+            // h* = keep h + h^eq(u2) - keep h^eq(u), u2 = u + F/rho, in the same even/odd form:
+            //   odd  = 3 e.(rho u2 - keep rho u) = 3 e.(omega rho u + F)   (momentum gains exactly F)
+            //   even = omega drho - 1.5 rho (u2^2 - keep u^2) + 4.5 rho ((e.u2)^2 - keep (e.u)^2)
+            const T inv_rho = T(1) / rho;
+            T u2[3], mo[3];
+#pragma unroll
+            for (int a = 0; a < 3; a++) {
+                u2[a] = v[a] + F[a] * inv_rho;
+                const T t = T(3) * rv[a], f3 = T(3) * F[a];
+                mo[a] = (t * rp.om36_hi + t * rp.om36_lo) + (f3 * rp.i36_hi + f3 * rp.i36_lo);
+            }
+            const T vv = v[0] * v[0] + v[1] * v[1] + v[2] * v[2];
+            const T vv2 = u2[0] * u2[0] + u2[1] * u2[1] + u2[2] * u2[2];
+            const T b0 = rp.inv_tau * drho - rho * (T(1.5) * (vv2 - keep * vv)), q0 = T(4.5) * rho;
+            const T base = b0 * rp.i36_hi + b0 * rp.i36_lo;
+            const T r45 = q0 * rp.i36_hi + q0 * rp.i36_lo;
+            h[0] = keep * h[0] + T(L::w36(0)) * base;
+#pragma unroll
+            for (int i = 1; i < Q; i++) {
+                if (i < L::opp(i)) {
+                    const int j = L::opp(i);
+                    const T wi = T(L::w36(i));
+                    const T ev = e_dot<L, T>(i, v), ev2 = e_dot<L, T>(i, u2);
+                    const T odd = e_dot<L, T>(i, mo);
+                    const T even = base + r45 * (ev2 * ev2 - keep * (ev * ev));
+                    h[i] = keep * h[i] + wi * (even + odd);
+                    h[j] = keep * h[j] + wi * (even - odd);
+                }
+            }
+            return;
+        }
         const T vv = v[0] * v[0] + v[1] * v[1] + v[2] * v[2];
         const T b0 = drho - rho * (T(1.5) * vv), q0 = T(4.5) * rho;
         const T base = b0 * rp.om36_hi + b0 * rp.om36_lo;
@@ -281,7 +320,7 @@ LBM_HD void collide(T (&h)[L::Q], T rho, T drho, const T (&v)[3], const T (&rv)[
         Mrt<L, T>::forward(d, m);
 #pragma unroll
         for (int k = 0; k < Q; k++) m[k] *= rp.cr[k];
-        if constexpr (FORCE) {
+        if constexpr (FORCE == FORCE_GUO) {
             T src[Q], ms[Q];
             guo_bracket<L, T>(v, F, src);
             Mrt<L, T>::forward(src, ms);
@@ -291,11 +330,20 @@ LBM_HD void collide(T (&h)[L::Q], T rho, T drho, const T (&v)[3], const T (&rv)[
         Mrt<L, T>::backward(m, d);
 #pragma unroll
         for (int i = 0; i < Q; i++) h[i] += d[i];
+        if constexpr (FORCE == FORCE_EDM) {
+            const T inv_rho = T(1) / rho;
+            T u2[3], heq2[Q];
+#pragma unroll
+            for (int a = 0; a < 3; a++) u2[a] = v[a] + F[a] * inv_rho;
+            equilibrium_dev<L, T>(rho, drho, u2, heq2);
+#pragma unroll
+            for (int i = 0; i < Q; i++) h[i] += heq2[i] - heq[i];
+        }
     }
 }
 
 // Single-component node update: moments, F = rho g, v = j/rho + g/2 (eq. 16), collide.
-template <class L, typename T, bool MRT, bool FORCE>
+template <class L, typename T, bool MRT, int FORCE>
 LBM_HD void update_node(T (&h)[L::Q], const Relax<T> &rp) {
     constexpr int Q = L::Q;
     if constexpr (MRT && Mrt<L, T>::closed_form_meq) {
@@ -309,13 +357,21 @@ LBM_HD void update_node(T (&h)[L::Q], const Relax<T> &rp) {
         for (int a = 0; a < 3; a++) {
             const T ja = m[3 + 2 * a];
             F[a] = FORCE ? rho * rp.g[a] : T(0);
-            v[a] = FORCE ? (ja + T(0.5) * F[a]) * inv_rho : ja * inv_rho;
+            v[a] = FORCE == FORCE_GUO ? (ja + T(0.5) * F[a]) * inv_rho : ja * inv_rho;
         }
         T q[Q];
         Mrt<L, T>::meq_dev(rho, drho, v, q);
 #pragma unroll
         for (int k = 0; k < Q; k++) m[k] = rp.cr[k] * (q[k] - m[k]);
-        if constexpr (FORCE) {
+        if constexpr (FORCE == FORCE_EDM) {  // + M^-1 (m^eq(u + F/rho) - m^eq(u)), eq. (18)
+            T u2[3], q2[Q];
+#pragma unroll
+            for (int a = 0; a < 3; a++) u2[a] = v[a] + F[a] * inv_rho;
+            Mrt<L, T>::meq_dev(rho, drho, u2, q2);
+#pragma unroll
+            for (int k = 0; k < Q; k++) m[k] += rp.in[k] * (q2[k] - q[k]);
+        }
+        if constexpr (FORCE == FORCE_GUO) {
             T src[Q], ms[Q];
             guo_bracket<L, T>(v, F, src);
             Mrt<L, T>::forward(src, ms);
@@ -334,7 +390,7 @@ LBM_HD void update_node(T (&h)[L::Q], const Relax<T> &rp) {
 #pragma unroll
         for (int a = 0; a < 3; a++) {
             F[a] = FORCE ? rho * rp.g[a] : T(0);
-            rv[a] = FORCE ? j[a] + T(0.5) * F[a] : j[a];
+            rv[a] = FORCE == FORCE_GUO ? j[a] + T(0.5) * F[a] : j[a];
             v[a] = rv[a] * inv_rho;
         }
         collide<L, T, MRT, FORCE>(h, rho, drho, v, rv, F, rp);

@@ -6,7 +6,7 @@
 
 using namespace lbm;
 
-template <class L, typename T, bool MRT, bool FORCE>
+template <class L, typename T, bool MRT, int FORCE>
 static void run(const double *f, double tau, const double *rates, const double *g, double *out) {
     Relax<T> rp{};
     set_bgk(rp, tau);
@@ -14,6 +14,7 @@ static void run(const double *f, double tau, const double *rates, const double *
     for (int k = 0; k < L::Q; k++) {
         rp.cr[k] = T(rates[k] / Mrt<L, double>::norm(k));
         rp.cs[k] = T((1.0 - 0.5 * rates[k]) / Mrt<L, double>::norm(k));
+        rp.in[k] = T(1.0 / Mrt<L, double>::norm(k));
     }
     T h[L::Q];
     for (int i = 0; i < L::Q; i++) h[i] = T(f[i] - L::template w<double>(i));
@@ -23,8 +24,16 @@ static void run(const double *f, double tau, const double *rates, const double *
 
 template <class L, typename T>
 static void dispatch(int mrt, int force, const double *f, double tau, const double *rates, const double *g, double *out) {
-    if (mrt) { if (force) run<L, T, true, true>(f, tau, rates, g, out); else run<L, T, true, false>(f, tau, rates, g, out); }
-    else     { if (force) run<L, T, false, true>(f, tau, rates, g, out); else run<L, T, false, false>(f, tau, rates, g, out); }
+    // force: 0 none, 1 Guo (eq. 17), 2 Exact Difference Method (eq. 18)
+    if (mrt) {
+        if (force == 2) run<L, T, true, 2>(f, tau, rates, g, out);
+        else if (force) run<L, T, true, 1>(f, tau, rates, g, out);
+        else run<L, T, true, 0>(f, tau, rates, g, out);
+    } else {
+        if (force == 2) run<L, T, false, 2>(f, tau, rates, g, out);
+        else if (force) run<L, T, false, 1>(f, tau, rates, g, out);
+        else run<L, T, false, 0>(f, tau, rates, g, out);
+    }
 }
 
 extern "C" int host_update_node(int lattice, int f32, int mrt, int force, const double *f, double tau,

@@ -47,7 +47,7 @@ def test_mrt_transforms_match_oracle_matrix(host, orc, lattice):
 
 @pytest.mark.parametrize("lattice", [wl.D2Q9, wl.D3Q19])
 @pytest.mark.parametrize("mrt", [0, 1])
-@pytest.mark.parametrize("force", [0, 1])
+@pytest.mark.parametrize("force", [0, 1, 2])  # none | Guo (eq. 17) | Exact Difference Method (eq. 18)
 @pytest.mark.parametrize("f32", [0, 1])
 def test_update_node_matches_oracle_collision(host, orc, lattice, mrt, force, f32):
     rng = np.random.default_rng(100 * lattice + 10 * mrt + force)
@@ -56,12 +56,13 @@ def test_update_node_matches_oracle_collision(host, orc, lattice, mrt, force, f3
     rates = np.array(wl.mrt_rates_d2q9(tau) if lattice == wl.D2Q9 else wl.mrt_rates_d3q19(tau))
     # conserved-moment rates are given non-zero here so that the force path exercises them
     rates = np.where(rates == 0.0, 0.7, rates)
-    g = np.array([3e-4, -2e-4, 1e-4 if lattice == wl.D3Q19 else 0.0]) * force
+    g = np.array([3e-4, -2e-4, 1e-4 if lattice == wl.D3Q19 else 0.0]) * (force != 0)
     for trial in range(5):
         v = rng.uniform(-0.05, 0.05, 3)
         f = orc.feq(lattice, 1.0 + rng.uniform(-0.05, 0.05), v[: 2 if lattice == wl.D2Q9 else 3])
         f = f * (1.0 + rng.uniform(-0.05, 0.05, Q))          # off equilibrium
-        o = orc.Oracle(lattice, wl.MRT if mrt else wl.BGK, 1, 1, 1, tau=tau, rates=list(rates), force=tuple(g))
+        o = orc.Oracle(lattice, wl.MRT if mrt else wl.BGK, 1, 1, 1, tau=tau, rates=list(rates), force=tuple(g),
+                       force_scheme=1 if force == 2 else 0)
         o.set_distributions(f.reshape(Q, 1, 1, 1))
         o.step(1)
         ref = o.get_distributions().ravel()

@@ -256,3 +256,26 @@ def test_all_node_types_shan_chen(B, orc):
 def test_lid_driven_cavity_reduced(B, orc, precision):
     """The paper's benchmark box at 40 x 36 x 32: full-way walls, equilibrium-velocity lid."""
     check_parity_live(B, orc, W.ldc_cavity(40, 36, 32, precision=precision))
+
+
+# ---- NEXT-3: Exact Difference Method force scheme (eq. 18, P:253-258; reading A22) --------------------
+@pytest.mark.parametrize("store", ["ab", "aa"])
+@pytest.mark.parametrize("lattice,model,precision,shape", [
+    (W.D3Q19, W.BGK, W.F32, (48, 21, 10)), (W.D3Q19, W.BGK, W.F64, (37, 14, 9)), (W.D3Q19, W.MRT, W.F32, (40, 12, 11)),
+    (W.D3Q19, W.MRT, W.F64, (26, 12, 7)), (W.D2Q9, W.BGK, W.F32, (66, 31, 1)), (W.D2Q9, W.MRT, W.F64, (52, 30, 1))])
+def test_edm_single_component(B, orc, lattice, model, precision, shape, store):
+    nx, ny, nz = shape
+    D = 2 if lattice == W.D2Q9 else 3
+    w = generic(lattice, model, precision, shape, 61, tau=(0.7, 0.7), force_scheme=W.FORCE_EDM,
+                rates=(W.mrt_rates_d3q19(0.7) if lattice == W.D3Q19 else W.mrt_rates_d2q9(0.7)) if model == W.MRT else None,
+                force=(1e-4, -2e-4, 3e-4 if D == 3 else 0.0))
+    check_parity_live(B, orc, w, store=B.LBM_STORE_AA if store == "aa" else B.LBM_STORE_AB)
+
+
+@pytest.mark.parametrize("precision,lattice,shape", [(W.F32, W.D3Q19, (32, 20, 12)), (W.F64, W.D3Q19, (21, 14, 9)),
+                                                     (W.F64, W.D2Q9, (40, 33, 1))])
+def test_edm_shan_chen(B, orc, precision, lattice, shape):
+    """Shan-Chen with the EDM, tau_A != tau_B, body force: the paper's binary Poiseuille set-up."""
+    w = generic(lattice, W.SC2, precision, shape, 62, solid=0.05, tau=(1.0, 0.625), sc_G=0.9,
+                force=(1e-5, 2e-5, 0.0), force_scheme=W.FORCE_EDM)
+    check_parity_live(B, orc, w, steps=60)
