@@ -15,10 +15,13 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "liblbm_b200.so")
 OBJDIR = os.path.join(_HERE, "build")
-# one translation unit for the C ABI and one per <lattice, real> pair of kernel instantiations
-SOURCES = [os.path.join(CSRC, n) for n in ("lbm_b200.cu", "lbm_impl_d2q9_f32.cu", "lbm_impl_d2q9_f64.cu",
-                                           "lbm_impl_d3q19_f32.cu", "lbm_impl_d3q19_f64.cu")]
-HEADERS = [os.path.join(CSRC, n) for n in ("lbm_impl.cuh", "lbm_kernels.cuh", "lbm_node.cuh", "lbm_lattice.cuh")] + [
+# one translation unit for the C ABI, one per <lattice, real> pair for the conversion kernels, and
+# one per <lattice, real, model> for the step kernels: they are independent and compile side by side
+SOURCES = [os.path.join(CSRC, "lbm_b200.cu")] + [
+    os.path.join(CSRC, "lbm_impl_%s_%s.cu" % (lat, pr)) for lat in ("d2q9", "d3q19") for pr in ("f32", "f64")] + [
+    os.path.join(CSRC, "lbm_step_%s_%s_%s.cu" % (lat, pr, m))
+    for lat in ("d3q19", "d2q9") for pr in ("f32", "f64") for m in ("bgk", "mrt", "sc")]
+HEADERS = [os.path.join(CSRC, n) for n in ("lbm_impl.cuh", "lbm_steps.cuh", "lbm_kernels.cuh", "lbm_node.cuh", "lbm_lattice.cuh")] + [
     os.path.join(os.path.dirname(_HERE), "include", "lbm.h")]
 
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
@@ -44,12 +47,19 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if force or stale():
         os.makedirs(OBJDIR, exist_ok=True)
         extra = (["-Xptxas", "-v"] if verbose else []) + os.environ.get("LBM_NVCC_EXTRA", "").split()
-        objs, procs = [], []
-        for src in SOURCES:  # the translation units are independent: compile them side by side
+        objs, jobs = [], []
+        for src in SOURCES:
             obj = os.path.join(OBJDIR, os.path.basename(src)[:-3] + ".o")
             objs.append(obj)
-            procs.append((src, subprocess.Popen([nvcc()] + NVCC_FLAGS + extra + ["-c", "-o", obj, src])))
-        failed = [src for src, p in procs if p.wait() != 0]
+            jobs.append((src, [nvcc()] + NVCC_FLAGS + extra + ["-c", "-o", obj, src]))
+        failed, running, width = [], [], max(2, os.cpu_count() or 2)
+        while jobs or running:  # at most one nvcc per core
+            while jobs and len(running) < width:
+                src, cmd = jobs.pop(0)
+                running.append((src, subprocess.Popen(cmd)))
+            src, proc = running.pop(0)
+            if proc.wait() != 0:
+                failed.append(src)
         if failed:
             raise RuntimeError("nvcc failed on " + ", ".join(failed))
         tmp = LIB + ".tmp.%d" % os.getpid()

@@ -1,0 +1,107 @@
+// lbm_steps.cuh -- host-side launch loops of the step kernels (rows a1-a12), included by the
+// lbm_step_*.cu translation units, which instantiate one model each for one <lattice, real> pair.
+#pragma once
+#include "lbm_impl.cuh"
+
+namespace {
+
+template <class L, typename T> struct Steps {
+    static const T *src(lbm_ctx *c, int s) { return at<T>(c, c->lay.store[s][c->cur]); }
+    static T *dst(lbm_ctx *c, int s) { return at<T>(c, c->lay.store[s][c->cur ^ 1]); }
+    static uint8_t *type(lbm_ctx *c) { return at<uint8_t>(c, c->lay.type); }
+    static uint32_t *link(lbm_ctx *c) { return at<uint32_t>(c, c->lay.link); }
+
+    template <int V, bool MRT, int FORCE> static int step_single_v(lbm_ctx *c, int n, const Relax<T> &rp) {
+        return c->idx32 ? step_single_vi<V, uint32_t, MRT, FORCE>(c, n, rp) : step_single_vi<V, int64_t, MRT, FORCE>(c, n, rp);
+    }
+
+    template <int V, typename I, bool MRT, int FORCE> static int step_single_vi(lbm_ctx *c, int n, const Relax<T> &rp) {
+        const Launch l = span_launch(c, V);
+        if (c->aa) {  // in place: even steps are local (V-node packs), odd steps move data (one node per thread)
+            const Launch l1 = span_launch(c, 1);
+            T *f = at<T>(c, c->lay.store[0][0]);
+            for (int t = 0; t < n; t++) {
+                if (c->cur == 0) aa_even_kernel<L, T, V, I, MRT, FORCE><<<l.grid, l.block, 0, c->stream>>>(c->g, type(c), f, rp);
+                else aa_odd_kernel<L, T, I, MRT, FORCE><<<l1.grid, l1.block, 0, c->stream>>>(c->g, type(c), link(c), f, rp);
+                if (int rc = check_launch(c, "aa_step_kernel")) return rc;
+                c->cur ^= 1;
+                c->steps++;
+            }
+            return LBM_OK;
+        }
+        for (int t = 0; t < n; t++) {
+            step_kernel<L, T, V, I, MRT, FORCE><<<l.grid, l.block, 0, c->stream>>>(c->g, type(c), link(c), src(c, 0), dst(c, 0), rp);
+            if (int rc = check_launch(c, "step_kernel")) return rc;
+            c->cur ^= 1;
+            c->steps++;
+        }
+        return LBM_OK;
+    }
+
+    template <bool MRT, int FORCE> static int step_single(lbm_ctx *c, int n, const Relax<T> &rp) {
+        if constexpr (sizeof(T) == 4) {
+            if (c->vec == 4) return step_single_v<4, MRT, FORCE>(c, n, rp);
+        }
+        if (c->vec == 2) return step_single_v<2, MRT, FORCE>(c, n, rp);
+        return step_single_v<1, MRT, FORCE>(c, n, rp);
+    }
+
+    template <int V, int PSI> static int step_sc_v(lbm_ctx *c, int n) {
+        if (c->p.force_scheme == LBM_FORCE_EDM)
+            return c->idx32 ? step_sc_vi<V, uint32_t, PSI, FORCE_EDM>(c, n) : step_sc_vi<V, int64_t, PSI, FORCE_EDM>(c, n);
+        return c->idx32 ? step_sc_vi<V, uint32_t, PSI, FORCE_GUO>(c, n) : step_sc_vi<V, int64_t, PSI, FORCE_GUO>(c, n);
+    }
+
+    template <int V, typename I, int PSI, int FS> static int step_sc_vi(lbm_ctx *c, int n) {
+        const Launch l = span_launch(c, V);
+        const Relax<T> rA = make_relax<T>(c, 0), rB = make_relax<T>(c, 1);
+        auto *psi = at<typename Pair<T>::type>(c, c->lay.psi[0]);
+        for (int t = 0; t < n; t++) {
+            sc_fields_kernel<L, T, V, I, PSI><<<l.grid, l.block, 0, c->stream>>>(c->g, type(c), link(c), src(c, 0), src(c, 1), psi);
+            if (int rc = check_launch(c, "sc_fields_kernel")) return rc;
+            sc_step_kernel<L, T, V, I, PSI, FS><<<l.grid, l.block, 0, c->stream>>>(
+                c->g, type(c), link(c), src(c, 0), src(c, 1), dst(c, 0), dst(c, 1), psi, rA, rB, T(c->p.sc_G));
+            if (int rc = check_launch(c, "sc_step_kernel")) return rc;
+            c->cur ^= 1;
+            c->steps++;
+        }
+        return LBM_OK;
+    }
+
+    template <int PSI> static int step_sc(lbm_ctx *c, int n) {
+        if constexpr (sizeof(T) == 4) {  // fp64 with two components and V = 2 would spill
+            if (c->vec >= 2) return step_sc_v<2, PSI>(c, n);
+        }
+        return step_sc_v<1, PSI>(c, n);
+    }
+
+    template <bool MRT> static int step_model(lbm_ctx *c, int n) {
+        Relax<T> rp = make_relax<T>(c, 0);
+        const bool force = c->p.force[0] != 0.0 || c->p.force[1] != 0.0 || c->p.force[2] != 0.0;
+        const bool edm = c->p.force_scheme == LBM_FORCE_EDM;
+        if (MRT)
+            for (int k = 0; k < L::Q; k++) {  // M^-1 = M^T diag(1/|M_k|^2): rows are orthogonal (A5)
+                rp.cr[k] = T(c->p.rates[k] / Mrt<L, T>::norm(k));
+                rp.cs[k] = T((1.0 - 0.5 * c->p.rates[k]) / Mrt<L, T>::norm(k));
+                rp.in[k] = T(1.0 / Mrt<L, T>::norm(k));
+            }
+        if (!force) return step_single<MRT, FORCE_NONE>(c, n, rp);
+        return edm ? step_single<MRT, FORCE_EDM>(c, n, rp) : step_single<MRT, FORCE_GUO>(c, n, rp);
+    }
+
+    static int step_shan_chen(lbm_ctx *c, int n) {
+        return c->p.sc_psi == LBM_PSI_RHO ? step_sc<0>(c, n) : step_sc<1>(c, n);
+    }
+};
+
+}  // namespace
+
+// Which model a translation unit instantiates is chosen by the macro it defines before including
+// this header: LBM_STEP_BGK, LBM_STEP_MRT or LBM_STEP_SC.
+#if defined(LBM_STEP_BGK)
+template <class L, typename T> int lbm_step_bgk(lbm_ctx *c, int n) { return Steps<L, T>::template step_model<false>(c, n); }
+#elif defined(LBM_STEP_MRT)
+template <class L, typename T> int lbm_step_mrt(lbm_ctx *c, int n) { return Steps<L, T>::template step_model<true>(c, n); }
+#elif defined(LBM_STEP_SC)
+template <class L, typename T> int lbm_step_sc(lbm_ctx *c, int n) { return Steps<L, T>::step_shan_chen(c, n); }
+#endif
