@@ -34,8 +34,8 @@ from paper_1311_2404_b200 import workloads as W  # noqa: E402
 METRIC = "MLUPS on 1 B200 and achieved HBM GB/s as % of peak (D3Q19 LBGK fp32)"
 UNIT = "MLUPS"
 # ncu --set full: dram__bytes_read.sum + dram__bytes_write.sum per step (one step_kernel launch;
-# for c5 the sc_fields + sc_step pair), from the committed captures in profiles/r01c_step_kernels.md.
-NCU_TRAFFIC_BYTES = {"c2": 2.499e9, "c3": 8.921e9, "c4": 10.048e9, "c5": 7.902e9}
+# for c5 the sc_fields + sc_step pair), from the committed captures in profiles/r01d_step_kernels.md.
+NCU_TRAFFIC_BYTES = {"c2": 2.497e9, "c3": 8.922e9, "c4": 10.048e9, "c5": 7.903e9, "ldc": 2.506e9}
 
 
 def algorithmic_bytes_per_site(w) -> float:
