@@ -60,7 +60,7 @@
 #endif
 
 enum { ORC_D2Q9 = 0, ORC_D3Q19 = 1 };
-enum { ORC_BGK = 0, ORC_MRT = 1, ORC_SC2 = 2 };
+enum { ORC_BGK = 0, ORC_MRT = 1, ORC_SC2 = 2, ORC_REG = 3, ORC_LES = 4 };
 enum { ORC_PSI_RHO = 0, ORC_PSI_1MEXP = 1 };
 #define ORC_QMAX 19
 /* node types (P:446 reduced; readings A8, A20, A21) */
@@ -77,6 +77,7 @@ typedef struct {
     int32_t sc_psi;
     double bc_velocity[3]; /* velocity imposed on ORC_VELOCITY nodes (reading A21) */
     int32_t force_scheme;  /* ORC_FORCE_GUO (eq. 17) | ORC_FORCE_EDM (eq. 18) */
+    double smagorinsky_cs; /* C_S of eq. (9), ORC_LES only */
 } orc_params;
 
 /* ---- velocity sets (reading A2; weights from Table 1) ------------- */
@@ -274,7 +275,9 @@ orc_ctx *orc_create(const orc_params *p)
     if (!c) return NULL;
     c->p = *p;
     if (lattice_fill(p->lattice, &c->L) || p->nx < 1 || p->ny < 1 || p->nz < 1 ||
-        (p->lattice == ORC_D2Q9 && p->nz != 1) || p->model < ORC_BGK || p->model > ORC_SC2) {
+        (p->lattice == ORC_D2Q9 && p->nz != 1) || p->model < ORC_BGK || p->model > ORC_LES ||
+        (p->model == ORC_REG && p->force_scheme == ORC_FORCE_GUO &&
+         (p->force[0] != 0 || p->force[1] != 0 || p->force[2] != 0))) { /* reading A23 */
         free(c);
         return NULL;
     }
@@ -364,6 +367,40 @@ static void collide_node(const orc_ctx *c, const double *f, double rho, const do
     const lattice_t *L = &c->L;
     const int Q = L->Q;
     double fe[ORC_QMAX], src[ORC_QMAX];
+    double freg_store[ORC_QMAX];
+    if (c->p.model == ORC_REG) {
+        /* Regularized LBGK, P:130 (reading A23): replace f^neq = f - f^eq by its projection
+         * f^reg_i = w_i / (2 c_s^4) (e_ia e_ib - c_s^2 delta_ab) Pi^neq_ab,
+         * Pi^neq_ab = sum_i f^neq_i (e_ia e_ib - c_s^2 delta_ab), c_s^2 = 1/3; then collide as LBGK.
+         * The equilibrium is taken at the bare velocity (a force enters through the EDM only). */
+        double Pi[3][3] = {{0}};
+        feq(L, rho, ub, fe);
+        for (int i = 0; i < Q; i++)
+            for (int a = 0; a < 3; a++)
+                for (int b = 0; b < 3; b++)
+                    Pi[a][b] += (f[i] - fe[i]) * (L->e[i][a] * L->e[i][b] - (a == b ? 1.0 / 3.0 : 0.0));
+        for (int i = 0; i < Q; i++) {
+            double s = 0;
+            for (int a = 0; a < 3; a++)
+                for (int b = 0; b < 3; b++) s += (L->e[i][a] * L->e[i][b] - (a == b ? 1.0 / 3.0 : 0.0)) * Pi[a][b];
+            freg_store[i] = fe[i] + 4.5 * L->w[i] * s;
+        }
+        f = freg_store; /* "after this regularization step, the collision ... proceeds as in LBGK" */
+    }
+    if (c->p.model == ORC_LES) {
+        /* Smagorinsky subgrid model, eq. (8)-(9) P:164-173: tau = tau_0 + tau_t,
+         * tau_t = ( sqrt(tau_0^2 + 4 c_s^-4 C_S^2 |Q|) - tau_0 ) / 2, Q_ab = sum_i e_ia e_ib (f_i - f^eq_i),
+         * |Q| = (Q_ab Q_ab)^(1/2); f^eq at the velocity the collision uses (Guo: v, EDM: u). */
+        double Qt[3][3] = {{0}}, q2 = 0;
+        feq(L, rho, c->p.force_scheme == ORC_FORCE_EDM ? ub : v, fe);
+        for (int i = 0; i < Q; i++)
+            for (int a = 0; a < 3; a++)
+                for (int b = 0; b < 3; b++) Qt[a][b] += L->e[i][a] * L->e[i][b] * (f[i] - fe[i]);
+        for (int a = 0; a < 3; a++)
+            for (int b = 0; b < 3; b++) q2 += Qt[a][b] * Qt[a][b];
+        double cs = c->p.smagorinsky_cs;
+        tau = tau + 0.5 * (sqrt(tau * tau + 4.0 * 9.0 * cs * cs * sqrt(q2)) - tau);
+    }
     if (c->p.force_scheme == ORC_FORCE_EDM) {
         /* Exact Difference Method, eq. (18) P:253-258 (reading A22): relax towards f^eq(rho, u) at
          * the bare velocity u = ub (sum e f / rho; the common velocity u' for Shan-Chen) and add

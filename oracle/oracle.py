@@ -20,7 +20,7 @@ _LIB = os.path.join(_HERE, "liblbm_oracle.so")
 D2Q9, D3Q19 = 0, 1
 FLUID, SOLID, WALL_FULLWAY, VELOCITY = 0, 1, 2, 3
 FORCE_GUO, FORCE_EDM = 0, 1
-BGK, MRT, SC2 = 0, 1, 2
+BGK, MRT, SC2, REG, LES = 0, 1, 2, 3, 4
 PSI_RHO, PSI_1MEXP = 0, 1
 QMAX = 19
 
@@ -36,6 +36,7 @@ class _Params(C.Structure):
         ("sc_psi", C.c_int32),
         ("bc_velocity", C.c_double * 3),
         ("force_scheme", C.c_int32),
+        ("smagorinsky_cs", C.c_double),
     ]
 
 
@@ -114,7 +115,7 @@ class Oracle:
 
     def __init__(self, lattice, model, nx, ny, nz=1, tau=(1.0, 1.0), rates=None,
                  force=(0.0, 0.0, 0.0), sc_G=0.0, sc_psi=PSI_RHO, bc_velocity=(0.0, 0.0, 0.0),
-                 force_scheme=0):
+                 force_scheme=0, smagorinsky_cs=0.0):
         p = _Params()
         p.lattice, p.model = lattice, model
         p.nx, p.ny, p.nz = nx, ny, nz
@@ -127,6 +128,7 @@ class Oracle:
             p.force[a] = float(force[a]) if a < len(force) else 0.0
         p.sc_G, p.sc_psi = float(sc_G), int(sc_psi)
         p.force_scheme = int(force_scheme)
+        p.smagorinsky_cs = float(smagorinsky_cs)
         for a in range(3):
             p.bc_velocity[a] = float(bc_velocity[a]) if a < len(bc_velocity) else 0.0
         self._h = lib().orc_create(C.byref(p))

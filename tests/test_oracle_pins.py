@@ -765,3 +765,154 @@ def test_edm_step_against_numpy_roll_reference(orc, lat, shp):
         f = new
     o.step(12)
     assert np.max(np.abs(o.get_distributions() - f)[:, fluid]) < 1e-14
+
+
+# ---------------------------------------------------------------- NEXT-4: regularized LBGK and the
+# Smagorinsky subgrid model (eq. 8-9); reading A23
+def _np_step_bgk_variant(orc, lat, f, mask, tau, steps, variant, cs=0.0, g=None):
+    """Whole-array numpy LBGK step with half-way bounce-back; variant in {"reg", "les"}; force by EDM."""
+    e, w, opp = orc.lattice_tables(lat)
+    Q = len(e)
+    ef, fluid = e.astype(float), mask == 0
+    wq = w[:, None, None, None]
+    H = np.einsum("qa,qb->qab", ef, ef) - np.eye(3)[None] / 3.0
+    EE = np.einsum("qa,qb->qab", ef, ef)
+    g = np.zeros(3) if g is None else g
+
+    def feq(r, v):
+        ev = np.einsum("qa,azyx->qzyx", ef, v)
+        return r * wq * (1 + 3 * ev + 4.5 * ev ** 2 - 1.5 * (v ** 2).sum(0))
+
+    for _ in range(steps):
+        r = f.sum(0)
+        ub = np.einsum("qzyx,qa->azyx", f, ef) / r
+        fe = feq(r, ub)
+        t = tau
+        fin = f
+        if variant == "reg":
+            Pi = np.einsum("qzyx,qab->abzyx", f - fe, H)
+            fin = fe + 4.5 * wq * np.einsum("qab,abzyx->qzyx", H, Pi)
+        else:
+            Qt = np.einsum("qzyx,qab->abzyx", f - fe, EE)
+            t = tau + 0.5 * (np.sqrt(tau * tau + 36.0 * cs * cs * np.sqrt((Qt ** 2).sum((0, 1)))) - tau)
+        fs = fin + (fe - fin) / t + feq(r, ub + g[:, None, None, None]) - fe
+        new = f.copy()
+        for i in range(Q):
+            sh = (e[i][2], e[i][1], e[i][0])
+            moved = np.roll(fs[i], shift=sh, axis=(0, 1, 2))
+            from_solid = np.roll(mask, shift=sh, axis=(0, 1, 2)) == 1
+            new[i] = np.where(fluid, np.where(from_solid, fs[opp[i]], moved), f[i])
+        f = new
+    return f
+
+
+@pytest.mark.parametrize("lat,shp", [(0, (7, 6, 1)), (1, (5, 6, 4))])
+@pytest.mark.parametrize("variant", ["reg", "les"])
+def test_reg_and_les_step_against_numpy_reference(orc, lat, shp, variant):
+    from paper_1311_2404_b200 import workloads as W
+    nx, ny, nz = shp
+    D = 2 if lat == 0 else 3
+    mask, rho, u = W.random_state(lat, nx, ny, nz, seed=71, solid_fraction=0.2, du=0.05)
+    tau, cs = 0.6, 0.17
+    g = np.array([1e-4, -2e-4, 3e-4 if D == 3 else 0.0])
+    o = orc.Oracle(lat, orc.REG if variant == "reg" else orc.LES, nx, ny, nz, tau=tau, force=g,
+                   force_scheme=orc.FORCE_EDM, smagorinsky_cs=cs)
+    o.set_geometry(mask)
+    o.init_equilibrium(rho[0], u[0])
+    f = o.get_distributions().copy()
+    rng = np.random.default_rng(5)
+    f *= 1 + rng.uniform(-0.02, 0.02, f.shape)            # off equilibrium, so that Pi^neq and Q matter
+    o.set_distributions(f)
+    want = _np_step_bgk_variant(orc, lat, f.copy(), mask, tau, 8, variant, cs, g)
+    o.step(8)
+    assert np.max(np.abs(o.get_distributions() - want)[:, mask == 0]) < 1e-14
+
+
+@pytest.mark.parametrize("lat", [0, 1])
+def test_regularization_is_a_projection(orc, lat):
+    """If f^neq already has the form w_i/(2 c_s^4) (e e - c_s^2 delta) : S with S symmetric, the
+    regularization step changes nothing (sum_i w_i H_iab H_icd = (delta_ac delta_bd + delta_ad
+    delta_bc)/9 on both lattices), so one regularized step equals one LBGK step."""
+    e, w, _ = orc.lattice_tables(lat)
+    Q, D = len(e), (2 if lat == 0 else 3)
+    rng = np.random.default_rng(9)
+    S = rng.uniform(-1e-3, 1e-3, (3, 3))
+    S = S + S.T
+    if D == 2:
+        S[2, :] = S[:, 2] = 0
+    ef = e.astype(float)
+    H = np.einsum("qa,qb->qab", ef, ef) - np.eye(3)[None] / 3.0
+    v = np.array([0.03, -0.02, 0.01 if D == 3 else 0.0])
+    f = orc.feq(lat, 1.05, v[:D]) + 4.5 * w * np.einsum("qab,ab->q", H, S)
+    out = []
+    for model in (orc.BGK, orc.REG):
+        o = orc.Oracle(lat, model, 1, 1, 1, tau=0.7)
+        o.set_distributions(f.reshape(Q, 1, 1, 1))
+        o.step(1)
+        out.append(o.get_distributions().ravel())
+    assert np.max(np.abs(out[0] - out[1])) < 1e-16
+
+
+def test_regularized_keeps_the_viscosity_and_the_conservation_laws(orc):
+    """Taylor-Green decay at nu = (tau - 1/2)/3 within 1e-3, mass and momentum conserved."""
+    n, tau, u0, T = 32, 0.8, 0.01, 300
+    k = 2 * np.pi / n
+    y, x = np.meshgrid(np.arange(n, dtype=float), np.arange(n, dtype=float), indexing="ij")
+    u = np.stack([-u0 * np.cos(k * x) * np.sin(k * y), u0 * np.sin(k * x) * np.cos(k * y)])[:, None]
+    o = orc.Oracle(0, orc.REG, n, n, 1, tau=tau)
+    o.init_equilibrium(np.ones((1, n, n)), u)
+    f0 = o.get_distributions()
+    o.step(T)
+    f1 = o.get_distributions()
+    _, v = o.macro()
+    nu = (tau - 0.5) / 3.0
+    ratio = np.sqrt((v ** 2).sum() / (u ** 2).sum())
+    assert abs(-np.log(ratio) / (2 * k * k * T) / nu - 1.0) < 5e-3   # O(k^2) lattice error at n = 32
+    e = orc.lattice_tables(0)[0].astype(float)
+    assert abs(f1.sum() - f0.sum()) < 1e-11
+    assert np.max(np.abs(np.einsum("qzyx,qa->a", f1 - f0, e))) < 1e-12
+
+
+def test_regularized_with_guo_force_is_rejected_and_edm_force_is_exact(orc):
+    """Regularizing drops the first moment of f^neq, which under Guo's scheme carries -F/2: the
+    momentum balance would be off by (1 - 1/tau) F/2 per step (reading A23), so only the EDM is
+    accepted; with it v(n) = u0 + (n + 1/2) g as for every other operator."""
+    with pytest.raises(ValueError):
+        orc.Oracle(1, orc.REG, 4, 4, 4, tau=0.8, force=(1e-5, 0, 0))
+    g, u0 = (1e-5, -2e-5, 3e-5), (0.01, 0.02, -0.015)
+    for model in (orc.REG, orc.LES):
+        o = orc.Oracle(1, model, 4, 5, 6, tau=0.8, force=g, force_scheme=orc.FORCE_EDM, smagorinsky_cs=0.1)
+        o.init_equilibrium(*_uniform(o, 1.1, u0))
+        o.step(37)
+        r, v = o.macro()
+        for a in range(3):
+            assert np.max(np.abs(v[a] - (u0[a] + 37.5 * g[a]))) < 1e-15
+
+
+@pytest.mark.parametrize("scheme", [0, 1])
+def test_smagorinsky_with_zero_constant_is_lbgk_and_positive_constant_adds_viscosity(orc, scheme):
+    from paper_1311_2404_b200 import workloads as W
+    mask, rho, u = W.random_state(1, 6, 5, 4, seed=81, solid_fraction=0.15, du=0.05)
+    g = (1e-4, 0, -1e-4)
+    a = orc.Oracle(1, orc.BGK, 6, 5, 4, tau=0.56, force=g, force_scheme=scheme)
+    b = orc.Oracle(1, orc.LES, 6, 5, 4, tau=0.56, force=g, force_scheme=scheme, smagorinsky_cs=0.0)
+    for o in (a, b):
+        o.set_geometry(mask)
+        o.init_equilibrium(rho[0], u[0])
+        o.step(20)
+    assert np.array_equal(a.get_distributions(), b.get_distributions())
+    # C_S > 0: tau_t >= 0 everywhere, so a shear wave decays faster than with the molecular viscosity
+    n, tau, T = 32, 0.51, 200
+    k = 2 * np.pi / n
+    yy = np.arange(n, dtype=float)
+    uu = np.zeros((2, 1, n, 4))
+    uu[0] = (0.08 * np.sin(k * yy))[None, :, None]
+    amp = []
+    for cs in (0.0, 0.17):
+        o = orc.Oracle(0, orc.LES, 4, n, 1, tau=tau, smagorinsky_cs=cs)
+        o.init_equilibrium(np.ones((1, n, 4)), uu)
+        o.step(T)
+        amp.append(np.abs(o.macro()[1][0]).max())
+    nu = (tau - 0.5) / 3.0
+    assert abs(amp[0] / (0.08 * np.exp(-nu * k * k * T)) - 1.0) < 5e-3
+    assert amp[1] < 0.97 * amp[0]
