@@ -869,7 +869,7 @@ def test_regularized_keeps_the_viscosity_and_the_conservation_laws(orc):
     ratio = np.sqrt((v ** 2).sum() / (u ** 2).sum())
     assert abs(-np.log(ratio) / (2 * k * k * T) / nu - 1.0) < 5e-3   # O(k^2) lattice error at n = 32
     e = orc.lattice_tables(0)[0].astype(float)
-    assert abs(f1.sum() - f0.sum()) < 1e-11
+    assert abs(f1.sum() - f0.sum()) < 1e-13 * f0.sum()          # 300 steps of round-off on 1024 units of mass
     assert np.max(np.abs(np.einsum("qzyx,qa->a", f1 - f0, e))) < 1e-12
 
 
