@@ -33,8 +33,10 @@ extern "C" {
 
 enum { LBM_OK = 0, LBM_EINVAL = -1, LBM_EUNSUPPORTED = -2, LBM_ENOMEM = -3, LBM_ECUDA = -4, LBM_ESTATE = -5 };
 enum { LBM_D2Q9 = 0, LBM_D3Q19 = 1 };            /* lattice, Table 1              */
-enum { LBM_BGK = 0, LBM_MRT = 1, LBM_SC2 = 2 };  /* model: SC2 = two LBGK components coupled
+enum { LBM_BGK = 0, LBM_MRT = 1, LBM_SC2 = 2,    /* model: SC2 = two LBGK components coupled
                                                     by the Shan-Chen force       */
+       LBM_BGK_REG = 3,                          /* regularized LBGK (reading A23)    */
+       LBM_BGK_LES = 4 };                        /* LBGK + Smagorinsky subgrid model, eq. (8)-(9) */
 enum { LBM_F32 = 0, LBM_F64 = 1 };               /* precision of storage and arithmetic      */
 enum { LBM_PSI_RHO = 0, LBM_PSI_1MEXP = 1 };     /* psi(rho) = rho | 1 - exp(-rho)   */
 enum { LBM_STORE_AB = 0, LBM_STORE_AA = 1 };     /* two copies | in-place AA */
@@ -75,6 +77,7 @@ typedef struct {
     int32_t force_scheme;     /* LBM_FORCE_GUO (default 0, eq. 17) | LBM_FORCE_EDM (eq. 18); applies to
                                  the body force and to the Shan-Chen coupling force alike          */
     int32_t reserved_;        /* keeps sizeof a multiple of 8; set to 0                            */
+    double smagorinsky_cs;    /* LBM_BGK_LES: Smagorinsky constant C_S of eq. (9) (0.1), >= 0  */
 } lbm_params;
 
 /* Static description of a lattice (Table 1; ordering = reading A2).

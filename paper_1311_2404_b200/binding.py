@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "liblbm_b200.so")
 
 LBM_OK, LBM_EINVAL, LBM_EUNSUPPORTED, LBM_ENOMEM, LBM_ECUDA, LBM_ESTATE = 0, -1, -2, -3, -4, -5
 LBM_D2Q9, LBM_D3Q19 = 0, 1
-LBM_BGK, LBM_MRT, LBM_SC2 = 0, 1, 2
+LBM_BGK, LBM_MRT, LBM_SC2, LBM_BGK_REG, LBM_BGK_LES = 0, 1, 2, 3, 4
 LBM_F32, LBM_F64 = 0, 1
 LBM_PSI_RHO, LBM_PSI_1MEXP = 0, 1
 LBM_STORE_AB, LBM_STORE_AA = 0, 1
@@ -43,6 +43,7 @@ class lbm_params(C.Structure):
         ("bc_velocity", C.c_double * 3),
         ("force_scheme", C.c_int32),
         ("reserved_", C.c_int32),
+        ("smagorinsky_cs", C.c_double),
     ]
 
 
@@ -90,7 +91,7 @@ def load():
 
 def make_params(lattice, model, precision, nx, ny, nz=1, tau=(1.0, 1.0), rates=None,
                 force=(0.0, 0.0, 0.0), sc_G=0.0, sc_psi=LBM_PSI_RHO, store=LBM_STORE_AB,
-                bc_velocity=(0.0, 0.0, 0.0), force_scheme=0) -> lbm_params:
+                bc_velocity=(0.0, 0.0, 0.0), force_scheme=0, smagorinsky_cs=0.0) -> lbm_params:
     p = lbm_params()
     p.struct_size = C.sizeof(lbm_params)
     p.lattice, p.model, p.precision = int(lattice), int(model), int(precision)
@@ -104,6 +105,7 @@ def make_params(lattice, model, precision, nx, ny, nz=1, tau=(1.0, 1.0), rates=N
         p.force[a] = float(force[a]) if a < len(force) else 0.0
     p.sc_G, p.sc_psi, p.store = float(sc_G), int(sc_psi), int(store)
     p.force_scheme = int(force_scheme)
+    p.smagorinsky_cs = float(smagorinsky_cs)
     for a in range(3):
         p.bc_velocity[a] = float(bc_velocity[a]) if a < len(bc_velocity) else 0.0
     return p
@@ -261,4 +263,4 @@ class Lbm:
 def from_workload(w, device="cuda:0", **kw) -> "Lbm":
     """Context for a workloads.Workload (parameters only; arrays are passed separately)."""
     return Lbm(w.lattice, w.model, w.precision, w.nx, w.ny, w.nz, device=device, tau=w.tau, rates=w.rates,
-               force=w.force, sc_G=w.sc_G, sc_psi=w.sc_psi, bc_velocity=w.bc_velocity, force_scheme=w.force_scheme, **kw)
+               force=w.force, sc_G=w.sc_G, sc_psi=w.sc_psi, bc_velocity=w.bc_velocity, force_scheme=w.force_scheme, smagorinsky_cs=w.smagorinsky_cs, **kw)

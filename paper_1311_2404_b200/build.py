@@ -20,7 +20,7 @@ OBJDIR = os.path.join(_HERE, "build")
 SOURCES = [os.path.join(CSRC, "lbm_b200.cu")] + [
     os.path.join(CSRC, "lbm_impl_%s_%s.cu" % (lat, pr)) for lat in ("d2q9", "d3q19") for pr in ("f32", "f64")] + [
     os.path.join(CSRC, "lbm_step_%s_%s_%s.cu" % (lat, pr, m))
-    for lat in ("d3q19", "d2q9") for pr in ("f32", "f64") for m in ("bgk", "mrt", "sc")]
+    for lat in ("d3q19", "d2q9") for pr in ("f32", "f64") for m in ("bgk", "mrt", "sc", "reg", "les")]
 HEADERS = [os.path.join(CSRC, n) for n in ("lbm_impl.cuh", "lbm_steps.cuh", "lbm_kernels.cuh", "lbm_node.cuh", "lbm_lattice.cuh")] + [
     os.path.join(os.path.dirname(_HERE), "include", "lbm.h")]
 

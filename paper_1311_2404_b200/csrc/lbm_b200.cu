@@ -9,13 +9,16 @@ namespace {
 constexpr uint32_t LBM_PARAMS_SIZE_V1 = 240;
 // ... and before force_scheme was appended; such callers get the Guo scheme
 constexpr uint32_t LBM_PARAMS_SIZE_V2 = 264;
+// ... and before smagorinsky_cs was appended
+constexpr uint32_t LBM_PARAMS_SIZE_V3 = 272;
 
 int validate(const lbm_params *p, int *Q, int *D) {
     if (!p) return fail(nullptr, LBM_EINVAL, "params is NULL");
-    if (p->struct_size != sizeof(lbm_params) && p->struct_size != LBM_PARAMS_SIZE_V1 && p->struct_size != LBM_PARAMS_SIZE_V2)
+    if (p->struct_size != sizeof(lbm_params) && p->struct_size != LBM_PARAMS_SIZE_V1 && p->struct_size != LBM_PARAMS_SIZE_V2 &&
+        p->struct_size != LBM_PARAMS_SIZE_V3)
         return fail(nullptr, LBM_EINVAL, "struct_size is not a known sizeof(lbm_params)");
     if (p->lattice != LBM_D2Q9 && p->lattice != LBM_D3Q19) return fail(nullptr, LBM_EINVAL, "unknown lattice");
-    if (p->model < LBM_BGK || p->model > LBM_SC2) return fail(nullptr, LBM_EINVAL, "unknown model");
+    if (p->model < LBM_BGK || p->model > LBM_BGK_LES) return fail(nullptr, LBM_EINVAL, "unknown model");
     if (p->precision != LBM_F32 && p->precision != LBM_F64) return fail(nullptr, LBM_EINVAL, "unknown precision");
     if (p->store != LBM_STORE_AB && p->store != LBM_STORE_AA) return fail(nullptr, LBM_EINVAL, "unknown store");
     if (p->nx < 1 || p->ny < 1 || p->nz < 1) return fail(nullptr, LBM_EINVAL, "extents must be >= 1");
@@ -31,7 +34,12 @@ int validate(const lbm_params *p, int *Q, int *D) {
             if (!(p->rates[k] >= 0.0 && p->rates[k] <= 2.0)) return fail(nullptr, LBM_EINVAL, "MRT rates must be in [0, 2]");
     for (int a = 0; a < 3; a++)
         if (!(p->force[a] == p->force[a])) return fail(nullptr, LBM_EINVAL, "force is NaN");
-    if (p->struct_size == sizeof(lbm_params) && p->force_scheme != LBM_FORCE_GUO && p->force_scheme != LBM_FORCE_EDM)
+    if (p->model == LBM_BGK_LES && (p->struct_size != sizeof(lbm_params) || !(p->smagorinsky_cs >= 0.0 && p->smagorinsky_cs < 10.0)))
+        return fail(nullptr, LBM_EINVAL, "LBM_BGK_LES needs smagorinsky_cs in [0, 10)");
+    if (p->model == LBM_BGK_REG && (p->struct_size < LBM_PARAMS_SIZE_V3 || p->force_scheme != LBM_FORCE_EDM) &&
+        (p->force[0] != 0.0 || p->force[1] != 0.0 || p->force[2] != 0.0))
+        return fail(nullptr, LBM_EUNSUPPORTED, "regularized LBGK takes a body force through LBM_FORCE_EDM only (reading A23)");
+    if (p->struct_size >= LBM_PARAMS_SIZE_V3 && p->force_scheme != LBM_FORCE_GUO && p->force_scheme != LBM_FORCE_EDM)
         return fail(nullptr, LBM_EINVAL, "unknown force_scheme");
     if (p->struct_size >= LBM_PARAMS_SIZE_V2)
         for (int a = 0; a < 3; a++)

@@ -111,6 +111,8 @@ template <typename T> Relax<T> make_relax(const lbm_ctx *c, int comp) {
 template <class L, typename T> int lbm_step_bgk(lbm_ctx *c, int n);
 template <class L, typename T> int lbm_step_mrt(lbm_ctx *c, int n);
 template <class L, typename T> int lbm_step_sc(lbm_ctx *c, int n);
+template <class L, typename T> int lbm_step_reg(lbm_ctx *c, int n);
+template <class L, typename T> int lbm_step_les(lbm_ctx *c, int n);
 
 namespace {
 
@@ -190,6 +192,8 @@ template <class L, typename T> struct Impl {
     // they compile in parallel; here only the dispatch.
     static int step(lbm_ctx *c, int n) {
         if (c->p.model == LBM_SC2) return lbm_step_sc<L, T>(c, n);
+        if (c->p.model == LBM_BGK_REG) return lbm_step_reg<L, T>(c, n);
+        if (c->p.model == LBM_BGK_LES) return lbm_step_les<L, T>(c, n);
         return c->p.model == LBM_MRT ? lbm_step_mrt<L, T>(c, n) : lbm_step_bgk<L, T>(c, n);
     }
 

@@ -288,28 +288,28 @@ __device__ __forceinline__ void store_span(T *__restrict__ dst, int64_t N, int n
 }
 
 // Collision by node type (t = the node's type byte).
-template <class L, typename T, bool MRT, int FORCE>
+template <class L, typename T, int MODEL, int FORCE>
 __device__ __forceinline__ void update_typed(T (&h)[L::Q], uint32_t t, const Relax<T> &rp) {
     if (t & NODE_FULLWAY) fullway_reverse<L, T>(h);
     else if (t & NODE_VELOCITY) velocity_node<L, T>(h, rp.ubc);
-    else update_node<L, T, MRT, FORCE>(h, rp);
+    else update_node<L, T, MODEL, FORCE>(h, rp);
 }
 
 // All nodes of a pack; packs without FULLWAY / VELOCITY nodes take the branch-free path.
-template <class L, typename T, int V, bool MRT, int FORCE>
+template <class L, typename T, int V, int MODEL, int FORCE>
 __device__ __forceinline__ void update_span(T (&h)[V][L::Q], uint32_t types, const Relax<T> &rp) {
     if ((types & PACK_SPECIAL) == 0) {
 #pragma unroll
-        for (int k = 0; k < V; k++) update_node<L, T, MRT, FORCE>(h[k], rp);
+        for (int k = 0; k < V; k++) update_node<L, T, MODEL, FORCE>(h[k], rp);
     } else {
 #pragma unroll
-        for (int k = 0; k < V; k++) update_typed<L, T, MRT, FORCE>(h[k], (types >> (8 * k)) & 0xffu, rp);
+        for (int k = 0; k < V; k++) update_typed<L, T, MODEL, FORCE>(h[k], (types >> (8 * k)) & 0xffu, rp);
     }
 }
 
 // ---- the fused step: pull-stream + moments + equilibrium + collision (+ Guo) + store ---------
 // Rows a1-a8 of DESIGN.md.  All loads of the pack are issued before first use (bytes in flight).
-template <class L, typename T, int V, typename I, bool MRT, int FORCE>
+template <class L, typename T, int V, typename I, int MODEL, int FORCE>
 __global__ void __launch_bounds__(256)
 step_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restrict__ link,
             const T *__restrict__ src, T *__restrict__ dst, Relax<T> rp) {
@@ -320,7 +320,7 @@ step_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restrict
     T h[V][L::Q];
     gather_span<L, T, V, I>(src, g.N, s, h);
     pull_reflected_span<L, T, V, I>(src, g.N, s.row + s.x0, types, link, h);
-    update_span<L, T, V, MRT, FORCE>(h, types, rp);
+    update_span<L, T, V, MODEL, FORCE>(h, types, rp);
     store_span<L, T, V, I>(dst, g.N, s.row + s.x0, h);
 }
 
@@ -420,7 +420,7 @@ __device__ __forceinline__ I aa_slot(int parity, int i, int n, int64_t N, const 
     return reflected(link, i) ? I(i) * I(N) + I(n) : I(L::opp(i)) * I(N) + I(n + shift<L>(i, -1, o));
 }
 
-template <class L, typename T, int V, typename I, bool MRT, int FORCE>
+template <class L, typename T, int V, typename I, int MODEL, int FORCE>
 __global__ void __launch_bounds__(256)
 aa_even_kernel(Geom g, const uint8_t *__restrict__ type, T *f, Relax<T> rp) {
     Span s;
@@ -436,7 +436,7 @@ aa_even_kernel(Geom g, const uint8_t *__restrict__ type, T *f, Relax<T> rp) {
 #pragma unroll
         for (int k = 0; k < V; k++) h[k][i] = a[k];
     }
-    update_span<L, T, V, MRT, FORCE>(h, types, rp);
+    update_span<L, T, V, MODEL, FORCE>(h, types, rp);
 #pragma unroll
     for (int i = 0; i < L::Q; i++) {
         T a[V];
@@ -446,7 +446,7 @@ aa_even_kernel(Geom g, const uint8_t *__restrict__ type, T *f, Relax<T> rp) {
     }
 }
 
-template <class L, typename T, typename I, bool MRT, int FORCE>
+template <class L, typename T, typename I, int MODEL, int FORCE>
 __global__ void __launch_bounds__(256)
 aa_odd_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restrict__ link, T *f, Relax<T> rp) {
     Span s;
@@ -463,7 +463,7 @@ aa_odd_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restri
         slot[i] = aa_slot<L, I>(1, i, n, g.N, o, w);
         h[i] = f[slot[i]];
     }
-    update_typed<L, T, MRT, FORCE>(h, t, rp);
+    update_typed<L, T, MODEL, FORCE>(h, t, rp);
 #pragma unroll
     for (int i = 0; i < L::Q; i++) f[slot[L::opp(i)]] = h[i];
 }
@@ -657,8 +657,8 @@ sc_step_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restr
             mA[a] = rA * vA[a];
             mB[a] = rB * vB[a];
         }
-        collide<L, T, false, FS>(hA[k], rA, dA, vA, mA, FA, rpA);
-        collide<L, T, false, FS>(hB[k], rB, dB, vB, mB, FB, rpB);
+        collide<L, T, MODEL_BGK, FS>(hA[k], rA, dA, vA, mA, FA, rpA);
+        collide<L, T, MODEL_BGK, FS>(hB[k], rB, dB, vB, mB, FB, rpB);
     }
     store_span<L, T, V, I>(dstA, g.N, n0, hA);
     store_span<L, T, V, I>(dstB, g.N, n0, hB);

@@ -7,6 +7,7 @@
 // collision is affine in f, so it carries over unchanged: sum_i h_i = rho - 1, sum_i h_i e_i = j,
 // h_i^eq = w_i (drho + rho (3 e.v + 4.5 (e.v)^2 - 1.5 v.v)).
 #pragma once
+#include <cmath>
 #include "lbm_lattice.cuh"
 
 namespace lbm {
@@ -19,6 +20,7 @@ template <typename T> struct Relax {
     // omega / 36 and (1 - omega / 2) / 36 as unevaluated sums hi + lo of two T (see collide()):
     T om36_hi, om36_lo, sc36_hi, sc36_lo;
     T i36_hi, i36_lo; // 1 / 36 likewise (Exact Difference Method)
+    T tau0, cs2x36;   // Smagorinsky: molecular tau_0 and 4 c_s^-4 C_S^2 = 36 C_S^2 of eq. (9)
     T in[19];         // MRT: 1 / |M_k|^2 (Exact Difference Method increment)
     T g[3];           // body acceleration
     T ubc[3];         // velocity imposed on equilibrium-velocity nodes (reading A21)
@@ -40,6 +42,7 @@ template <typename T> inline void set_bgk(Relax<T> &r, double tau) {
     r.om36_hi = T(c); r.om36_lo = T(c - double(r.om36_hi));
     r.sc36_hi = T(s); r.sc36_lo = T(s - double(r.sc36_hi));
     r.i36_hi = T(1.0 / 36.0); r.i36_lo = T(1.0 / 36.0 - double(r.i36_hi));
+    r.tau0 = T(tau); r.cs2x36 = T(0);
 }
 
 template <class L, typename T> LBM_HD void moments(const T (&h)[L::Q], T &drho, T (&j)[3]) {
@@ -59,6 +62,33 @@ template <class L, typename T> LBM_HD T e_dot(int i, const T (&a)[3]) {
     if (L::ex(i) == 1) s += a[0]; else if (L::ex(i) == -1) s -= a[0];
     if (L::ey(i) == 1) s += a[1]; else if (L::ey(i) == -1) s -= a[1];
     if (L::ez(i) == 1) s += a[2]; else if (L::ez(i) == -1) s -= a[2];
+    return s;
+}
+
+// Second moments P_ab = sum_i e_ia e_ib h_i in the order xx, yy, zz, xy, yz, xz, and e_i.P.e_i.
+template <class L, typename T> LBM_HD void second_moments(const T (&h)[L::Q], T (&P)[6]) {
+#pragma unroll
+    for (int c = 0; c < 6; c++) P[c] = T(0);
+#pragma unroll
+    for (int i = 1; i < L::Q; i++) {
+        const int x = L::ex(i), y = L::ey(i), z = L::ez(i);
+        if (x) P[0] += h[i];
+        if (y) P[1] += h[i];
+        if (z) P[2] += h[i];
+        if (x * y == 1) P[3] += h[i]; else if (x * y == -1) P[3] -= h[i];
+        if (y * z == 1) P[4] += h[i]; else if (y * z == -1) P[4] -= h[i];
+        if (x * z == 1) P[5] += h[i]; else if (x * z == -1) P[5] -= h[i];
+    }
+}
+template <class L, typename T> LBM_HD T e_quad(int i, const T (&P)[6]) {
+    const int x = L::ex(i), y = L::ey(i), z = L::ez(i);
+    T s = T(0);
+    if (x) s += P[0];
+    if (y) s += P[1];
+    if (z) s += P[2];
+    if (x * y == 1) s += T(2) * P[3]; else if (x * y == -1) s -= T(2) * P[3];
+    if (y * z == 1) s += T(2) * P[4]; else if (y * z == -1) s -= T(2) * P[4];
+    if (x * z == 1) s += T(2) * P[5]; else if (x * z == -1) s -= T(2) * P[5];
     return s;
 }
 
@@ -217,15 +247,17 @@ template <typename T> struct Mrt<D2Q9, T> {
 
 // FORCE: 0 no body force, 1 Guo (eq. 17), 2 Exact Difference Method (eq. 18).
 constexpr int FORCE_NONE = 0, FORCE_GUO = 1, FORCE_EDM = 2;
+// MODEL: LBGK (Alg. 1 l.13) | MRT (eq. 4) | regularized LBGK | LBGK + Smagorinsky (eq. 8-9).
+constexpr int MODEL_BGK = 0, MODEL_MRT = 1, MODEL_REG = 2, MODEL_LES = 3;
 
 // ---- collision: h (pre-collision deviations) -> h* (post-collision), in place ---------------
 // rho, drho = rho - 1, v = velocity entering f^eq and eq. (17) (reading A3), rv = rho v as formed
 // from the moments (j + F/2, eq. 16), F = force density.  With FORCE_EDM v is the bare velocity u
 // (reading A22), rv = rho u, and the routine adds f^eq(rho, u + F/rho) - f^eq(rho, u).
-template <class L, typename T, bool MRT, int FORCE>
+template <class L, typename T, int MODEL, int FORCE>
 LBM_HD void collide(T (&h)[L::Q], T rho, T drho, const T (&v)[3], const T (&rv)[3], const T (&F)[3], const Relax<T> &rp) {
     constexpr int Q = L::Q;
-    if constexpr (!MRT) {
+    if constexpr (MODEL != MODEL_MRT) {
         // LBGK (Alg. 1 l.13) + eq. (17), evaluated per +/- pair of directions: with e_ibar = -e_i
         // the equilibrium and the source split into a part even in e_i (shared by the pair) and a
         // part odd in e_i (opposite signs), which halves the arithmetic per node.
@@ -237,7 +269,63 @@ LBM_HD void collide(T (&h)[L::Q], T rho, T drho, const T (&v)[3], const T (&rv)[
         // of two on all moving directions), omega / 36 multiplies the three per-node scalars as a
         // two-term sum hi + lo (rounding then depends on the node's data, not on a constant), and
         // the old value is scaled by keep = 1 - omega, which set_bgk makes exact for the omega in use.
-        const T keep = rp.keep;
+        // relaxation constants: host-prepared (set_bgk) or, for the Smagorinsky model, per node
+        T keep = rp.keep, om = rp.inv_tau, om36_hi = rp.om36_hi, om36_lo = rp.om36_lo;
+        T sc36_hi = rp.sc36_hi, sc36_lo = rp.sc36_lo;
+        if constexpr (MODEL == MODEL_REG || MODEL == MODEL_LES) {
+            // non-equilibrium second moment sum_i e_ia e_ib (h_i - h_i^eq) = P_ab - (rho - 1) delta_ab / 3
+            // - rho v_a v_b; it is Pi^neq of P:130 and Q of eq. (9) at once because sum_i f_i^neq = 0
+            T Pi[6];
+            second_moments<L, T>(h, Pi);
+            const T third = drho * T(1.0 / 3.0);
+            Pi[0] -= third + rho * v[0] * v[0];
+            Pi[1] -= third + rho * v[1] * v[1];
+            Pi[2] -= L::D == 3 ? third + rho * v[2] * v[2] : T(0);
+            Pi[3] -= rho * v[0] * v[1];
+            Pi[4] -= rho * v[1] * v[2];
+            Pi[5] -= rho * v[0] * v[2];
+            if constexpr (MODEL == MODEL_LES) {
+                // eq. (9): tau = tau_0 + ( sqrt(tau_0^2 + 36 C_S^2 |Q|) - tau_0 ) / 2, |Q| = (Q_ab Q_ab)^(1/2)
+                const T q2 = Pi[0] * Pi[0] + Pi[1] * Pi[1] + Pi[2] * Pi[2] +
+                             T(2) * (Pi[3] * Pi[3] + Pi[4] * Pi[4] + Pi[5] * Pi[5]);
+                const T tau = T(0.5) * (rp.tau0 + sqrt(rp.tau0 * rp.tau0 + rp.cs2x36 * sqrt(q2)));
+                om = T(1) / tau;
+                keep = T(1) - om;
+                om36_hi = om * T(1.0 / 36.0); om36_lo = T(0);
+                sc36_hi = (T(1) - T(0.5) * om) * T(1.0 / 36.0); sc36_lo = T(0);
+            } else {
+                // regularized: h* = keep f^reg + h^eq(u2), f^reg_i = 4.5 w_i (e_i.Pi.e_i - tr Pi / 3),
+                // u2 = u + F / rho (the EDM increment; u2 = u without a force).  Reading A23.
+                const T inv_rho = T(1) / rho;
+                T u2[3], mo[3];
+#pragma unroll
+                for (int a = 0; a < 3; a++) {
+                    u2[a] = FORCE ? v[a] + F[a] * inv_rho : v[a];
+                    const T t = T(3) * (FORCE ? rv[a] + F[a] : rv[a]);
+                    mo[a] = t * rp.i36_hi + t * rp.i36_lo;
+                }
+                const T vv2 = u2[0] * u2[0] + u2[1] * u2[1] + u2[2] * u2[2];
+                const T b0 = drho - rho * (T(1.5) * vv2), q0 = T(4.5) * rho;
+                const T k8 = keep * T(0.125);  // keep * 4.5 / 36
+                const T tr3 = (Pi[0] + Pi[1] + Pi[2]) * T(1.0 / 3.0);
+                const T base = (b0 * rp.i36_hi + b0 * rp.i36_lo) - k8 * tr3;
+                const T r45 = q0 * rp.i36_hi + q0 * rp.i36_lo;
+                h[0] = T(L::w36(0)) * base;
+#pragma unroll
+                for (int i = 1; i < Q; i++) {
+                    if (i < L::opp(i)) {
+                        const int j = L::opp(i);
+                        const T wi = T(L::w36(i));
+                        const T ev2 = e_dot<L, T>(i, u2);
+                        const T odd = e_dot<L, T>(i, mo);
+                        const T even = base + r45 * ev2 * ev2 + k8 * e_quad<L, T>(i, Pi);
+                        h[i] = wi * (even + odd);
+                        h[j] = wi * (even - odd);
+                    }
+                }
+                return;
+            }
+        }
         if constexpr (FORCE == FORCE_EDM) {
             // h* = keep h + h^eq(u2) - keep h^eq(u), u2 = u + F/rho, in the same even/odd form:
             //   odd  = 3 e.(rho u2 - keep rho u) = 3 e.(omega rho u + F)   (momentum gains exactly F)
@@ -248,11 +336,11 @@ LBM_HD void collide(T (&h)[L::Q], T rho, T drho, const T (&v)[3], const T (&rv)[
             for (int a = 0; a < 3; a++) {
                 u2[a] = v[a] + F[a] * inv_rho;
                 const T t = T(3) * rv[a], f3 = T(3) * F[a];
-                mo[a] = (t * rp.om36_hi + t * rp.om36_lo) + (f3 * rp.i36_hi + f3 * rp.i36_lo);
+                mo[a] = (t * om36_hi + t * om36_lo) + (f3 * rp.i36_hi + f3 * rp.i36_lo);
             }
             const T vv = v[0] * v[0] + v[1] * v[1] + v[2] * v[2];
             const T vv2 = u2[0] * u2[0] + u2[1] * u2[1] + u2[2] * u2[2];
-            const T b0 = rp.inv_tau * drho - rho * (T(1.5) * (vv2 - keep * vv)), q0 = T(4.5) * rho;
+            const T b0 = om * drho - rho * (T(1.5) * (vv2 - keep * vv)), q0 = T(4.5) * rho;
             const T base = b0 * rp.i36_hi + b0 * rp.i36_lo;
             const T r45 = q0 * rp.i36_hi + q0 * rp.i36_lo;
             h[0] = keep * h[0] + T(L::w36(0)) * base;
@@ -272,8 +360,8 @@ LBM_HD void collide(T (&h)[L::Q], T rho, T drho, const T (&v)[3], const T (&rv)[
         }
         const T vv = v[0] * v[0] + v[1] * v[1] + v[2] * v[2];
         const T b0 = drho - rho * (T(1.5) * vv), q0 = T(4.5) * rho;
-        const T base = b0 * rp.om36_hi + b0 * rp.om36_lo;
-        const T r45 = q0 * rp.om36_hi + q0 * rp.om36_lo;
+        const T base = b0 * om36_hi + b0 * om36_lo;
+        const T r45 = q0 * om36_hi + q0 * om36_lo;
         // odd part: omega w_i 3 rho (e_i . v) = 36 w_i e_i . m3 with m3 = (omega / 12) * (rho v),
         // and rho v = j + F/2 is taken from the moments directly (no round trip through 1/rho),
         // so that sum_i e_i f_i^eq reproduces it up to unbiased rounding.
@@ -283,13 +371,13 @@ LBM_HD void collide(T (&h)[L::Q], T rho, T drho, const T (&v)[3], const T (&rv)[
 #pragma unroll
         for (int a = 0; a < 3; a++) {
             const T t = T(3) * rv[a];
-            mo[a] = t * rp.om36_hi + t * rp.om36_lo;
+            mo[a] = t * om36_hi + t * om36_lo;
         }
         if constexpr (FORCE) {
             T vF = T(0);
 #pragma unroll
             for (int a = 0; a < 3; a++) {
-                const T Fs = F[a] * rp.sc36_hi + F[a] * rp.sc36_lo;
+                const T Fs = F[a] * sc36_hi + F[a] * sc36_lo;
                 mo[a] += T(3) * Fs;
                 F9[a] = T(9) * Fs;
                 vF += v[a] * Fs;
@@ -343,10 +431,10 @@ LBM_HD void collide(T (&h)[L::Q], T rho, T drho, const T (&v)[3], const T (&rv)[
 }
 
 // Single-component node update: moments, F = rho g, v = j/rho + g/2 (eq. 16), collide.
-template <class L, typename T, bool MRT, int FORCE>
+template <class L, typename T, int MODEL, int FORCE>
 LBM_HD void update_node(T (&h)[L::Q], const Relax<T> &rp) {
     constexpr int Q = L::Q;
-    if constexpr (MRT && Mrt<L, T>::closed_form_meq) {
+    if constexpr (MODEL == MODEL_MRT && Mrt<L, T>::closed_form_meq) {
         // eq. (4) in moment space: m = M h once (it also yields rho - 1 and j), relax towards the
         // closed-form equilibrium moments, transform back the increment only.
         T m[Q];
@@ -393,7 +481,7 @@ LBM_HD void update_node(T (&h)[L::Q], const Relax<T> &rp) {
             rv[a] = FORCE == FORCE_GUO ? j[a] + T(0.5) * F[a] : j[a];
             v[a] = rv[a] * inv_rho;
         }
-        collide<L, T, MRT, FORCE>(h, rho, drho, v, rv, F, rp);
+        collide<L, T, MODEL, FORCE>(h, rho, drho, v, rv, F, rp);
     }
 }
 

@@ -11,18 +11,18 @@ template <class L, typename T> struct Steps {
     static uint8_t *type(lbm_ctx *c) { return at<uint8_t>(c, c->lay.type); }
     static uint32_t *link(lbm_ctx *c) { return at<uint32_t>(c, c->lay.link); }
 
-    template <int V, bool MRT, int FORCE> static int step_single_v(lbm_ctx *c, int n, const Relax<T> &rp) {
-        return c->idx32 ? step_single_vi<V, uint32_t, MRT, FORCE>(c, n, rp) : step_single_vi<V, int64_t, MRT, FORCE>(c, n, rp);
+    template <int V, int MODEL, int FORCE> static int step_single_v(lbm_ctx *c, int n, const Relax<T> &rp) {
+        return c->idx32 ? step_single_vi<V, uint32_t, MODEL, FORCE>(c, n, rp) : step_single_vi<V, int64_t, MODEL, FORCE>(c, n, rp);
     }
 
-    template <int V, typename I, bool MRT, int FORCE> static int step_single_vi(lbm_ctx *c, int n, const Relax<T> &rp) {
+    template <int V, typename I, int MODEL, int FORCE> static int step_single_vi(lbm_ctx *c, int n, const Relax<T> &rp) {
         const Launch l = span_launch(c, V);
         if (c->aa) {  // in place: even steps are local (V-node packs), odd steps move data (one node per thread)
             const Launch l1 = span_launch(c, 1);
             T *f = at<T>(c, c->lay.store[0][0]);
             for (int t = 0; t < n; t++) {
-                if (c->cur == 0) aa_even_kernel<L, T, V, I, MRT, FORCE><<<l.grid, l.block, 0, c->stream>>>(c->g, type(c), f, rp);
-                else aa_odd_kernel<L, T, I, MRT, FORCE><<<l1.grid, l1.block, 0, c->stream>>>(c->g, type(c), link(c), f, rp);
+                if (c->cur == 0) aa_even_kernel<L, T, V, I, MODEL, FORCE><<<l.grid, l.block, 0, c->stream>>>(c->g, type(c), f, rp);
+                else aa_odd_kernel<L, T, I, MODEL, FORCE><<<l1.grid, l1.block, 0, c->stream>>>(c->g, type(c), link(c), f, rp);
                 if (int rc = check_launch(c, "aa_step_kernel")) return rc;
                 c->cur ^= 1;
                 c->steps++;
@@ -30,7 +30,7 @@ template <class L, typename T> struct Steps {
             return LBM_OK;
         }
         for (int t = 0; t < n; t++) {
-            step_kernel<L, T, V, I, MRT, FORCE><<<l.grid, l.block, 0, c->stream>>>(c->g, type(c), link(c), src(c, 0), dst(c, 0), rp);
+            step_kernel<L, T, V, I, MODEL, FORCE><<<l.grid, l.block, 0, c->stream>>>(c->g, type(c), link(c), src(c, 0), dst(c, 0), rp);
             if (int rc = check_launch(c, "step_kernel")) return rc;
             c->cur ^= 1;
             c->steps++;
@@ -38,12 +38,12 @@ template <class L, typename T> struct Steps {
         return LBM_OK;
     }
 
-    template <bool MRT, int FORCE> static int step_single(lbm_ctx *c, int n, const Relax<T> &rp) {
+    template <int MODEL, int FORCE> static int step_single(lbm_ctx *c, int n, const Relax<T> &rp) {
         if constexpr (sizeof(T) == 4) {
-            if (c->vec == 4) return step_single_v<4, MRT, FORCE>(c, n, rp);
+            if (c->vec == 4) return step_single_v<4, MODEL, FORCE>(c, n, rp);
         }
-        if (c->vec == 2) return step_single_v<2, MRT, FORCE>(c, n, rp);
-        return step_single_v<1, MRT, FORCE>(c, n, rp);
+        if (c->vec == 2) return step_single_v<2, MODEL, FORCE>(c, n, rp);
+        return step_single_v<1, MODEL, FORCE>(c, n, rp);
     }
 
     template <int V, int PSI> static int step_sc_v(lbm_ctx *c, int n) {
@@ -75,18 +75,21 @@ template <class L, typename T> struct Steps {
         return step_sc_v<1, PSI>(c, n);
     }
 
-    template <bool MRT> static int step_model(lbm_ctx *c, int n) {
+    template <int MODEL> static int step_model(lbm_ctx *c, int n) {
         Relax<T> rp = make_relax<T>(c, 0);
         const bool force = c->p.force[0] != 0.0 || c->p.force[1] != 0.0 || c->p.force[2] != 0.0;
         const bool edm = c->p.force_scheme == LBM_FORCE_EDM;
-        if (MRT)
+        if (MODEL == MODEL_MRT)
             for (int k = 0; k < L::Q; k++) {  // M^-1 = M^T diag(1/|M_k|^2): rows are orthogonal (A5)
                 rp.cr[k] = T(c->p.rates[k] / Mrt<L, T>::norm(k));
                 rp.cs[k] = T((1.0 - 0.5 * c->p.rates[k]) / Mrt<L, T>::norm(k));
                 rp.in[k] = T(1.0 / Mrt<L, T>::norm(k));
             }
-        if (!force) return step_single<MRT, FORCE_NONE>(c, n, rp);
-        return edm ? step_single<MRT, FORCE_EDM>(c, n, rp) : step_single<MRT, FORCE_GUO>(c, n, rp);
+        if (!force) return step_single<MODEL, FORCE_NONE>(c, n, rp);
+        if (MODEL == MODEL_LES) rp.cs2x36 = T(36.0 * c->p.smagorinsky_cs * c->p.smagorinsky_cs);
+        if (edm) return step_single<MODEL, FORCE_EDM>(c, n, rp);
+        if constexpr (MODEL == MODEL_REG) return fail(c, LBM_EUNSUPPORTED, "regularized LBGK takes a body force through the EDM only");
+        else return step_single<MODEL, FORCE_GUO>(c, n, rp);
     }
 
     static int step_shan_chen(lbm_ctx *c, int n) {
@@ -97,11 +100,15 @@ template <class L, typename T> struct Steps {
 }  // namespace
 
 // Which model a translation unit instantiates is chosen by the macro it defines before including
-// this header: LBM_STEP_BGK, LBM_STEP_MRT or LBM_STEP_SC.
+// this header: LBM_STEP_BGK, LBM_STEP_MRT, LBM_STEP_REG, LBM_STEP_LES or LBM_STEP_SC.
 #if defined(LBM_STEP_BGK)
-template <class L, typename T> int lbm_step_bgk(lbm_ctx *c, int n) { return Steps<L, T>::template step_model<false>(c, n); }
+template <class L, typename T> int lbm_step_bgk(lbm_ctx *c, int n) { return Steps<L, T>::template step_model<MODEL_BGK>(c, n); }
 #elif defined(LBM_STEP_MRT)
-template <class L, typename T> int lbm_step_mrt(lbm_ctx *c, int n) { return Steps<L, T>::template step_model<true>(c, n); }
+template <class L, typename T> int lbm_step_mrt(lbm_ctx *c, int n) { return Steps<L, T>::template step_model<MODEL_MRT>(c, n); }
+#elif defined(LBM_STEP_REG)
+template <class L, typename T> int lbm_step_reg(lbm_ctx *c, int n) { return Steps<L, T>::template step_model<MODEL_REG>(c, n); }
+#elif defined(LBM_STEP_LES)
+template <class L, typename T> int lbm_step_les(lbm_ctx *c, int n) { return Steps<L, T>::template step_model<MODEL_LES>(c, n); }
 #elif defined(LBM_STEP_SC)
 template <class L, typename T> int lbm_step_sc(lbm_ctx *c, int n) { return Steps<L, T>::step_shan_chen(c, n); }
 #endif

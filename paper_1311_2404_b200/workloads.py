@@ -21,7 +21,7 @@ from dataclasses import dataclass, field
 import numpy as np
 
 D2Q9, D3Q19 = 0, 1
-BGK, MRT, SC2 = 0, 1, 2
+BGK, MRT, SC2, REG, LES = 0, 1, 2, 3, 4   # LBGK | MRT | Shan-Chen 2 x LBGK | regularized LBGK | LBGK + Smagorinsky
 F32, F64 = 0, 1
 FLUID, SOLID, WALL_FULLWAY, VELOCITY = 0, 1, 2, 3   # node types of the geometry mask
 FORCE_GUO, FORCE_EDM = 0, 1
@@ -55,6 +55,7 @@ class Workload:
     sc_psi: int = 0
     bc_velocity: tuple = (0.0, 0.0, 0.0)
     force_scheme: int = 0                          # 0 Guo (eq. 17), 1 Exact Difference Method (eq. 18)
+    smagorinsky_cs: float = 0.0                    # C_S of eq. (9), model LES only
     seed: int | None = None
     mask: np.ndarray | None = None                 # uint8 [nz][ny][nx], 0 FLUID 1 SOLID
     rho: list = field(default_factory=list)        # per component, fp64 [nz][ny][nx]
@@ -79,7 +80,8 @@ class Workload:
     def params(self) -> dict:
         return dict(lattice=self.lattice, model=self.model, nx=self.nx, ny=self.ny, nz=self.nz,
                     tau=self.tau, rates=self.rates, force=self.force, sc_G=self.sc_G, sc_psi=self.sc_psi,
-                    bc_velocity=self.bc_velocity, force_scheme=self.force_scheme)
+                    bc_velocity=self.bc_velocity, force_scheme=self.force_scheme,
+                    smagorinsky_cs=self.smagorinsky_cs)
 
 
 def c1_taylor_green(n: int = 128, steps: int = 1000, u0: float = 0.01, tau: float = 0.8,

@@ -6,8 +6,8 @@
 
 using namespace lbm;
 
-template <class L, typename T, bool MRT, int FORCE>
-static void run(const double *f, double tau, const double *rates, const double *g, double *out) {
+template <class L, typename T, int MODEL, int FORCE>
+static void run(const double *f, double tau, const double *rates, const double *g, double *out, double cs = 0.0) {
     Relax<T> rp{};
     set_bgk(rp, tau);
     for (int a = 0; a < 3; a++) rp.g[a] = T(g[a]);
@@ -18,21 +18,30 @@ static void run(const double *f, double tau, const double *rates, const double *
     }
     T h[L::Q];
     for (int i = 0; i < L::Q; i++) h[i] = T(f[i] - L::template w<double>(i));
-    update_node<L, T, MRT, FORCE>(h, rp);
+    rp.cs2x36 = T(36.0 * cs * cs);
+    update_node<L, T, MODEL, FORCE>(h, rp);
     for (int i = 0; i < L::Q; i++) out[i] = double(h[i]) + L::template w<double>(i);
 }
 
 template <class L, typename T>
 static void dispatch(int mrt, int force, const double *f, double tau, const double *rates, const double *g, double *out) {
     // force: 0 none, 1 Guo (eq. 17), 2 Exact Difference Method (eq. 18)
-    if (mrt) {
-        if (force == 2) run<L, T, true, 2>(f, tau, rates, g, out);
-        else if (force) run<L, T, true, 1>(f, tau, rates, g, out);
-        else run<L, T, true, 0>(f, tau, rates, g, out);
+    // mrt = model: 0 LBGK, 1 MRT, 2 regularized LBGK, 3 LBGK + Smagorinsky (C_S = 0.17 here)
+    if (mrt == 1) {
+        if (force == 2) run<L, T, 1, 2>(f, tau, rates, g, out);
+        else if (force) run<L, T, 1, 1>(f, tau, rates, g, out);
+        else run<L, T, 1, 0>(f, tau, rates, g, out);
+    } else if (mrt == 2) {
+        if (force == 2) run<L, T, 2, 2>(f, tau, rates, g, out);
+        else run<L, T, 2, 0>(f, tau, rates, g, out);
+    } else if (mrt == 3) {
+        if (force == 2) run<L, T, 3, 2>(f, tau, rates, g, out, 0.17);
+        else if (force) run<L, T, 3, 1>(f, tau, rates, g, out, 0.17);
+        else run<L, T, 3, 0>(f, tau, rates, g, out, 0.17);
     } else {
-        if (force == 2) run<L, T, false, 2>(f, tau, rates, g, out);
-        else if (force) run<L, T, false, 1>(f, tau, rates, g, out);
-        else run<L, T, false, 0>(f, tau, rates, g, out);
+        if (force == 2) run<L, T, 0, 2>(f, tau, rates, g, out);
+        else if (force) run<L, T, 0, 1>(f, tau, rates, g, out);
+        else run<L, T, 0, 0>(f, tau, rates, g, out);
     }
 }
 

@@ -34,12 +34,12 @@ def test_header_symbols_exported(lib):
 
 def test_params_struct_matches_header(lib):
     # uint32 + 6 int32 (28) -> pad to 32; 2 + 19 + 3 + 1 doubles (200); 2 int32 (8) => 240 (v1);
-    # + bc_velocity[3] => 264 (v2); + force_scheme + reserved => 272
-    assert C.sizeof(binding.lbm_params) == 272
+    # + bc_velocity[3] => 264 (v2); + force_scheme + reserved => 272 (v3); + smagorinsky_cs => 280
+    assert C.sizeof(binding.lbm_params) == 280
     p = binding.make_params(1, 0, 0, 8, 8, 8, tau=0.6)
     n = binding.lbm_workspace_bytes(p)
     assert n > 0
-    for older in (240, 264):  # callers built against an earlier layout: accepted, newer fields read as 0
+    for older in (240, 264, 272):  # callers built against an earlier layout: accepted, newer fields read as 0
         p.struct_size = older
         assert binding.lbm_workspace_bytes(p) == n
     p.struct_size = 16
@@ -73,6 +73,9 @@ def test_lattice_info_table1(lib):
     (dict(store=7), binding.LBM_EINVAL),
     (dict(bc_velocity=(1.5, 0.0, 0.0)), binding.LBM_EINVAL),
     (dict(force_scheme=5), binding.LBM_EINVAL),
+    (dict(model=5), binding.LBM_EINVAL),
+    (dict(model=4, smagorinsky_cs=-1.0), binding.LBM_EINVAL),
+    (dict(model=3, force=(1e-5, 0.0, 0.0)), binding.LBM_EUNSUPPORTED),
 ])
 def test_bad_params_rejected(lib, kw, code):
     args = dict(lattice=1, model=0, precision=0, nx=8, ny=8, nz=8, tau=0.8)

@@ -279,3 +279,38 @@ def test_edm_shan_chen(B, orc, precision, lattice, shape):
     w = generic(lattice, W.SC2, precision, shape, 62, solid=0.05, tau=(1.0, 0.625), sc_G=0.9,
                 force=(1e-5, 2e-5, 0.0), force_scheme=W.FORCE_EDM)
     check_parity_live(B, orc, w, steps=60)
+
+
+# ---- NEXT-4: regularized LBGK and the Smagorinsky subgrid model (eq. 8-9); reading A23 --------
+@pytest.mark.parametrize("store", ["ab", "aa"])
+@pytest.mark.parametrize("model", [W.REG, W.LES])
+@pytest.mark.parametrize("lattice,precision,shape,scheme", [
+    (W.D3Q19, W.F32, (48, 21, 10), W.FORCE_EDM), (W.D3Q19, W.F64, (37, 14, 9), W.FORCE_EDM),
+    (W.D3Q19, W.F32, (40, 12, 11), W.FORCE_GUO), (W.D2Q9, W.F64, (66, 31, 1), W.FORCE_EDM),
+    (W.D2Q9, W.F32, (52, 30, 1), W.FORCE_GUO)])
+def test_regularized_and_smagorinsky(B, orc, model, lattice, precision, shape, scheme, store):
+    D = 2 if lattice == W.D2Q9 else 3
+    force = (1e-4, -2e-4, 3e-4 if D == 3 else 0.0)
+    if model == W.REG and scheme == W.FORCE_GUO:
+        force = (0.0, 0.0, 0.0)  # regularized LBGK takes a force through the EDM only (A23)
+    w = generic(lattice, model, precision, shape, 71, tau=(0.58, 0.58), force=force, force_scheme=scheme,
+                smagorinsky_cs=0.17)
+    for u in w.u:  # larger velocities so that the eddy viscosity is not negligible
+        u *= 2.5
+    check_parity_live(B, orc, w, store=B.LBM_STORE_AA if store == "aa" else B.LBM_STORE_AB)
+
+
+def test_smagorinsky_zero_constant_matches_lbgk_bitwise(B):
+    """C_S = 0 makes tau_t = 0 (eq. 9): same relaxation time, so the results agree to round-off
+    of the per-node constants (the LBGK kernel uses host-prepared two-term constants)."""
+    import torch
+    w = generic(W.D3Q19, W.BGK, W.F64, (24, 10, 9), 72, tau=(0.6, 0.6), force=(1e-5, 0, 0))
+    out = []
+    for model in (W.BGK, W.LES):
+        w.model = model
+        sim = B.from_workload(w)
+        sim.set_geometry(w.mask)
+        sim.init_equilibrium(w.rho[0], w.u[0])
+        sim.step(50)
+        out.append(sim.get_distributions())
+    assert float((out[0] - out[1]).abs().max()) < 1e-14
