@@ -55,9 +55,17 @@ def measured_peak():
 
 
 def make_workload(args):
-    if args.precision is None:
-        return W.CONFIGS[args.config]()
-    return W.CONFIGS[args.config](precision=W.F32 if args.precision == "f32" else W.F64)
+    kw = {} if args.precision is None else {"precision": W.F32 if args.precision == "f32" else W.F64}
+    w = W.CONFIGS[args.config](**kw)
+    if getattr(args, "model", None) and w.model != W.SC2:
+        w.model = {"bgk": W.BGK, "mrt": W.MRT, "reg": W.REG, "les": W.LES}[args.model]
+        if w.model == W.MRT and w.rates is None:
+            w.rates = W.mrt_rates_d3q19(w.tau[0]) if w.lattice == W.D3Q19 else W.mrt_rates_d2q9(w.tau[0])
+        if w.model == W.LES:
+            w.smagorinsky_cs = 0.1
+        if w.model == W.REG and any(w.force):
+            w.force_scheme = W.FORCE_EDM  # reading A23
+    return w
 
 
 def sample_workload(cfg: str):
@@ -88,7 +96,7 @@ def time_oracle(cfg: str, steps: int, warmup: int):
 
 def config_dict(w, cfg, extra=None, store="ab"):
     d = {"workload": "%s: %s %s %s %dx%dx%d" % (cfg, "D2Q9" if w.lattice == W.D2Q9 else "D3Q19",
-                                                 ["LBGK", "MRT", "Shan-Chen 2xLBGK"][w.model],
+                                                 ["LBGK", "MRT", "Shan-Chen 2xLBGK", "regularized LBGK", "LBGK+Smagorinsky"][w.model],
                                                  "fp32" if w.precision == W.F32 else "fp64", w.nx, w.ny, w.nz),
          "tau": list(w.tau)[: w.ncomp], "force": list(w.force), "seed": w.seed,
          "solid_fraction": float(w.mask.mean()), "store": ("AA in place" if store == "aa" else "AB double buffer") + ", SoA real[Q][N]",
@@ -269,6 +277,8 @@ def main():
     ap.add_argument("--cpu-steps", type=int, default=250, help="oracle steps on the bounded sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--precision", default=None, choices=["f32", "f64"], help="override the config's precision (c3 is quoted in both)")
+    ap.add_argument("--model", default=None, choices=["bgk", "mrt", "reg", "les"],
+                    help="override the collision operator of a single-component config (NEXT-4 variants)")
     ap.add_argument("--store", default="ab", choices=["ab", "aa"], help="AB double buffer (default) or in-place AA")
     args = ap.parse_args()
     if args.impl == "reference":

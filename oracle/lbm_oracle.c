@@ -37,6 +37,9 @@
  *   full-way BB  wall node (dry): f* = f reversed, no relaxation; back in the fluid at t+2     P:237 Fig. 2 (1), A20
  *   velocity BC  f* = f^eq(rho, u_bc), rho from the node's own populations, missing ones
  *              are bounce-back copies (the half-way rule behind a SOLID node)              P:239, A21
+ *   EDM        F_i = f^eq(rho, u + F/rho) - f^eq(rho, u), any collision operator          P:253-258 eq. (18), A22
+ *   regularized f^neq -> w_i/(2 c_s^4)(e e - c_s^2 delta):Pi^neq, then LBGK               P:130, A23
+ *   Smagorinsky tau = tau_0 + (sqrt(tau_0^2 + 4 c_s^-4 C_S^2 |Q|) - tau_0)/2                P:164-173 eq. (8)-(9), A23
  *   init       f_i(x,0) = f^eq_i(rho0(x), u0(x))
  *   macro      rho = sum f_i, velocity v of eq. (16)
  *

@@ -98,6 +98,10 @@ int pick_vec(const lbm_params *p, double nonbulk_fraction) {
     const int widest = p->precision == LBM_F32 ? 4 : 2;
     int v = 1;
     if (p->model != LBM_SC2) v = p->precision == LBM_F64 ? 2 : (nonbulk_fraction < 0.2 ? 4 : 2);
+    // regularized LBGK / Smagorinsky carry six second moments per node: 2-node packs (cavity box:
+    // LES 43.0 vs 33.9 GLUPS at V = 4, regularized 42.9 vs 41.4)
+    // and so does MRT with its 19 moments (cavity box: 43.0 vs 41.0 GLUPS)
+    if (p->model == LBM_BGK_REG || p->model == LBM_BGK_LES || p->model == LBM_MRT) v = v > 2 ? 2 : v;
     v = env_int("LBM_VEC", v, 1, widest);
     if (v == 3) v = 2;
     while (v > 1 && p->nx % v) v /= 2;
