@@ -261,6 +261,7 @@ LBM_API int lbm_step(lbm_ctx *c, int n) {
         if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
         if (e != cudaSuccess) return fail(c, LBM_ECUDA, "reading the geometry counter: %s", cudaGetErrorString(e));
         c->vec = pick_vec(&c->p, (double)nonbulk / (double)c->g.N);
+        c->eager_links = env_int("LBM_EAGER_LINKS", (double)nonbulk / (double)c->g.N >= 0.2 ? 1 : 0, 0, 1);
         c->vec_pending = false;
     }
     while (c->use_graph && n >= GRAPH_STEPS) {

@@ -307,19 +307,49 @@ __device__ __forceinline__ void update_span(T (&h)[V][L::Q], uint32_t types, con
     }
 }
 
+// Link words of a pack with one vector load (geometries where most nodes are BOUNDARY: the words
+// are then fetched together with the types and the pull, not after the types have arrived).
+template <int V> __device__ __forceinline__ void load_links(const uint32_t *__restrict__ link, int n0, uint32_t (&w)[V]) {
+    if (V == 4) { const uint4 v = __ldg(reinterpret_cast<const uint4 *>(link + n0)); w[0] = v.x; w[1] = v.y; w[2] = v.z; w[V - 1] = v.w; }
+    else if (V == 2) { const uint2 v = __ldg(reinterpret_cast<const uint2 *>(link + n0)); w[0] = v.x; w[V - 1] = v.y; }
+    else w[0] = __ldg(link + n0);
+}
+
+template <class L, typename T, int V, typename I>
+__device__ __forceinline__ void pull_reflected_span_eager(const T *__restrict__ src, int64_t N, int n0, uint32_t types,
+                                                          const uint32_t (&w)[V], T (&h)[V][L::Q]) {
+    if (types & PACK_LINKS) {
+#pragma unroll
+        for (int k = 0; k < V; k++)
+            if (((types >> (8 * k)) & 0xffu) & NODE_LINKS) pull_reflected<L, T, I>(src, n0 + k, N, w[k], h[k]);
+    }
+}
+
 // ---- the fused step: pull-stream + moments + equilibrium + collision (+ Guo) + store ---------
 // Rows a1-a8 of DESIGN.md.  All loads of the pack are issued before first use (bytes in flight).
 template <class L, typename T, int V, typename I, int MODEL, int FORCE>
 __global__ void __launch_bounds__(256)
 step_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restrict__ link,
-            const T *__restrict__ src, T *__restrict__ dst, Relax<T> rp) {
+            const T *__restrict__ src, T *__restrict__ dst, Relax<T> rp, int eager_links) {
     Span s;
     if (!thread_span<V>(g, s)) return;
-    const uint32_t types = load_types<V>(type, s.row + s.x0);
-    if (all_solid<V>(types)) return;
+    const int n0 = s.row + s.x0;
+    const uint32_t types = load_types<V>(type, n0);
     T h[V][L::Q];
-    gather_span<L, T, V, I>(src, g.N, s, h);
-    pull_reflected_span<L, T, V, I>(src, g.N, s.row + s.x0, types, link, h);
+    if (eager_links) {
+        // obstacle-rich geometry (c3: 57 % BOUNDARY nodes): types, link words and the pull are
+        // issued together, the reflected links follow one memory round trip later (ncu showed
+        // half of the stalls of this kernel on the type -> link -> fix-up dependency chain)
+        uint32_t w[V];
+        load_links<V>(link, n0, w);
+        gather_span<L, T, V, I>(src, g.N, s, h);
+        if (all_solid<V>(types)) return;
+        pull_reflected_span_eager<L, T, V, I>(src, g.N, n0, types, w, h);
+    } else {
+        if (all_solid<V>(types)) return;
+        gather_span<L, T, V, I>(src, g.N, s, h);
+        pull_reflected_span<L, T, V, I>(src, g.N, n0, types, link, h);
+    }
     update_span<L, T, V, MODEL, FORCE>(h, types, rp);
     store_span<L, T, V, I>(dst, g.N, s.row + s.x0, h);
 }

@@ -30,7 +30,7 @@ template <class L, typename T> struct Steps {
             return LBM_OK;
         }
         for (int t = 0; t < n; t++) {
-            step_kernel<L, T, V, I, MODEL, FORCE><<<l.grid, l.block, 0, c->stream>>>(c->g, type(c), link(c), src(c, 0), dst(c, 0), rp);
+            step_kernel<L, T, V, I, MODEL, FORCE><<<l.grid, l.block, 0, c->stream>>>(c->g, type(c), link(c), src(c, 0), dst(c, 0), rp, c->eager_links);
             if (int rc = check_launch(c, "step_kernel")) return rc;
             c->cur ^= 1;
             c->steps++;
