@@ -47,8 +47,6 @@ int validate(const lbm_params *p, int *Q, int *D) {
     if (p->model == LBM_SC2 && p->sc_psi != LBM_PSI_RHO && p->sc_psi != LBM_PSI_1MEXP)
         return fail(nullptr, LBM_EINVAL, "unknown sc_psi");
     if (p->lattice == LBM_D2Q9 && p->force[2] != 0.0) return fail(nullptr, LBM_EINVAL, "D2Q9 force has no z component");
-    if (p->store == LBM_STORE_AA && p->model == LBM_SC2)
-        return fail(nullptr, LBM_EUNSUPPORTED, "AA store is built for the single-component models only");
     if (p->ny > 65535 || p->nz > 65535) return fail(nullptr, LBM_EUNSUPPORTED, "ny and nz must be <= 65535");
     return LBM_OK;
 }

@@ -148,35 +148,36 @@ template <class L, typename T> struct Impl {
         return check_launch(c, "build_links_kernel");
     }
 
-    template <int MODE> static int aa_convert(lbm_ctx *c, const void *in0, const void *in1, void *out0, void *out1) {
+    template <int MODE> static int aa_convert(lbm_ctx *c, int s, const void *in0, const void *in1, void *out0, void *out1) {
+        const double hf = c->p.model == LBM_SC2 ? 0.0 : 0.5;  // SC2 reports the bare component velocity
         aa_convert_kernel<L, T, MODE><<<grid_of(c), c->block_x, 0, c->stream>>>(
-            c->g, c->cur, type(c), link(c), at<T>(c, c->lay.store[0][0]), (const T *)in0, (const T *)in1, (T *)out0,
-            (T *)out1, T(0.5 * c->p.force[0]), T(0.5 * c->p.force[1]), T(0.5 * c->p.force[2]));
+            c->g, c->cur, type(c), link(c), at<T>(c, c->lay.store[s][0]), (const T *)in0, (const T *)in1, (T *)out0,
+            (T *)out1, T(hf * c->p.force[0]), T(hf * c->p.force[1]), T(hf * c->p.force[2]));
         return check_launch(c, "aa_convert_kernel");
     }
 
     static int init_equilibrium(lbm_ctx *c, int s, const void *rho, const void *u) {
-        if (c->aa) return aa_convert<2>(c, rho, u, nullptr, nullptr);
+        if (c->aa) return aa_convert<2>(c, s, rho, u, nullptr, nullptr);
         init_equilibrium_kernel<L, T><<<grid_of(c), c->block_x, 0, c->stream>>>(
             c->g, type(c), link(c), (const T *)rho, (const T *)u, at<T>(c, c->lay.store[s][c->cur]));
         return check_launch(c, "init_equilibrium_kernel");
     }
 
     static int set_distributions(lbm_ctx *c, int s, const void *f) {
-        if (c->aa) return aa_convert<0>(c, f, nullptr, nullptr, nullptr);
+        if (c->aa) return aa_convert<0>(c, s, f, nullptr, nullptr, nullptr);
         set_distributions_kernel<L, T><<<grid_of(c), c->block_x, 0, c->stream>>>(
             c->g, type(c), link(c), (const T *)f, at<T>(c, c->lay.store[s][c->cur]));
         return check_launch(c, "set_distributions_kernel");
     }
 
     static int get_distributions(lbm_ctx *c, int s, void *f) {
-        if (c->aa) return aa_convert<1>(c, nullptr, nullptr, f, nullptr);
+        if (c->aa) return aa_convert<1>(c, s, nullptr, nullptr, f, nullptr);
         get_distributions_kernel<L, T><<<grid_of(c), c->block_x, 0, c->stream>>>(c->g, type(c), link(c), src(c, s), (T *)f);
         return check_launch(c, "get_distributions_kernel");
     }
 
     static int macro(lbm_ctx *c, int s, void *rho, void *u) {
-        if (c->aa) return aa_convert<3>(c, nullptr, nullptr, rho, u);
+        if (c->aa) return aa_convert<3>(c, s, nullptr, nullptr, rho, u);
         const bool sc = c->p.model == LBM_SC2;  // SC2: bare component velocity (lbm.h)
         macro_kernel<L, T><<<grid_of(c), c->block_x, 0, c->stream>>>(
             c->g, type(c), link(c), src(c, s), (T *)rho, (T *)u, sc ? T(0) : T(0.5 * c->p.force[0]),

@@ -636,6 +636,43 @@ __device__ __forceinline__ void psi_gradient(const typename Pair<T>::type *__res
     }
 }
 
+// Collision of both components at one node (rows a10-a11): moments, common velocity u',
+// coupling forces (eq. 10, sign A11) + body force, Guo (A13) or EDM (A22) per component; node types
+// FULLWAY / VELOCITY replace the collision of both components.
+template <class L, typename T, int PSI, int FS>
+__device__ __forceinline__ void sc_collide_node(T (&hA)[L::Q], T (&hB)[L::Q], uint32_t t,
+                                                const typename Pair<T>::type *__restrict__ psi, int n, const Nbr &o,
+                                                const Relax<T> &rpA, const Relax<T> &rpB, T G) {
+    if (t & (NODE_FULLWAY | NODE_VELOCITY)) {
+        if (t & NODE_FULLWAY) { fullway_reverse<L, T>(hA); fullway_reverse<L, T>(hB); }
+        else { velocity_node<L, T>(hA, rpA.ubc); velocity_node<L, T>(hB, rpB.ubc); }
+        return;
+    }
+    T SA[3], SB[3];
+    psi_gradient<L, T>(psi, n, o, SA, SB);
+    T dA, dB, jA[3], jB[3];
+    moments<L, T>(hA, dA, jA);
+    moments<L, T>(hB, dB, jB);
+    const T rA = T(1) + dA, rB = T(1) + dB;
+    const T pA = psi_dev<T, PSI>(dA) + psi_one<T, PSI>(), pB = psi_dev<T, PSI>(dB) + psi_one<T, PSI>();
+    const T inv_den = T(1) / (rA * rpA.inv_tau + rB * rpB.inv_tau);
+    const T irA = T(0.5) / rA, irB = T(0.5) / rB;
+    T vA[3], vB[3], mA[3], mB[3], FA[3], FB[3];
+#pragma unroll
+    for (int a = 0; a < 3; a++) {
+        const T up = (jA[a] * rpA.inv_tau + jB[a] * rpB.inv_tau) * inv_den;
+        FA[a] = -G * pA * SB[a] + rA * rpA.g[a];
+        FB[a] = -G * pB * SA[a] + rB * rpB.g[a];
+        // Guo: v_s = u' + F_s / (2 rho_s) (A13); EDM: the bare common velocity u' (A22)
+        vA[a] = FS == FORCE_EDM ? up : up + FA[a] * irA;
+        vB[a] = FS == FORCE_EDM ? up : up + FB[a] * irB;
+        mA[a] = rA * vA[a];
+        mB[a] = rB * vB[a];
+    }
+    collide<L, T, MODEL_BGK, FS>(hA, rA, dA, vA, mA, FA, rpA);
+    collide<L, T, MODEL_BGK, FS>(hB, rB, dB, vB, mB, FB, rpB);
+}
+
 // Pass 2 (rows a10-a11): both components in one kernel: gather, moments, common velocity u'
 // (P:188), forces (eq. 10, sign A11) + body force, v_s = u' + F_s / (2 rho_s), LBGK + Guo (A13).
 template <class L, typename T, int V, typename I, int PSI, int FS>
@@ -656,42 +693,69 @@ sc_step_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restr
     pull_reflected_span<L, T, V, I>(srcB, g.N, n0, types, link, hB);
 #pragma unroll
     for (int k = 0; k < V; k++) {
-        const uint32_t t = (types >> (8 * k)) & 0xffu;
-        if (t & (NODE_FULLWAY | NODE_VELOCITY)) {  // these replace the collision of both components
-            if (t & NODE_FULLWAY) { fullway_reverse<L, T>(hA[k]); fullway_reverse<L, T>(hB[k]); }
-            else { velocity_node<L, T>(hA[k], rpA.ubc); velocity_node<L, T>(hB[k], rpB.ubc); }
-            continue;
-        }
         Nbr o = s.o;
         const int x = s.x0 + k;
         o.xm = (x == 0) ? (g.nx - 1) : -1;
         o.xp = (x == g.nx - 1) ? -(g.nx - 1) : 1;
-        T SA[3], SB[3];
-        psi_gradient<L, T>(psi, n0 + k, o, SA, SB);
-        T dA, dB, jA[3], jB[3];
-        moments<L, T>(hA[k], dA, jA);
-        moments<L, T>(hB[k], dB, jB);
-        const T rA = T(1) + dA, rB = T(1) + dB;
-        const T pA = psi_dev<T, PSI>(dA) + psi_one<T, PSI>(), pB = psi_dev<T, PSI>(dB) + psi_one<T, PSI>();
-        const T inv_den = T(1) / (rA * rpA.inv_tau + rB * rpB.inv_tau);
-        const T irA = T(0.5) / rA, irB = T(0.5) / rB;
-        T vA[3], vB[3], mA[3], mB[3], FA[3], FB[3];
-#pragma unroll
-        for (int a = 0; a < 3; a++) {
-            const T up = (jA[a] * rpA.inv_tau + jB[a] * rpB.inv_tau) * inv_den;
-            FA[a] = -G * pA * SB[a] + rA * rpA.g[a];
-            FB[a] = -G * pB * SA[a] + rB * rpB.g[a];
-            // Guo: v_s = u' + F_s / (2 rho_s) (A13); EDM: the bare common velocity u' (A22)
-            vA[a] = FS == FORCE_EDM ? up : up + FA[a] * irA;
-            vB[a] = FS == FORCE_EDM ? up : up + FB[a] * irB;
-            mA[a] = rA * vA[a];
-            mB[a] = rB * vB[a];
-        }
-        collide<L, T, MODEL_BGK, FS>(hA[k], rA, dA, vA, mA, FA, rpA);
-        collide<L, T, MODEL_BGK, FS>(hB[k], rB, dB, vB, mB, FB, rpB);
+        sc_collide_node<L, T, PSI, FS>(hA[k], hB[k], (types >> (8 * k)) & 0xffu, psi, n0 + k, o, rpA, rpB, G);
     }
     store_span<L, T, V, I>(dstA, g.N, n0, hA);
     store_span<L, T, V, I>(dstB, g.N, n0, hB);
+}
+
+
+// ---- Shan-Chen on the in-place AA store: one node per thread, both parities (see aa_slot) ------
+template <class L, typename T, typename I, int PSI>
+__global__ void __launch_bounds__(256)
+aa_sc_fields_kernel(Geom g, int parity, const uint8_t *__restrict__ type, const uint32_t *__restrict__ link,
+                    const T *fA, const T *fB, typename Pair<T>::type *__restrict__ psi) {
+    Span s;
+    if (!thread_span<1>(g, s)) return;
+    const int n = s.row + s.x0;
+    const uint8_t t = type[n];
+    typename Pair<T>::type p;
+    p.x = p.y = -psi_one<T, PSI>();  // dry nodes: psi = 0 (A14)
+    if (!(t & (NODE_SOLID | NODE_FULLWAY))) {
+        const uint32_t w = (t & NODE_LINKS) ? __ldg(link + n) : 0u;
+        const Nbr o = neighbours(g, s.x0, s.y, s.z);
+        T sA = T(0), sB = T(0);
+#pragma unroll
+        for (int i = 0; i < L::Q; i++) {
+            const I sl = aa_slot<L, I>(parity, i, n, g.N, o, w);
+            sA += fA[sl];
+            sB += fB[sl];
+        }
+        p.x = psi_dev<T, PSI>(sA);
+        p.y = psi_dev<T, PSI>(sB);
+    }
+    psi[n] = p;
+}
+
+template <class L, typename T, typename I, int PSI, int FS>
+__global__ void __launch_bounds__(256)
+aa_sc_step_kernel(Geom g, int parity, const uint8_t *__restrict__ type, const uint32_t *__restrict__ link, T *fA,
+                  T *fB, const typename Pair<T>::type *__restrict__ psi, Relax<T> rpA, Relax<T> rpB, T G) {
+    Span s;
+    if (!thread_span<1>(g, s)) return;
+    const int n = s.row + s.x0;
+    const uint8_t t = type[n];
+    if (t & NODE_SOLID) return;
+    const uint32_t w = (t & NODE_LINKS) ? __ldg(link + n) : 0u;
+    const Nbr o = neighbours(g, s.x0, s.y, s.z);
+    I slot[L::Q];
+    T hA[L::Q], hB[L::Q];
+#pragma unroll
+    for (int i = 0; i < L::Q; i++) {
+        slot[i] = aa_slot<L, I>(parity, i, n, g.N, o, w);
+        hA[i] = fA[slot[i]];
+        hB[i] = fB[slot[i]];
+    }
+    sc_collide_node<L, T, PSI, FS>(hA, hB, t, psi, n, o, rpA, rpB, G);
+#pragma unroll
+    for (int i = 0; i < L::Q; i++) {  // the slot the read of ibar came from (even: (ibar, x); odd: (i, x + e_i) ...)
+        fA[slot[L::opp(i)]] = hA[i];
+        fB[slot[L::opp(i)]] = hB[i];
+    }
 }
 
 }  // namespace lbm

@@ -56,6 +56,22 @@ template <class L, typename T> struct Steps {
         const Launch l = span_launch(c, V);
         const Relax<T> rA = make_relax<T>(c, 0), rB = make_relax<T>(c, 1);
         auto *psi = at<typename Pair<T>::type>(c, c->lay.psi[0]);
+        if (c->aa) {  // in place: one node per thread, `cur` is the parity
+            if constexpr (V != 1) return fail(c, LBM_EUNSUPPORTED, "internal: AA Shan-Chen runs one node per thread");
+            else {
+                T *fA = at<T>(c, c->lay.store[0][0]), *fB = at<T>(c, c->lay.store[1][0]);
+                for (int t = 0; t < n; t++) {
+                    aa_sc_fields_kernel<L, T, I, PSI><<<l.grid, l.block, 0, c->stream>>>(c->g, c->cur, type(c), link(c), fA, fB, psi);
+                    if (int rc = check_launch(c, "aa_sc_fields_kernel")) return rc;
+                    aa_sc_step_kernel<L, T, I, PSI, FS><<<l.grid, l.block, 0, c->stream>>>(
+                        c->g, c->cur, type(c), link(c), fA, fB, psi, rA, rB, T(c->p.sc_G));
+                    if (int rc = check_launch(c, "aa_sc_step_kernel")) return rc;
+                    c->cur ^= 1;
+                    c->steps++;
+                }
+                return LBM_OK;
+            }
+        }
         for (int t = 0; t < n; t++) {
             sc_fields_kernel<L, T, V, I, PSI><<<l.grid, l.block, 0, c->stream>>>(c->g, type(c), link(c), src(c, 0), src(c, 1), psi);
             if (int rc = check_launch(c, "sc_fields_kernel")) return rc;
@@ -70,7 +86,7 @@ template <class L, typename T> struct Steps {
 
     template <int PSI> static int step_sc(lbm_ctx *c, int n) {
         if constexpr (sizeof(T) == 4) {  // fp64 with two components and V = 2 would spill
-            if (c->vec >= 2) return step_sc_v<2, PSI>(c, n);
+            if (c->vec >= 2 && !c->aa) return step_sc_v<2, PSI>(c, n);
         }
         return step_sc_v<1, PSI>(c, n);
     }

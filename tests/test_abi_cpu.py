@@ -69,7 +69,6 @@ def test_lattice_info_table1(lib):
     (dict(nx=2048, ny=2048, nz=1024), binding.LBM_EINVAL),
     (dict(lattice=0, nz=4), binding.LBM_EINVAL),
     (dict(model=1, rates=[2.5] * 19), binding.LBM_EINVAL),
-    (dict(store=1, model=2, tau=(1.0, 1.0)), binding.LBM_EUNSUPPORTED),
     (dict(store=7), binding.LBM_EINVAL),
     (dict(bc_velocity=(1.5, 0.0, 0.0)), binding.LBM_EINVAL),
     (dict(force_scheme=5), binding.LBM_EINVAL),

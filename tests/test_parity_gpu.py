@@ -314,3 +314,18 @@ def test_smagorinsky_zero_constant_matches_lbgk_bitwise(B):
         sim.step(50)
         out.append(sim.get_distributions())
     assert float((out[0] - out[1]).abs().max()) < 1e-14
+
+
+# ---- Shan-Chen on the in-place AA store ------------------------------------------------------------------
+@pytest.mark.parametrize("precision,shape", [(W.F32, (48, 40, 32)), (W.F64, (35, 30, 21))])
+def test_aa_c5_shan_chen(B, orc, precision, shape):
+    check_parity_live(B, orc, W.c5_shan_chen(*shape, precision=precision), steps=101, store=B.LBM_STORE_AA)
+
+
+@pytest.mark.parametrize("scheme", [W.FORCE_GUO, W.FORCE_EDM])
+def test_aa_shan_chen_with_node_types_and_force(B, orc, scheme):
+    mask, rho, u = W.random_types(W.D3Q19, 30, 16, 9, seed=47, ncomp=2)
+    w = W.Workload("types_sc_aa", W.D3Q19, W.SC2, W.F64, 30, 16, 9, (0.8, 1.1), 100, sc_G=0.6, sc_psi=1,
+                   force=(1e-5, 2e-5, 0.0), bc_velocity=(0.01, 0.0, -0.01), force_scheme=scheme)
+    w.mask, w.rho, w.u = mask, rho, u
+    check_parity_live(B, orc, w, steps=61, store=B.LBM_STORE_AA)
