@@ -106,6 +106,19 @@ int pick_vec(const lbm_params *p, double nonbulk_fraction) {
     return v;
 }
 
+// Cluster-resident path (resident_kernel): single component, AB store, and both buffers of a CTA's
+// share of the lattice within ~200 KB of shared memory with at most 2 nodes per thread.
+int pick_resident(const lbm_params *p, int Q, int64_t N) {
+    if (p->model == LBM_SC2 || p->store != LBM_STORE_AB || env_int("LBM_NO_RESIDENT", 0, 0, 1)) return 0;
+    const size_t rs = p->precision == LBM_F32 ? 4 : 8;
+    int slog2 = 5;
+    while (((int64_t)RESIDENT_CTAS << slog2) < N) slog2++;
+    const size_t S = (size_t)1 << slog2;
+    if (S > (size_t)RESIDENT_THREADS * RESIDENT_NODES_PER_THREAD) return 0;
+    if (2 * (size_t)Q * S * rs > 200 * 1024) return 0;
+    return slog2;
+}
+
 int pick_block_x(int nx) {
     if (const char *e = getenv("LBM_BLOCK_X")) {
         const int v = atoi(e);
@@ -178,7 +191,8 @@ LBM_API int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, voi
     c->block_threads = env_int("LBM_BLOCK_THREADS", 64, 32, 256);
     c->vt = select_impl(p);
     c->err[0] = 0;
-    c->use_graph = c->g.N <= GRAPH_MAX_SITES && !env_int("LBM_NO_GRAPH", 0, 0, 1);
+    c->resident_slog2 = pick_resident(p, Q, c->g.N);
+    c->use_graph = c->resident_slog2 == 0 && c->g.N <= GRAPH_MAX_SITES && !env_int("LBM_NO_GRAPH", 0, 0, 1);
     if (c->use_graph && cudaStreamCreateWithFlags(&c->capture_stream, cudaStreamNonBlocking) != cudaSuccess) {
         cudaGetLastError();
         c->use_graph = false;

@@ -42,6 +42,7 @@ struct lbm_ctx {
     bool vec_pending;   // geometry changed: re-pick `vec` from the non-bulk node count at the next step
     int64_t steps, launches;
     bool aa;            // LBM_STORE_AA: one buffer, `cur` is the step parity (0 even, 1 odd)
+    int resident_slog2; // > 0: the AB store fits one cluster's shared memory; log2 of nodes per CTA
     int eager_links;    // fetch link words with the types (set when >= 20 % of the nodes are not BULK)
     bool idx32;         // Q * N < 2^32: slot numbers fit 32 bits (cheaper address arithmetic)
     int block_x;        // one-node-per-thread kernels: 1-D block along x

@@ -38,7 +38,23 @@ template <class L, typename T> struct Steps {
         return LBM_OK;
     }
 
+    // Whole lbm_step(n) in one launch for lattices that fit the shared memory of an 8-CTA cluster.
+    template <int MODEL, int FORCE> static int step_resident(lbm_ctx *c, int n, const Relax<T> &rp) {
+        auto kernel = resident_kernel<L, T, MODEL, FORCE>;
+        const size_t smem = 2 * (size_t)L::Q * ((size_t)1 << c->resident_slog2) * sizeof(T);
+        cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return fail(c, LBM_ECUDA, "cudaFuncSetAttribute(resident_kernel): %s", cudaGetErrorString(e));
+        const int after = c->cur ^ (n & 1);
+        kernel<<<RESIDENT_CTAS, RESIDENT_THREADS, smem, c->stream>>>(c->g, c->resident_slog2, type(c), link(c), src(c, 0),
+                                                                      at<T>(c, c->lay.store[0][after]), rp, n);
+        if (int rc = check_launch(c, "resident_kernel")) return rc;
+        c->cur = after;
+        c->steps += n;
+        return LBM_OK;
+    }
+
     template <int MODEL, int FORCE> static int step_single(lbm_ctx *c, int n, const Relax<T> &rp) {
+        if (c->resident_slog2 > 0 && n >= 2 && !c->aa) return step_resident<MODEL, FORCE>(c, n, rp);
         if constexpr (sizeof(T) == 4) {
             if (c->vec == 4) return step_single_v<4, MODEL, FORCE>(c, n, rp);
         }

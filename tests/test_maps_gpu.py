@@ -93,7 +93,8 @@ def test_set_get_distributions_round_trip_bit_exact(B):
 def test_graph_replay_is_bit_identical_to_single_launches(B, cfg):
     """Small lattices replay 50-step CUDA graphs (launch-bound regime): step(120) must give
     exactly the bits of 120 x step(1), which never reaches the graph threshold."""
-    w = W.c1_taylor_green(64) if cfg == "c1" else W.c5_shan_chen(24, 20, 16)
+    # 96^2 = 9216 nodes: above the cluster-resident limit (4096), below the graph limit (2^20)
+    w = W.c1_taylor_green(96) if cfg == "c1" else W.c5_shan_chen(24, 20, 16)
     out = []
     for chunks in ([120], [1] * 120, [50, 7, 63]):
         sim = B.from_workload(w)
@@ -178,3 +179,39 @@ def test_full_size_sampled_against_oracle(B, orc, cfg, n):
     for s in range(w.ncomp):  # mass of each component is conserved (A8 permutation; A13)
         m1 = float(sim.macro(s)[0].double().sum())
         assert abs(m1 - m0[s]) <= (2e-7 if w.precision == W.F32 else 1e-13) * m0[s]
+
+
+@pytest.mark.parametrize("lattice,shape,model", [(W.D2Q9, (64, 64, 1), W.BGK), (W.D2Q9, (50, 37, 1), W.MRT),
+                                                 (W.D3Q19, (16, 16, 16), W.BGK), (W.D3Q19, (13, 9, 7), W.LES)])
+def test_cluster_resident_path_matches_single_launches_and_oracle(B, orc, lattice, shape, model):
+    """Lattices of up to 4096 nodes run lbm_step(n) as ONE launch of a thread-block cluster that keeps
+    both buffers in distributed shared memory: must equal n single-step launches bit for bit (same
+    arithmetic, same streaming rule) and the oracle within tolerance; all node types included."""
+    import torch
+    nx, ny, nz = shape
+    mask, rho, u = W.random_types(lattice, nx, ny, nz, seed=91)
+    D = 2 if lattice == W.D2Q9 else 3
+    rates = (W.mrt_rates_d3q19(0.7) if lattice == W.D3Q19 else W.mrt_rates_d2q9(0.7)) if model == W.MRT else None
+    w = W.Workload("resident", lattice, model, W.F64, nx, ny, nz, (0.7, 0.7), 60, rates=rates, smagorinsky_cs=0.15,
+                   force=(1e-5, -2e-5, 3e-5 if D == 3 else 0.0), bc_velocity=(0.02, -0.01, 0.0))
+    w.mask, w.rho, w.u = mask, rho, u
+    out = []
+    for chunks in ([60], [1] * 60, [7, 53]):
+        sim = B.from_workload(w)
+        sim.set_geometry(w.mask)
+        sim.init_equilibrium(w.rho[0], w.u[0])
+        l0 = sim.counters()[1]
+        for n in chunks:
+            sim.step(n)
+        assert sim.counters()[0] == 60
+        if chunks == [60]:
+            assert sim.counters()[1] - l0 == 1      # one kernel for all 60 steps
+        out.append(sim.get_distributions().clone())
+        sim.close()
+    assert torch.equal(out[0], out[1]) and torch.equal(out[0], out[2])
+    ref = orc.Oracle(**w.params())
+    ref.set_geometry(w.mask)
+    ref.init_equilibrium(w.rho[0], w.u[0])
+    ref.step(60)
+    live = w.mask != W.SOLID
+    assert np.abs(out[0].cpu().numpy() - ref.get_distributions())[:, live].max() <= 1e-12
