@@ -112,7 +112,10 @@ int lbm_init_equilibrium(lbm_ctx *ctx, int comp, const void *d_rho, const void *
  * LBM_SC2 runs the macro-field pass and then the coupled collide pass (eq. 10).
  * LBM_ESTATE if a component has not been initialised.  Asynchronous, except that the first call
  * after lbm_set_geometry synchronises the stream once (it reads back how many nodes are not
- * bulk fluid to pick the kernel variant). */
+ * bulk fluid to pick the kernel variant).  Lattices of up to 2^20 nodes replay 50-step CUDA graphs,
+ * lattices of up to 4096 nodes (single component, AB store) run all n steps in one launch of a
+ * thread-block cluster that keeps the store in distributed shared memory; results are bit-identical
+ * to single-step launches. */
 int lbm_step(lbm_ctx *ctx, int n);
 
 /* rho = sum_i f_i, velocity v of eq. (16) (includes g/2) from the current state.
