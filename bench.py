@@ -176,10 +176,20 @@ def run_ours(args):
 
     rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
-    torch.cuda.set_device(local)
-    dev = torch.device("cuda", local)
+    ndev = torch.cuda.device_count()
+    if ndev == 0:
+        raise RuntimeError("bench.py needs a CUDA device (the CUDA library is the only implementation)")
+    dev_index = local % ndev  # one rank per GPU; ranks share a GPU only in the 1-GPU test of this code path
+    torch.cuda.set_device(dev_index)
+    dev = torch.device("cuda", dev_index)
     if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
+        # NCCL for the barrier and the max-over-ranks reduction; LBM_BENCH_BACKEND=gloo lets the N > 1
+        # code path be exercised on a box with fewer GPUs than ranks (NCCL refuses two ranks per GPU)
+        backend = os.environ.get("LBM_BENCH_BACKEND", "nccl")
+        if backend == "nccl":
+            dist.init_process_group("nccl", device_id=dev)
+        else:
+            dist.init_process_group(backend)
     binding.load()  # no fallback: raises if the CUDA library is missing
 
     K, Wm = args.steps, max(args.warmup, 3)
@@ -197,7 +207,7 @@ def run_ours(args):
         torch.cuda.synchronize(dev)
 
     # ---- device-resident: K steps between CUDA events on the context's stream -------------------
-    clocks = ClockSampler(local)  # runs through warm-up, the timed steps and the end-to-end call
+    clocks = ClockSampler(dev_index)  # runs through warm-up, the timed steps and the end-to-end call
     sim.step(Wm)
     l0 = sim.counters()[1]
     barrier()
