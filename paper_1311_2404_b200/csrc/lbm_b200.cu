@@ -100,6 +100,11 @@ int pick_vec(const lbm_params *p, double nonbulk_fraction) {
     // LES 43.0 vs 33.9 GLUPS at V = 4, regularized 42.9 vs 41.4)
     // and so does MRT with its 19 moments (cavity box: 43.0 vs 41.0 GLUPS)
     if (p->model == LBM_BGK_REG || p->model == LBM_BGK_LES || p->model == LBM_MRT) v = v > 2 ? 2 : v;
+    // small lattices cannot fill 148 SMs with wide packs (us per step at V = 1/2/4: D2Q9 128^2 1.68/1.83/2.14,
+    // 256^2 2.07/2.14/2.35, 512^2 3.46/3.20/3.67; D3Q19 48^3 3.86/3.53/4.92, 64^3 5.73/5.61/8.03, 96^3 23.3/22.2/23.3)
+    const int64_t sites = (int64_t)p->nx * p->ny * p->nz;
+    if (sites <= (1 << 16)) v = 1;
+    else if (sites < (1 << 20) && v > 2) v = 2;
     v = env_int("LBM_VEC", v, 1, widest);
     if (v == 3) v = 2;
     while (v > 1 && p->nx % v) v /= 2;
