@@ -117,8 +117,8 @@ template <class L, typename T> struct Steps {
                 rp.cs[k] = T((1.0 - 0.5 * c->p.rates[k]) / Mrt<L, T>::norm(k));
                 rp.in[k] = T(1.0 / Mrt<L, T>::norm(k));
             }
-        if (!force) return step_single<MODEL, FORCE_NONE>(c, n, rp);
         if (MODEL == MODEL_LES) rp.cs2x36 = T(36.0 * c->p.smagorinsky_cs * c->p.smagorinsky_cs);
+        if (!force) return step_single<MODEL, FORCE_NONE>(c, n, rp);
         if (edm) return step_single<MODEL, FORCE_EDM>(c, n, rp);
         if constexpr (MODEL == MODEL_REG) return fail(c, LBM_EUNSUPPORTED, "regularized LBGK takes a body force through the EDM only");
         else return step_single<MODEL, FORCE_GUO>(c, n, rp);

@@ -287,10 +287,12 @@ def test_edm_shan_chen(B, orc, precision, lattice, shape):
 @pytest.mark.parametrize("lattice,precision,shape,scheme", [
     (W.D3Q19, W.F32, (48, 21, 10), W.FORCE_EDM), (W.D3Q19, W.F64, (37, 14, 9), W.FORCE_EDM),
     (W.D3Q19, W.F32, (40, 12, 11), W.FORCE_GUO), (W.D2Q9, W.F64, (66, 31, 1), W.FORCE_EDM),
-    (W.D2Q9, W.F32, (52, 30, 1), W.FORCE_GUO)])
+    (W.D2Q9, W.F32, (52, 30, 1), W.FORCE_GUO), (W.D3Q19, W.F64, (16, 34, 7), None), (W.D2Q9, W.F32, (128, 16, 1), None)])
 def test_regularized_and_smagorinsky(B, orc, model, lattice, precision, shape, scheme, store):
     D = 2 if lattice == W.D2Q9 else 3
     force = (1e-4, -2e-4, 3e-4 if D == 3 else 0.0)
+    if scheme is None:  # no body force at all (regression: the Smagorinsky constant was dropped on this path)
+        force, scheme = (0.0, 0.0, 0.0), W.FORCE_GUO
     if model == W.REG and scheme == W.FORCE_GUO:
         force = (0.0, 0.0, 0.0)  # regularized LBGK takes a force through the EDM only (A23)
     w = generic(lattice, model, precision, shape, 71, tau=(0.58, 0.58), force=force, force_scheme=scheme,
