@@ -172,14 +172,16 @@ def test_shan_chen_binary_poiseuille(B):
     assert r1[n // 2] > 0.9 and r0[n // 2] < 0.1 and r0[3] > 0.9 and r1[3] < 0.1
 
 
-def test_regularized_and_mrt_survive_where_lbgk_diverges(B):
+def test_regularized_smagorinsky_and_mrt_survive_where_lbgk_diverges(B):
     """"Single fluid models with enhanced stability": lid-driven cavity 64^3 at
     Re = 5000 with U = 0.1, i.e. tau = 0.5037.  Plain LBGK blows up within a few thousand steps;
-    the regularized model and MRT (rates of reading A7) run 20000 steps and stay bounded."""
+    the regularized model, the Smagorinsky model (C_S = 0.1) and MRT (rates of reading A7) run
+    20000 steps and stay bounded."""
     import torch
     outcome = {}
-    for name, model in (("bgk", W.BGK), ("reg", W.REG), ("mrt", W.MRT)):
+    for name, model in (("bgk", W.BGK), ("reg", W.REG), ("les", W.LES), ("mrt", W.MRT)):
         w = W.ldc_cavity(64, 64, 64, Re=5000.0, U=0.1, model=model)
+        w.smagorinsky_cs = 0.1
         sim = start(B, w)
         ok = True
         for _ in range(20):
@@ -190,4 +192,4 @@ def test_regularized_and_mrt_survive_where_lbgk_diverges(B):
                 break
         outcome[name] = ok
         sim.close()
-    assert outcome == {"bgk": False, "reg": True, "mrt": True}, outcome
+    assert outcome == {"bgk": False, "reg": True, "les": True, "mrt": True}, outcome
