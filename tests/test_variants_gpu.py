@@ -1,0 +1,55 @@
+"""Every kernel variant the library can pick (pack width 1/2/4, 32- and 64-bit slot indices, link words
+fetched eagerly or lazily, graph replay on/off, cluster-resident path on/off) against the oracle.  The
+variants are normally chosen from the lattice size and geometry; the tuning environment variables
+(read at lbm_create / first lbm_step) force each one here so that none ships untested."""
+import itertools
+
+import numpy as np
+import pytest
+
+from paper_1311_2404_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+ENVS = [dict(LBM_VEC=v, LBM_IDX64=i, LBM_EAGER_LINKS=e, LBM_NO_GRAPH=g, LBM_NO_RESIDENT=g)
+        for v, i, e, g in itertools.product(("1", "2", "4"), ("0", "1"), ("0", "1"), ("0", "1"))]
+
+
+def cases():
+    mask, rho, u = W.random_types(W.D3Q19, 64, 12, 9, seed=3)
+    for model, precision, scheme in ((W.BGK, W.F32, W.FORCE_GUO), (W.MRT, W.F64, W.FORCE_EDM), (W.LES, W.F32, W.FORCE_GUO),
+                                     (W.REG, W.F64, W.FORCE_EDM)):
+        w = W.Workload("variants", W.D3Q19, model, precision, 64, 12, 9, (0.7, 0.7), 60, force=(1e-4, -2e-4, 1e-4),
+                       rates=W.mrt_rates_d3q19(0.7) if model == W.MRT else None, bc_velocity=(0.02, 0.0, -0.01),
+                       force_scheme=scheme, smagorinsky_cs=0.15)
+        w.mask, w.rho, w.u = mask, rho, u
+        yield w
+    mask, rho, u = W.random_types(W.D3Q19, 32, 10, 6, seed=4, ncomp=2)
+    w = W.Workload("variants_sc", W.D3Q19, W.SC2, W.F32, 32, 10, 6, (0.9, 1.1), 60, sc_G=0.7, force=(1e-5, 0, 0))
+    w.mask, w.rho, w.u = mask, rho, u
+    yield w
+
+
+@pytest.mark.parametrize("env", ENVS, ids=lambda e: "v%s_i64%s_eager%s_nograph%s" % (e["LBM_VEC"], e["LBM_IDX64"], e["LBM_EAGER_LINKS"], e["LBM_NO_GRAPH"]))
+def test_forced_variant_matches_oracle(orc, monkeypatch, env):
+    import torch
+    assert torch.cuda.is_available()
+    from paper_1311_2404_b200 import binding as B
+    for k, v in env.items():
+        monkeypatch.setenv(k, v)
+    for w in cases():
+        for store in (B.LBM_STORE_AB, B.LBM_STORE_AA):
+            sim = B.from_workload(w, store=store)
+            ref = orc.Oracle(**w.params())
+            sim.set_geometry(w.mask)
+            ref.set_geometry(w.mask)
+            for s in range(w.ncomp):
+                sim.init_equilibrium(w.rho[s], w.u[s], comp=s)
+                ref.init_equilibrium(w.rho[s], w.u[s], comp=s)
+            sim.step(61)
+            ref.step(61)
+            live = w.mask != W.SOLID
+            for s in range(w.ncomp):
+                d = np.abs(sim.get_distributions(s).cpu().numpy().astype(np.float64) - ref.get_distributions(s))
+                assert d[:, live].max() <= (1e-5 if w.precision == W.F32 else 1e-12), (env, w.model, store)
+            sim.close()
