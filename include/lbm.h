@@ -15,8 +15,8 @@
  *     planes, D = 2 for D2Q9, 3 for D3Q19).  Distributions: real[Q][nz][ny][nx] in the velocity
  *     order of reading A2 (lbm_lattice_info returns it).
  *   - The lattice is a torus: every axis is periodic.  Walls exist only through the
- *     node-type mask (0 = FLUID, 1 = SOLID); SOLID nodes are dry and reflect by half-way
- *     bounce-back (reading A8).
+ *     node-type mask (LBM_NODE_*): SOLID nodes are dry and reflect by half-way bounce-back
+ *     (reading A8); WALL_FULLWAY and VELOCITY nodes are described at the enum below.
  *   - All work is enqueued on the CUDA stream given to lbm_create; calls are asynchronous with
  *     respect to the host unless stated otherwise.  A context is not thread-safe.
  *   - `comp` is 0 except for LBM_SC2 (0 = component A, 1 = component B).
