@@ -51,6 +51,12 @@
  * laws / G = 0 / linear-gradient force, full-way wall (hand-tracked arrow, steady Poiseuille equals
  * the half-way profile), velocity node (uniform-flow fixed point, Couette flow), and one step with
  * all four node types against an independent whole-array numpy implementation.
+ * Round 2 (tests/test_oracle_pins_r2.py): Smagorinsky shear-wave decay predicted from eq. (9);
+ * Smagorinsky + Guo with C_S > 0 (exact momentum balance, numpy step); MRT + Guo with unequal rates
+ * (one collision in physical moments: trace / deviator / heat flux with their own rates and
+ * (1 - s_k/2) source prefactors; numpy step with np.linalg.inv; Poiseuille curvature); Shan-Chen
+ * with non-FLUID nodes (closed-form force beside a dry plane, numpy step with all node types,
+ * per-component mass with SOLID + WALL_FULLWAY nodes).
  * PARITY UNPINNED (no printed value in the paper): the physical sign of the
  * Shan-Chen coupling (reading A11) and the c3 rate s_m = 1.98 (a parameter, not arithmetic).
  */

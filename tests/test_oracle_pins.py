@@ -869,7 +869,11 @@ def test_regularized_keeps_the_viscosity_and_the_conservation_laws(orc):
     ratio = np.sqrt((v ** 2).sum() / (u ** 2).sum())
     assert abs(-np.log(ratio) / (2 * k * k * T) / nu - 1.0) < 5e-3   # O(k^2) lattice error at n = 32
     e = orc.lattice_tables(0)[0].astype(float)
-    assert abs(f1.sum() - f0.sum()) < 1e-13 * f0.sum()          # 300 steps of round-off on 1024 units of mass
+    # round-off bar, derived: a population is rounded a few times per step (projection, relaxation, sum); one
+    # rounding of every population is at most (ulp(4/9) + 4 ulp(1/9) + 4 ulp(1/36))/2 = 6.3e-17 per node and step,
+    # i.e. 1.9e-11 over 1024 nodes x 300 steps if all errors add coherently (measured drift: -1.9e-11, the
+    # projection's rounding is biased); allow five such roundings
+    assert abs(f1.sum() - f0.sum()) < 5 * 6.3e-17 * n * n * T
     assert np.max(np.abs(np.einsum("qzyx,qa->a", f1 - f0, e))) < 1e-12
 
 
@@ -915,4 +919,7 @@ def test_smagorinsky_with_zero_constant_is_lbgk_and_positive_constant_adds_visco
         amp.append(np.abs(o.macro()[1][0]).max())
     nu = (tau - 0.5) / 3.0
     assert abs(amp[0] / (0.08 * np.exp(-nu * k * k * T)) - 1.0) < 5e-3
-    assert amp[1] < (1 - 5e-4) * amp[0]                      # measured 0.9986: the eddy viscosity is small but positive
+    # C_S > 0 at the crest of the wave (zero strain) after 200 steps: only the sign of the effect shows here; the
+    # size of the eddy viscosity is pinned against eq. (9) on the wave's Fourier amplitude over 2000-4000 steps in
+    # test_oracle_pins_r2.py::test_smagorinsky_shear_wave_decay_follows_eq9
+    assert amp[1] < amp[0]
