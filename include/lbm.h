@@ -9,7 +9,7 @@
  *     (ctx == NULL: the last failure of lbm_workspace_bytes / lbm_create on this thread).
  *   - Every pointer named d_* is a DEVICE pointer, every pointer named h_* is a HOST pointer.
  *     The caller owns all memory, including the workspace: the library never allocates device
- *     memory (PyTorch allocates it; "PyTorch ... only for device memory and streams").
+ *     memory (the caller, e.g. PyTorch, allocates it and provides the stream).
  *   - Arrays are C-order [z][y][x], x fastest.  `real` is float (LBM_F32) or double
  *     (LBM_F64).  Scalar fields: real[nz][ny][nx].  Velocity: real[D][nz][ny][nx] (component
  *     planes, D = 2 for D2Q9, 3 for D3Q19).  Distributions: real[Q][nz][ny][nx] in the velocity
@@ -62,9 +62,10 @@ typedef struct lbm_ctx lbm_ctx;
 typedef struct {
     uint32_t struct_size;     /* = sizeof(lbm_params); lets the ABI grow                           */
     int32_t lattice;          /* LBM_D2Q9 | LBM_D3Q19                                              */
-    int32_t model;            /* LBM_BGK | LBM_MRT | LBM_SC2                                       */
+    int32_t model;            /* LBM_BGK | LBM_MRT | LBM_SC2 | LBM_BGK_REG | LBM_BGK_LES          */
     int32_t precision;        /* LBM_F32 | LBM_F64                                                 */
-    int32_t nx, ny, nz;       /* lattice extents, each >= 1 (nz == 1 for D2Q9), nx*ny*nz < 2^31    */
+    int32_t nx, ny, nz;       /* lattice extents, each >= 1 (nz == 1 for D2Q9), ny and nz <= 65535,
+                                 nx*ny*nz <= 2^31 - 512                                            */
     double tau[2];            /* BGK/MRT: tau[0] > 0.5.  SC2: tau[0] = tau_A, tau[1] = tau_B       */
     double rates[LBM_QMAX];   /* MRT: Q relaxation rates in the moment order of reading A5;
                                  each in [0, 2]; ignored by the other models (eq. 4)        */
@@ -73,11 +74,12 @@ typedef struct {
     int32_t sc_psi;           /* LBM_PSI_*                                                         */
     int32_t store;            /* LBM_STORE_AB (default 0) | LBM_STORE_AA                           */
     double bc_velocity[3];    /* velocity imposed on LBM_NODE_VELOCITY nodes (reading A21);
-                                 callers built against the 240-byte struct (no such field) get 0   */
+                                 each component within (-1, 1); callers built against the 240-byte
+                                 struct (no such field) get 0                                      */
     int32_t force_scheme;     /* LBM_FORCE_GUO (default 0, eq. 17) | LBM_FORCE_EDM (eq. 18); applies to
                                  the body force and to the Shan-Chen coupling force alike          */
-    int32_t reserved_;        /* keeps sizeof a multiple of 8; set to 0                            */
-    double smagorinsky_cs;    /* LBM_BGK_LES: Smagorinsky constant C_S of eq. (9) (0.1), >= 0  */
+    int32_t reserved_;        /* keeps sizeof a multiple of 8; must be 0 (LBM_EINVAL otherwise)    */
+    double smagorinsky_cs;    /* LBM_BGK_LES: Smagorinsky constant C_S of eq. (9) (0.1), in [0, 10) */
 } lbm_params;
 
 /* Static description of a lattice (Table 1; ordering = reading A2).
@@ -97,9 +99,11 @@ int lbm_workspace_bytes(const lbm_params *p, size_t *bytes);
 int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, void *cuda_stream, lbm_ctx **out);
 int lbm_destroy(lbm_ctx *ctx);
 
-/* Node types.  d_mask: uint8[nz][ny][nx] of LBM_NODE_* values.  Builds the internal link encoding (which of the Q pull sources are
- * reflected).  Must be called before lbm_init_equilibrium / lbm_set_distributions if the
- * geometry is not all-FLUID; calling it afterwards returns LBM_ESTATE. */
+/* Node types.  d_mask: uint8[nz][ny][nx] of LBM_NODE_* values.  Builds the internal link
+ * encoding (which of the Q pull sources are reflected).  Must be called before lbm_init_equilibrium /
+ * lbm_set_distributions if the geometry is not all-FLUID; calling it afterwards returns LBM_ESTATE.
+ * SYNCHRONISES the stream once: it reads back how many nodes touch a wall to pick the kernel variant
+ * (lbm_get_dispatch reports the choice), so that lbm_step never has to block. */
 int lbm_set_geometry(lbm_ctx *ctx, const uint8_t *d_mask);
 int lbm_get_geometry(lbm_ctx *ctx, uint8_t *d_mask);          /* writes LBM_NODE_* per node */
 
@@ -110,12 +114,12 @@ int lbm_init_equilibrium(lbm_ctx *ctx, int comp, const void *d_rho, const void *
 /* Advance n >= 0 time steps; each step is one fused pull-stream + moments + equilibrium +
  * collision (+ Guo source) + store pass over the lattice (Alg. 1; eqs. 1-4, 16-17);
  * LBM_SC2 runs the macro-field pass and then the coupled collide pass (eq. 10).
- * LBM_ESTATE if a component has not been initialised.  Asynchronous, except that the first call
- * after lbm_set_geometry synchronises the stream once (it reads back how many nodes are not
- * bulk fluid to pick the kernel variant).  Lattices of up to 2^20 nodes replay 50-step CUDA graphs,
- * lattices of up to 4096 nodes (single component, AB store) run all n steps in one launch of a
- * thread-block cluster that keeps the store in distributed shared memory; results are bit-identical
- * to single-step launches. */
+ * LBM_ESTATE if a component has not been initialised.  Asynchronous: never blocks the host.
+ * Lattices of up to 2^20 nodes replay 50-step CUDA graphs (captured on a private stream at the first
+ * call that needs them); single-component AB lattices of up to 4096 nodes (D2Q9: 16384) run all n steps
+ * in one launch of a thread-block cluster that keeps the store in distributed shared memory, falling
+ * back to the graph path where such a cluster cannot be scheduled; results are bit-identical to
+ * single-step launches. */
 int lbm_step(lbm_ctx *ctx, int n);
 
 /* rho = sum_i f_i, velocity v of eq. (16) (includes g/2) from the current state.
@@ -129,9 +133,9 @@ int lbm_get_distributions(lbm_ctx *ctx, int comp, void *d_f);
 int lbm_set_distributions(lbm_ctx *ctx, int comp, const void *d_f);
 
 /* Streaming index map (reading A8): d_map int64[Q][N]; map[i][x] = i' * N + x' = the slot of the
- * canonical post-collision array whose value becomes f_i(x, t+1): (i, x - e_i) if that node is
- * FLUID, else (ibar, x); -1 where x is SOLID.  Computed by the same device routine the step
- * kernels use for their gather. */
+ * canonical post-collision array whose value becomes f_i(x, t+1): (i, x - e_i) unless that node is
+ * SOLID (FLUID, WALL_FULLWAY and VELOCITY sources are pulled directly), else (ibar, x); -1 where x
+ * is SOLID.  Computed by the same device routine the step kernels use for their gather. */
 int lbm_get_stream_map(lbm_ctx *ctx, int64_t *d_map);
 
 /* Whole path with HOST buffers (what bench.py's e2e leg times): H2D of mask, rho0, u0 per
@@ -143,6 +147,27 @@ int lbm_run_host(lbm_ctx *ctx, const uint8_t *h_mask, const void *const *h_rho0,
 
 /* Time step counter since the last init/set, and number of kernels launched by this context. */
 int lbm_get_counters(const lbm_ctx *ctx, int64_t *steps, int64_t *launches);
+
+/* Which kernel variant lbm_step uses for this context (chosen from the lattice size at lbm_create and
+ * from the geometry at lbm_set_geometry).  For tests and benchmarks that must
+ * state what they measured. */
+typedef struct {
+    int32_t nodes_per_thread;        /* consecutive x-nodes per thread of the step kernels: 1, 2 or 4 */
+    int32_t index_bits;              /* 32 or 64: width of slot indices i * N + node                  */
+    int32_t graph_replay;            /* > 0: steps per replayed CUDA graph (small lattices), else 0   */
+    int32_t resident_nodes_per_cta;  /* > 0: cluster-resident path, nodes per CTA                     */
+    int32_t resident_ctas;           /* CTAs of that cluster (8 or 16), else 0                        */
+    int32_t rows_per_block;          /* > 0: row-walking kernel for obstacle-rich geometries          */
+    int32_t block_threads;           /* threads per block of the step kernels                         */
+    int32_t reserved_;
+} lbm_dispatch;
+int lbm_get_dispatch(const lbm_ctx *ctx, lbm_dispatch *out);
+
+/* Test-only tuning knobs.  Environment variables, read at lbm_create / lbm_set_geometry and honoured
+ * ONLY if LBM_TUNING=1 is set too: LBM_VEC (1|2|4 nodes per thread), LBM_IDX64 (1: 64-bit slot indices),
+ * LBM_BLOCK_X, LBM_BLOCK_THREADS (multiples of 32), LBM_ROWS (rows per block of the row-walking kernel,
+ * 0 = off), LBM_NO_GRAPH, LBM_NO_RESIDENT, LBM_RESIDENT_MAX (largest lattice of the cluster-resident
+ * path).  They select among kernels that all pass the same parity tests; they are not part of the ABI. */
 
 const char *lbm_last_error(const lbm_ctx *ctx);
 

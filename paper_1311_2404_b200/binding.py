@@ -26,7 +26,7 @@ LBM_QMAX = 19
 EXPORTS = ("lbm_lattice_info", "lbm_workspace_bytes", "lbm_create", "lbm_destroy", "lbm_set_geometry",
            "lbm_get_geometry", "lbm_init_equilibrium", "lbm_step", "lbm_macro", "lbm_get_distributions",
            "lbm_set_distributions", "lbm_get_stream_map", "lbm_run_host", "lbm_get_counters",
-           "lbm_last_error")
+           "lbm_get_dispatch", "lbm_last_error")
 
 
 class lbm_params(C.Structure):
@@ -80,6 +80,7 @@ def load():
     L.lbm_get_stream_map.argtypes = [vp, i64p]
     L.lbm_run_host.argtypes = [vp, vp, C.POINTER(vp), C.POINTER(vp), C.c_int, vp, vp]
     L.lbm_get_counters.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
+    L.lbm_get_dispatch.argtypes = [vp, C.POINTER(lbm_dispatch)]
     L.lbm_last_error.argtypes = [vp]
     L.lbm_last_error.restype = C.c_char_p
     for name in EXPORTS:
@@ -87,6 +88,11 @@ def load():
             getattr(L, name).restype = C.c_int
     _lib = L
     return L
+
+
+class lbm_dispatch(C.Structure):
+    _fields_ = [(n, C.c_int32) for n in ("nodes_per_thread", "index_bits", "graph_replay", "resident_nodes_per_cta",
+                                         "resident_ctas", "rows_per_block", "block_threads", "reserved_")]
 
 
 def make_params(lattice, model, precision, nx, ny, nz=1, tau=(1.0, 1.0), rates=None,
@@ -164,6 +170,12 @@ def lbm_get_counters(ctx):
     s, l = C.c_int64(), C.c_int64()
     _check(load().lbm_get_counters(ctx, C.byref(s), C.byref(l)), ctx)
     return s.value, l.value
+
+
+def lbm_get_dispatch(ctx) -> dict:
+    d = lbm_dispatch()
+    _check(load().lbm_get_dispatch(ctx, C.byref(d)), ctx)
+    return {n: getattr(d, n) for n, _ in lbm_dispatch._fields_ if n != "reserved_"}
 
 
 # ---- convenience wrapper: owns the torch workspace, takes/returns torch tensors ------------------
@@ -258,6 +270,9 @@ class Lbm:
 
     def counters(self):
         return lbm_get_counters(self.ctx)
+
+    def dispatch(self) -> dict:
+        return lbm_get_dispatch(self.ctx)
 
 
 def from_workload(w, device="cuda:0", **kw) -> "Lbm":

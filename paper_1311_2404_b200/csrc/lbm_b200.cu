@@ -23,7 +23,9 @@ int validate(const lbm_params *p, int *Q, int *D) {
     if (p->store != LBM_STORE_AB && p->store != LBM_STORE_AA) return fail(nullptr, LBM_EINVAL, "unknown store");
     if (p->nx < 1 || p->ny < 1 || p->nz < 1) return fail(nullptr, LBM_EINVAL, "extents must be >= 1");
     if (p->lattice == LBM_D2Q9 && p->nz != 1) return fail(nullptr, LBM_EINVAL, "D2Q9 needs nz == 1");
-    if ((double)p->nx * p->ny * p->nz >= 2147483648.0) return fail(nullptr, LBM_EINVAL, "nx*ny*nz must be < 2^31");
+    // node indices are ints and padded threads index up to one block beyond the last node
+    if ((double)p->nx * p->ny * p->nz > 2147483648.0 - 512.0) return fail(nullptr, LBM_EINVAL, "nx*ny*nz must be <= 2^31 - 512");
+    if (p->struct_size >= LBM_PARAMS_SIZE_V3 && p->reserved_ != 0) return fail(nullptr, LBM_EINVAL, "reserved_ must be 0");
     const int nt = p->model == LBM_SC2 ? 2 : 1;
     for (int s = 0; s < nt; s++)
         if (!(p->tau[s] > 0.5)) return fail(nullptr, LBM_EINVAL, "tau must be > 0.5");
@@ -78,7 +80,15 @@ const Vtbl *select_impl(const lbm_params *p) {
     return static_cast<const Vtbl *>(t);
 }
 
+// Test-only tuning knobs (include/lbm.h lists them): honoured only when LBM_TUNING=1 is set as well,
+// so that a stray variable in a user's environment cannot change the kernel selection.
+bool tuning_enabled() {
+    const char *e = getenv("LBM_TUNING");
+    return e && e[0] == '1' && e[1] == 0;
+}
+
 int env_int(const char *name, int dflt, int lo, int hi) {
+    if (!tuning_enabled()) return dflt;
     if (const char *e = getenv(name)) {
         const int v = atoi(e);
         if (v >= lo && v <= hi) return v;
@@ -111,24 +121,26 @@ int pick_vec(const lbm_params *p, double nonbulk_fraction) {
     return v;
 }
 
-// Cluster-resident path (resident_kernel): single component, AB store, and both buffers of a CTA's
-// share of the lattice within ~200 KB of shared memory with at most 2 nodes per thread.
-int pick_resident(const lbm_params *p, int Q, int64_t N) {
+// Cluster-resident path (resident_kernel): single component, AB store, one node per thread, both
+// buffers of a CTA's share of the lattice in its shared memory.  8 CTAs x 512 nodes up to 4096 nodes;
+// D2Q9 also 16 CTAs (non-portable cluster size) x 512 / 1024 nodes up to 16384 nodes (c1: 128^2).
+int pick_resident(const lbm_params *p, int Q, int64_t N, int *ctas) {
     if (p->model == LBM_SC2 || p->store != LBM_STORE_AB || env_int("LBM_NO_RESIDENT", 0, 0, 1)) return 0;
     const size_t rs = p->precision == LBM_F32 ? 4 : 8;
+    const int64_t limit = env_int("LBM_RESIDENT_MAX", Q == 9 ? 16384 : 4096, 0, 16384);
+    if (N > limit) return 0;
+    *ctas = N <= 4096 ? 8 : RESIDENT_MAX_CTAS;
     int slog2 = 5;
-    while (((int64_t)RESIDENT_CTAS << slog2) < N) slog2++;
+    while (((int64_t)*ctas << slog2) < N) slog2++;
     const size_t S = (size_t)1 << slog2;
-    if (S > (size_t)RESIDENT_THREADS * RESIDENT_NODES_PER_THREAD) return 0;
+    if (S > (Q == 9 ? 1024u : 512u)) return 0;
     if (2 * (size_t)Q * S * rs > 200 * 1024) return 0;
     return slog2;
 }
 
 int pick_block_x(int nx) {
-    if (const char *e = getenv("LBM_BLOCK_X")) {
-        const int v = atoi(e);
-        if (v >= 32 && v <= 256 && v % 32 == 0) return v;
-    }
+    const int forced = env_int("LBM_BLOCK_X", 0, 32, 256);
+    if (forced && forced % 32 == 0) return forced;
     if (nx % 256 == 0) return 256;
     if (nx % 128 == 0) return 128;
     if (nx <= 256) return (nx + 31) / 32 * 32;
@@ -192,17 +204,16 @@ LBM_API int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, voi
     c->vec = pick_vec(p, 0.0);
     c->aa = p->store == LBM_STORE_AA;
     c->idx32 = (double)Q * (double)c->g.N < 4294967296.0 && !env_int("LBM_IDX64", 0, 0, 1);
-    c->vec_pending = false;
-    c->block_threads = env_int("LBM_BLOCK_THREADS", 64, 32, 256);
+    c->rows = 0;
+    c->block_threads = env_int("LBM_BLOCK_THREADS", 64, 32, 256) / 32 * 32;
     c->vt = select_impl(p);
     c->err[0] = 0;
-    c->resident_slog2 = pick_resident(p, Q, c->g.N);
-    c->use_graph = c->resident_slog2 == 0 && c->g.N <= GRAPH_MAX_SITES && !env_int("LBM_NO_GRAPH", 0, 0, 1);
-    if (c->use_graph && cudaStreamCreateWithFlags(&c->capture_stream, cudaStreamNonBlocking) != cudaSuccess) {
-        cudaGetLastError();
-        c->use_graph = false;
-        c->capture_stream = nullptr;
-    }
+    c->resident_ctas = 8;
+    c->resident_state = 0;
+    c->resident_slog2 = pick_resident(p, Q, c->g.N, &c->resident_ctas);
+    c->no_graph = env_int("LBM_NO_GRAPH", 0, 0, 1) != 0;
+    c->use_graph = c->resident_slog2 == 0 && c->g.N <= GRAPH_MAX_SITES;
+    c->capture_stream = nullptr;  // created at the first capture
     // geometry starts all-FLUID: type = BULK, link = 0
     cudaError_t e = cudaMemsetAsync(c->ws + lay.type, 0, (size_t)c->g.N, c->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(c->ws + lay.link, 0, 4 * (size_t)c->g.N, c->stream);
@@ -228,7 +239,17 @@ LBM_API int lbm_set_geometry(lbm_ctx *c, const uint8_t *d_mask) {
     CHECK_CTX(c);
     if (!d_mask) return fail(c, LBM_EINVAL, "d_mask is NULL");
     if (c->geometry_frozen) return fail(c, LBM_ESTATE, "lbm_set_geometry after the state was initialised");
-    return c->vt->set_geometry(c, d_mask);
+    if (int rc = c->vt->set_geometry(c, d_mask)) return rc;
+    // How many nodes are not BULK decides the kernel variant (pack width; row-walking kernel for
+    // obstacle-rich geometries).  Read it back here, once per geometry, so that lbm_step never blocks.
+    unsigned nonbulk = 0;
+    cudaError_t e = cudaMemcpyAsync(&nonbulk, c->ws + c->lay.counters, sizeof nonbulk, cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) return fail(c, LBM_ECUDA, "reading the geometry counter: %s", cudaGetErrorString(e));
+    const double frac = (double)nonbulk / (double)c->g.N;
+    c->vec = pick_vec(&c->p, frac);
+    c->rows = env_int("LBM_ROWS", frac >= 0.2 ? 2 : 0, 0, 65535);
+    return LBM_OK;
 }
 
 LBM_API int lbm_get_geometry(lbm_ctx *c, uint8_t *d_mask) {
@@ -272,19 +293,17 @@ LBM_API int lbm_step(lbm_ctx *c, int n) {
     CHECK_CTX(c);
     if (n < 0) return fail(c, LBM_EINVAL, "n < 0");
     if (int rc = check_state(c)) return rc;
-    if (c->vec_pending && n > 0) {  // once per geometry: how many nodes are not BULK decides the pack width
-        unsigned nonbulk = 0;
-        cudaError_t e = cudaMemcpyAsync(&nonbulk, c->ws + c->lay.counters, sizeof nonbulk, cudaMemcpyDeviceToHost, c->stream);
-        if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
-        if (e != cudaSuccess) return fail(c, LBM_ECUDA, "reading the geometry counter: %s", cudaGetErrorString(e));
-        c->vec = pick_vec(&c->p, (double)nonbulk / (double)c->g.N);
-        c->eager_links = env_int("LBM_EAGER_LINKS", (double)nonbulk / (double)c->g.N >= 0.2 ? 1 : 0, 0, 1);
-        c->vec_pending = false;
-    }
-    while (c->use_graph && n >= GRAPH_STEPS) {
+    while (c->use_graph && !c->no_graph && n >= GRAPH_STEPS) {
         cudaGraphExec_t &exec = c->graph[c->cur];
         if (!exec) {  // capture GRAPH_STEPS ordinary step launches; nothing executes during capture
+            if (!c->capture_stream && cudaStreamCreateWithFlags(&c->capture_stream, cudaStreamNonBlocking) != cudaSuccess) {
+                cudaGetLastError();
+                c->capture_stream = nullptr;
+                c->no_graph = true;  // no private stream to capture on: plain launches
+                break;
+            }
             const int64_t steps0 = c->steps, launches0 = c->launches;
+            const int cur0 = c->cur;
             const cudaStream_t user = c->stream;
             cudaGraph_t g = nullptr;
             cudaError_t e = cudaStreamBeginCapture(c->capture_stream, cudaStreamCaptureModeThreadLocal);
@@ -296,6 +315,7 @@ LBM_API int lbm_step(lbm_ctx *c, int n) {
             c->graph_launches = c->launches - launches0;
             c->steps = steps0;
             c->launches = launches0;
+            c->cur = cur0;  // GRAPH_STEPS is even; a capture that failed half-way must not leave the parity flipped
             if (rc) { if (g) cudaGraphDestroy(g); return rc; }
             if (e == cudaSuccess) e = cudaGraphInstantiate(&exec, g, 0);
             if (g) cudaGraphDestroy(g);
@@ -373,6 +393,19 @@ LBM_API int lbm_get_counters(const lbm_ctx *c, int64_t *steps, int64_t *launches
     CHECK_CTX(c);
     if (steps) *steps = c->steps;
     if (launches) *launches = c->launches;
+    return LBM_OK;
+}
+
+LBM_API int lbm_get_dispatch(const lbm_ctx *c, lbm_dispatch *out) {
+    CHECK_CTX(c);
+    if (!out) return LBM_EINVAL;
+    out->nodes_per_thread = c->p.model == LBM_SC2 ? ((c->vec >= 2 && !c->aa && c->rs == 4) ? 2 : 1) : c->vec;
+    out->index_bits = c->idx32 ? 32 : 64;
+    out->graph_replay = (c->use_graph && !c->no_graph) ? GRAPH_STEPS : 0;
+    out->resident_nodes_per_cta = (c->resident_slog2 > 0 && c->resident_state >= 0) ? 1 << c->resident_slog2 : 0;
+    out->resident_ctas = out->resident_nodes_per_cta ? c->resident_ctas : 0;
+    out->rows_per_block = (c->rows > 0 && !c->aa && c->p.model != LBM_SC2 && c->idx32 && c->vec <= 2) ? c->rows : 0;
+    out->block_threads = c->block_threads;
     return LBM_OK;
 }
 

@@ -39,11 +39,12 @@ struct lbm_ctx {
     int cur;  // which of the two buffers holds the current state (AB)
     bool inited[2];
     bool geometry_frozen;
-    bool vec_pending;   // geometry changed: re-pick `vec` from the non-bulk node count at the next step
     int64_t steps, launches;
     bool aa;            // LBM_STORE_AA: one buffer, `cur` is the step parity (0 even, 1 odd)
     int resident_slog2; // > 0: the AB store fits one cluster's shared memory; log2 of nodes per CTA
-    int eager_links;    // fetch link words with the types (set when >= 20 % of the nodes are not BULK)
+    int resident_ctas;  // CTAs of that cluster (8, or 16 = non-portable size)
+    int resident_state; // 0 not probed yet, 1 launchable, -1 not launchable here (fall back for good)
+    int rows;           // > 0: obstacle-rich geometry (>= 20 % of the nodes not BULK): step_rows_kernel, rows per block
     bool idx32;         // Q * N < 2^32: slot numbers fit 32 bits (cheaper address arithmetic)
     int block_x;        // one-node-per-thread kernels: 1-D block along x
     int vec;            // nodes per thread of the step kernels (1, 2 or 4 consecutive x)
@@ -53,6 +54,7 @@ struct lbm_ctx {
     // parity into a CUDA graph and replayed; capture happens on a private stream because the
     // caller's stream may be the legacy default stream, which cannot be captured.
     bool use_graph;
+    bool no_graph;      // graph replay switched off (tuning knob, or no capture stream could be created)
     cudaStream_t capture_stream;
     cudaGraphExec_t graph[2];
     int64_t graph_launches;  // kernels inside one graph
@@ -144,7 +146,6 @@ template <class L, typename T> struct Impl {
         unsigned *cnt = at<unsigned>(c, c->lay.counters);
         if (cudaMemsetAsync(cnt, 0, sizeof(unsigned), c->stream) != cudaSuccess) return fail(c, LBM_ECUDA, "cudaMemsetAsync(counters)");
         build_links_kernel<L><<<grid_of(c), c->block_x, 0, c->stream>>>(c->g, d_mask, type(c), link(c), cnt);
-        c->vec_pending = true;
         drop_graphs(c);
         return check_launch(c, "build_links_kernel");
     }

@@ -120,6 +120,7 @@ __global__ void build_links_kernel(Geom g, const uint8_t *__restrict__ mask, uin
         for (int i = 1; i < L::Q; i++)
             if (mask_is_solid(mask[n + shift<L>(i, -1, o)])) w |= 1u << i;
         t = (w ? NODE_LINKS : NODE_BULK) | (m == MASK_FULLWAY ? NODE_FULLWAY : 0) | (m == MASK_VELOCITY ? NODE_VELOCITY : 0);
+        w |= (m == MASK_FULLWAY ? LINK_FULLWAY : 0u) | (m == MASK_VELOCITY ? LINK_VELOCITY : 0u);
     }
     link[n] = w;
     type[n] = t;
@@ -308,51 +309,99 @@ __device__ __forceinline__ void update_span(T (&h)[V][L::Q], uint32_t types, con
     }
 }
 
-// Link words of a pack with one vector load (geometries where most nodes are BOUNDARY: the words
-// are then fetched together with the types and the pull, not after the types have arrived).
-template <int V> __device__ __forceinline__ void load_links(const uint32_t *__restrict__ link, int n0, uint32_t (&w)[V]) {
-    if (V == 4) { const uint4 v = __ldg(reinterpret_cast<const uint4 *>(link + n0)); w[0] = v.x; w[1] = v.y; w[2] = v.z; w[V - 1] = v.w; }
-    else if (V == 2) { const uint2 v = __ldg(reinterpret_cast<const uint2 *>(link + n0)); w[0] = v.x; w[V - 1] = v.y; }
-    else w[0] = __ldg(link + n0);
-}
-
-template <class L, typename T, int V, typename I>
-__device__ __forceinline__ void pull_reflected_span_eager(const T *__restrict__ src, int64_t N, int n0, uint32_t types,
-                                                          const uint32_t (&w)[V], T (&h)[V][L::Q]) {
-    if (types & PACK_LINKS) {
-#pragma unroll
-        for (int k = 0; k < V; k++)
-            if (((types >> (8 * k)) & 0xffu) & NODE_LINKS) pull_reflected<L, T, I>(src, n0 + k, N, w[k], h[k]);
-    }
-}
-
 // ---- the fused step: pull-stream + moments + equilibrium + collision (+ Guo) + store ---------
 // Rows a1-a8 of DESIGN.md.  All loads of the pack are issued before first use (bytes in flight).
 template <class L, typename T, int V, typename I, int MODEL, int FORCE>
 __global__ void __launch_bounds__(256)
 step_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restrict__ link,
-            const T *__restrict__ src, T *__restrict__ dst, Relax<T> rp, int eager_links) {
+            const T *__restrict__ src, T *__restrict__ dst, Relax<T> rp) {
     Span s;
     if (!thread_span<V>(g, s)) return;
     const int n0 = s.row + s.x0;
     const uint32_t types = load_types<V>(type, n0);
+    if (all_solid<V>(types)) return;
     T h[V][L::Q];
-    if (eager_links) {
-        // obstacle-rich geometry (c3: 57 % BOUNDARY nodes): types, link words and the pull are
-        // issued together, the reflected links follow one memory round trip later (ncu showed
-        // half of the stalls of this kernel on the type -> link -> fix-up dependency chain)
-        uint32_t w[V];
-        load_links<V>(link, n0, w);
-        gather_span<L, T, V, I>(src, g.N, s, h);
-        if (all_solid<V>(types)) return;
-        pull_reflected_span_eager<L, T, V, I>(src, g.N, n0, types, w, h);
-    } else {
-        if (all_solid<V>(types)) return;
-        gather_span<L, T, V, I>(src, g.N, s, h);
-        pull_reflected_span<L, T, V, I>(src, g.N, n0, types, link, h);
-    }
+    gather_span<L, T, V, I>(src, g.N, s, h);
+    pull_reflected_span<L, T, V, I>(src, g.N, n0, types, link, h);
     update_span<L, T, V, MODEL, FORCE>(h, types, rp);
     store_span<L, T, V, I>(dst, g.N, s.row + s.x0, h);
+}
+
+// ---- the fused step for obstacle-rich geometries (c3: 57 % of the fluid nodes touch a SOLID) ---
+// step_kernel re-pulls reflected links after the link word has arrived: a second, dependent memory
+// round trip per thread, which at 80 registers / 24 warps per SM left it latency-bound (r01e: 68 % of
+// the DRAM peak, 74 % of the stall samples on long_scoreboard).  Here a thread walks `rows`
+// consecutive y-rows of one x-span and fetches the link words of row y+1 while row y is in flight,
+// so that when a row starts its link words are already in registers and EVERY population load --
+// pulled from (i, x - e_i) or, for a reflected link, from the node's own (ibar, x) -- is issued in
+// one batch with the address selected per lane: one round trip, no fix-up pass.  Loads are scalar
+// per node (a lane's source depends on its own link bit), the arithmetic and the aligned vector
+// stores stay V nodes wide.  Only the link array is read (it repeats the node types, lbm_lattice.cuh).
+template <class L, int V> __device__ __forceinline__ uint32_t types_of_links(const uint32_t (&w)[V]) {
+    uint32_t types = 0;
+#pragma unroll
+    for (int k = 0; k < V; k++) {
+        const uint32_t t = (w[k] >> 31) | ((w[k] & LINK_DIRECTIONS) ? NODE_LINKS : 0u) |
+                           ((w[k] & LINK_FULLWAY) ? NODE_FULLWAY : 0u) | ((w[k] & LINK_VELOCITY) ? NODE_VELOCITY : 0u);
+        types |= t << (8 * k);
+    }
+    return types;
+}
+
+template <class L, typename T, int V, typename I>
+__device__ __forceinline__ void gather_selected_span(const T *__restrict__ src, int64_t N, const Span &s,
+                                                     const uint32_t (&w)[V], T (&h)[V][L::Q]) {
+#pragma unroll
+    for (int i = 0; i < L::Q; i++) {
+        const int r = s.row + shift_yz<L>(i, -1, s.o);
+        const I plane = I(i) * I(N), own = I(L::opp(i)) * I(N) + I(s.row + s.x0);
+#pragma unroll
+        for (int k = 0; k < V; k++) {
+            const int xs = L::ex(i) == 0 ? s.x0 + k
+                         : L::ex(i) == 1 ? (k == 0 ? s.xm : s.x0 + k - 1)
+                                         : (k == V - 1 ? s.xp : s.x0 + k + 1);
+            const I idx = (i > 0 && reflected(w[k], i)) ? own + I(k) : plane + I(r + xs);
+            h[k][i] = __ldg(src + idx);
+        }
+    }
+}
+
+template <int V> __device__ __forceinline__ void load_links(const uint32_t *__restrict__ link, int n0, uint32_t (&w)[V]) {
+    if (V == 4) { const uint4 v = __ldg(reinterpret_cast<const uint4 *>(link + n0)); w[0] = v.x; w[1 % V] = v.y; w[2 % V] = v.z; w[V - 1] = v.w; }
+    else if (V == 2) { const uint2 v = __ldg(reinterpret_cast<const uint2 *>(link + n0)); w[0] = v.x; w[V - 1] = v.y; }
+    else w[0] = __ldg(link + n0);
+}
+
+// 64-thread blocks; fp32: 12 blocks per SM (80 registers, 24 warps), fp64: 6 (168 registers), by measurement
+// on c3 (fp32 at 96 registers / 20 warps: the same; at 64 registers / 32 warps: -10 %, spills).
+template <class L, typename T, int V, typename I, int MODEL, int FORCE>
+__global__ void __launch_bounds__(64, sizeof(T) == 4 ? 12 : 6)
+step_rows_kernel(Geom g, const uint32_t *__restrict__ link, const T *__restrict__ src, T *__restrict__ dst,
+                 Relax<T> rp, int rows) {
+    Span s;
+    s.x0 = (blockIdx.x * blockDim.x + threadIdx.x) * V;
+    if (s.x0 >= g.nx) return;
+    s.z = blockIdx.z;
+    s.xm = (s.x0 == 0) ? g.nx - 1 : s.x0 - 1;
+    s.xp = (s.x0 + V == g.nx) ? 0 : s.x0 + V;
+    const int y0 = blockIdx.y * rows, y1 = min(y0 + rows, g.ny);
+    uint32_t wn[V];
+    load_links<V>(link, (s.z * g.ny + y0) * g.nx + s.x0, wn);
+    for (int y = y0; y < y1; y++) {
+        uint32_t w[V];
+#pragma unroll
+        for (int k = 0; k < V; k++) w[k] = wn[k];
+        s.y = y;
+        s.row = (s.z * g.ny + y) * g.nx;
+        s.o = neighbours(g, 1, y, s.z);
+        if (y + 1 < y1) load_links<V>(link, s.row + g.nx + s.x0, wn);  // next row: in flight during this row's pull
+        const uint32_t types = types_of_links<L, V>(w);
+        if (all_solid<V>(types)) continue;
+        T h[V][L::Q];
+        gather_selected_span<L, T, V, I>(src, g.N, s, w, h);
+        update_span<L, T, V, MODEL, FORCE>(h, types, rp);
+        store_span<L, T, V, I>(dst, g.N, s.row + s.x0, h);
+    }
 }
 
 // ---- canonical <-> internal conversions (off the hot loop; reading A9) ----------------------
@@ -438,21 +487,32 @@ __global__ void macro_kernel(Geom g, const uint8_t *__restrict__ type, const uin
     }
 }
 
-// ---- small lattices: the whole AB store resident in the shared memory of one 8-CTA cluster ---
+// ---- small lattices: the whole AB store resident in the shared memory of one thread-block cluster ---
 // The paper's saturation plot is the launch-bound regime: a 128^2 D2Q9 lattice is 0.6 MB
-// per buffer and one step of it takes 2 us however it is launched.  For lattices of up to 4096
-// nodes CTA r of a thread-block
-// cluster keeps slots [Q][S] of nodes [r S, (r+1) S) of both buffers in its shared memory; a pull
-// from a node owned by another CTA is a distributed-shared-memory load (cluster.map_shared_rank),
-// steps are separated by cluster.sync(), and global memory is touched only before the first and
-// after the last step of an lbm_step(n) call.  Same arithmetic and streaming rule as step_kernel.
-// Measured (D2Q9 LBGK fp32, us per step, resident vs 50-step graphs): 32^2 0.66 vs 2.01, 64^2 1.05 vs
-// 2.05, 96^2 3.22 vs 2.05, 128^2 3.23 vs 2.09: eight SMs run out of issue slots beyond ~4096 nodes,
-// so the path is used up to 512 nodes per CTA, one node per thread.
-constexpr int RESIDENT_CTAS = 8, RESIDENT_THREADS = 512, RESIDENT_NODES_PER_THREAD = 1;
+// per buffer and one step of it takes ~2 us however it is launched.  Here CTA r of a cluster of 8
+// (portable) or 16 (non-portable size, D2Q9 only) CTAs keeps slots [Q][S] of nodes [r S, (r+1) S) of
+// both buffers in its shared memory, one node per thread; a pull from a node owned by another CTA
+// is a distributed-shared-memory load, steps are separated by cluster.sync(), and global memory is
+// touched only before the first and after the last step of an lbm_step(n) call.  A node's Q source
+// addresses (shared::cluster window, reflected links resolved) never change, so they are computed
+// once and kept in registers.  Same arithmetic and streaming rule as step_kernel: bit-identical.
+constexpr int RESIDENT_MAX_CTAS = 16;
 
-template <class L, typename T, int MODEL, int FORCE>
-__global__ void __cluster_dims__(RESIDENT_CTAS, 1, 1) __launch_bounds__(RESIDENT_THREADS)
+__device__ __forceinline__ uint32_t dsmem_address(const void *smem_ptr, unsigned cta_rank) {
+    uint32_t local = (uint32_t)__cvta_generic_to_shared(smem_ptr), remote;
+    asm("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(local), "r"(cta_rank));
+    return remote;
+}
+template <typename T> __device__ __forceinline__ T dsmem_load(uint32_t addr);
+template <> __device__ __forceinline__ float dsmem_load<float>(uint32_t addr) {
+    float v; asm volatile("ld.shared::cluster.f32 %0, [%1];" : "=f"(v) : "r"(addr) : "memory"); return v;
+}
+template <> __device__ __forceinline__ double dsmem_load<double>(uint32_t addr) {
+    double v; asm volatile("ld.shared::cluster.f64 %0, [%1];" : "=d"(v) : "r"(addr) : "memory"); return v;
+}
+
+template <class L, typename T, int MODEL, int FORCE, int THREADS>
+__global__ void __launch_bounds__(THREADS)
 resident_kernel(Geom g, int s_log2, const uint8_t *__restrict__ type, const uint32_t *__restrict__ link,
                 const T *src, T *dst, Relax<T> rp, int nsteps) {
     extern __shared__ __align__(16) unsigned char resident_smem[];
@@ -462,53 +522,46 @@ resident_kernel(Geom g, int s_log2, const uint8_t *__restrict__ type, const uint
     const int S = 1 << s_log2, mask = S - 1, N = (int)g.N;
     const int base = (int)cluster.block_rank() * S;
     const int tid = threadIdx.x;
-    for (int idx = tid; idx < L::Q * S; idx += RESIDENT_THREADS) {
+    for (int idx = tid; idx < L::Q * S; idx += THREADS) {
         const int i = idx >> s_log2, n = base + (idx & mask);
         buf[idx] = n < N ? src[(int64_t)i * N + n] : T(0);
     }
-    // per-thread nodes: type, link word and neighbour offsets stay in registers for all steps
-    uint32_t t[RESIDENT_NODES_PER_THREAD], w[RESIDENT_NODES_PER_THREAD];
-    Nbr o[RESIDENT_NODES_PER_THREAD];
+    // this thread's node: type and the Q source addresses (buffer 0) stay in registers for all steps
+    const int n = base + tid;
+    uint32_t t = NODE_SOLID;  // threads beyond the lattice or beyond S do nothing
+    uint32_t from[L::Q];
+    if (tid < S && n < N) {
+        t = type[n];
+        const uint32_t w = (t & NODE_LINKS) ? link[n] : 0u;
+        const int x = n % g.nx, y = (n / g.nx) % g.ny, z = n / (g.nx * g.ny);
+        const Nbr o = neighbours(g, x, y, z);
 #pragma unroll
-    for (int k = 0; k < RESIDENT_NODES_PER_THREAD; k++) {
-        const int l = tid + k * RESIDENT_THREADS, n = base + l;
-        t[k] = NODE_SOLID;  // nodes beyond the lattice or beyond S do nothing
-        w[k] = 0;
-        o[k] = Nbr{0, 0, 0, 0, 0, 0};
-        if (l < S && n < N) {
-            t[k] = type[n];
-            w[k] = (t[k] & NODE_LINKS) ? link[n] : 0u;
-            const int x = n % g.nx, y = (n / g.nx) % g.ny, z = n / (g.nx * g.ny);
-            o[k] = neighbours(g, x, y, z);
+        for (int i = 0; i < L::Q; i++) {
+            const bool refl = reflected(w, i);
+            const int m = refl ? n : n + shift<L>(i, -1, o);  // source node
+            const int plane = refl ? L::opp(i) : i;
+            from[i] = dsmem_address(buf + plane * S + (m & mask), (unsigned)(m >> s_log2));
         }
     }
     cluster.sync();
+    const uint32_t flip = (uint32_t)(L::Q * S * sizeof(T));  // byte distance between the two buffers
     int cur = 0;
     for (int step = 0; step < nsteps; step++) {
-        T *A = buf + cur * L::Q * S, *B = buf + (cur ^ 1) * L::Q * S;
-#pragma unroll
-        for (int k = 0; k < RESIDENT_NODES_PER_THREAD; k++) {
-            if (t[k] & NODE_SOLID) continue;
-            const int l = tid + k * RESIDENT_THREADS, n = base + l;
+        if (!(t & NODE_SOLID)) {
             T h[L::Q];
 #pragma unroll
-            for (int i = 0; i < L::Q; i++) {
-                const bool refl = reflected(w[k], i);
-                const int m = refl ? n : n + shift<L>(i, -1, o[k]);  // source node
-                const int plane = refl ? L::opp(i) : i;
-                const T *owner = cluster.map_shared_rank(A, m >> s_log2);
-                h[i] = owner[plane * S + (m & mask)];
-            }
-            update_typed<L, T, MODEL, FORCE>(h, t[k], rp);
+            for (int i = 0; i < L::Q; i++) h[i] = dsmem_load<T>(from[i] + (cur ? flip : 0u));
+            update_typed<L, T, MODEL, FORCE>(h, t, rp);
+            T *B = buf + (cur ^ 1) * L::Q * S;
 #pragma unroll
-            for (int i = 0; i < L::Q; i++) B[i * S + l] = h[i];
+            for (int i = 0; i < L::Q; i++) B[i * S + tid] = h[i];
         }
         cluster.sync();  // every CTA has written step t+1 before anyone pulls from it
         cur ^= 1;
     }
-    for (int idx = tid; idx < L::Q * S; idx += RESIDENT_THREADS) {
-        const int i = idx >> s_log2, n = base + (idx & mask);
-        if (n < N) dst[(int64_t)i * N + n] = buf[cur * L::Q * S + idx];
+    for (int idx = tid; idx < L::Q * S; idx += THREADS) {
+        const int i = idx >> s_log2, m = base + (idx & mask);
+        if (m < N) dst[(int64_t)i * N + m] = buf[cur * L::Q * S + idx];
     }
 }
 

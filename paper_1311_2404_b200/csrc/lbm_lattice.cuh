@@ -55,5 +55,9 @@ struct D3Q19 {
 // Bit 31 of a node's link word marks the node itself SOLID; bit i (< Q) marks the pull source
 // x - e_i SOLID, i.e. population i arrives by half-way bounce-back (reading A8).
 constexpr uint32_t LINK_SELF_SOLID = 0x80000000u;
+// Bits 30 / 29 repeat the node's WALL_FULLWAY / VELOCITY type, so that the kernel for obstacle-rich
+// geometries (step_rows_kernel) needs the link word only, not the type byte as well.
+constexpr uint32_t LINK_FULLWAY = 0x40000000u, LINK_VELOCITY = 0x20000000u;
+constexpr uint32_t LINK_DIRECTIONS = 0x000ffffeu;  // bits 1 .. 19: "some pull source is SOLID"
 
 }  // namespace lbm

@@ -29,8 +29,21 @@ template <class L, typename T> struct Steps {
             }
             return LBM_OK;
         }
+        if constexpr (V <= 2 && sizeof(I) == 4) {
+            if (c->rows > 0) {  // obstacle-rich geometry: row-walking kernel, link words one row ahead
+                const int nxv = c->g.nx / V, bx = nxv > 32 ? 64 : 32;
+                const dim3 grid((nxv + bx - 1) / bx, (c->g.ny + c->rows - 1) / c->rows, c->g.nz);
+                for (int t = 0; t < n; t++) {
+                    step_rows_kernel<L, T, V, I, MODEL, FORCE><<<grid, bx, 0, c->stream>>>(c->g, link(c), src(c, 0), dst(c, 0), rp, c->rows);
+                    if (int rc = check_launch(c, "step_rows_kernel")) return rc;
+                    c->cur ^= 1;
+                    c->steps++;
+                }
+                return LBM_OK;
+            }
+        }
         for (int t = 0; t < n; t++) {
-            step_kernel<L, T, V, I, MODEL, FORCE><<<l.grid, l.block, 0, c->stream>>>(c->g, type(c), link(c), src(c, 0), dst(c, 0), rp, c->eager_links);
+            step_kernel<L, T, V, I, MODEL, FORCE><<<l.grid, l.block, 0, c->stream>>>(c->g, type(c), link(c), src(c, 0), dst(c, 0), rp);
             if (int rc = check_launch(c, "step_kernel")) return rc;
             c->cur ^= 1;
             c->steps++;
@@ -38,23 +51,57 @@ template <class L, typename T> struct Steps {
         return LBM_OK;
     }
 
-    // Whole lbm_step(n) in one launch for lattices that fit the shared memory of an 8-CTA cluster.
-    template <int MODEL, int FORCE> static int step_resident(lbm_ctx *c, int n, const Relax<T> &rp) {
-        auto kernel = resident_kernel<L, T, MODEL, FORCE>;
+    // Whole lbm_step(n) in one launch for lattices that fit the shared memory of one thread-block cluster.
+    // The first call probes the launch (shared-memory opt-in, non-portable cluster size, at least one
+    // co-schedulable cluster: a MIG/MPS slice may have too few SMs); if it cannot run, the context falls
+    // back to the ordinary step kernels with graph replay for good.
+    template <int MODEL, int FORCE, int THREADS> static int launch_resident(lbm_ctx *c, int n, const Relax<T> &rp, bool *unavailable) {
+        auto kernel = resident_kernel<L, T, MODEL, FORCE, THREADS>;
         const size_t smem = 2 * (size_t)L::Q * ((size_t)1 << c->resident_slog2) * sizeof(T);
-        cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return fail(c, LBM_ECUDA, "cudaFuncSetAttribute(resident_kernel): %s", cudaGetErrorString(e));
+        cudaLaunchConfig_t cfg = {};
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = c->resident_ctas; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+        cfg.gridDim = dim3(c->resident_ctas); cfg.blockDim = dim3(THREADS); cfg.dynamicSmemBytes = smem;
+        cfg.stream = c->stream; cfg.attrs = attr; cfg.numAttrs = 1;
+        if (c->resident_state == 0) {
+            int clusters = 0;
+            cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e == cudaSuccess && c->resident_ctas > 8) e = cudaFuncSetAttribute(kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+            if (e == cudaSuccess) e = cudaOccupancyMaxActiveClusters(&clusters, kernel, &cfg);
+            if (e != cudaSuccess || clusters < 1) {
+                cudaGetLastError();
+                c->resident_state = -1;
+                *unavailable = true;
+                return LBM_OK;
+            }
+            c->resident_state = 1;
+        }
         const int after = c->cur ^ (n & 1);
-        kernel<<<RESIDENT_CTAS, RESIDENT_THREADS, smem, c->stream>>>(c->g, c->resident_slog2, type(c), link(c), src(c, 0),
-                                                                      at<T>(c, c->lay.store[0][after]), rp, n);
+        cudaError_t e = cudaLaunchKernelEx(&cfg, kernel, c->g, c->resident_slog2, (const uint8_t *)type(c), (const uint32_t *)link(c),
+                                           src(c, 0), at<T>(c, c->lay.store[0][after]), rp, n);
+        if (e != cudaSuccess) return fail(c, LBM_ECUDA, "resident_kernel: %s", cudaGetErrorString(e));
         if (int rc = check_launch(c, "resident_kernel")) return rc;
         c->cur = after;
         c->steps += n;
         return LBM_OK;
     }
 
+    template <int MODEL, int FORCE> static int step_resident(lbm_ctx *c, int n, const Relax<T> &rp, bool *unavailable) {
+        if constexpr (L::Q == 9) {
+            if (c->resident_slog2 == 10) return launch_resident<MODEL, FORCE, 1024>(c, n, rp, unavailable);
+        }
+        return launch_resident<MODEL, FORCE, 512>(c, n, rp, unavailable);
+    }
+
     template <int MODEL, int FORCE> static int step_single(lbm_ctx *c, int n, const Relax<T> &rp) {
-        if (c->resident_slog2 > 0 && n >= 2 && !c->aa) return step_resident<MODEL, FORCE>(c, n, rp);
+        if (c->resident_slog2 > 0 && c->resident_state >= 0 && n >= 2 && !c->aa) {
+            bool unavailable = false;
+            const int rc = step_resident<MODEL, FORCE>(c, n, rp, &unavailable);
+            if (!unavailable) return rc;
+            c->resident_slog2 = 0;  // fall through to the step kernels, graphs from the next call on
+            c->use_graph = c->g.N <= GRAPH_MAX_SITES;
+        }
         if constexpr (sizeof(T) == 4) {
             if (c->vec == 4) return step_single_v<4, MODEL, FORCE>(c, n, rp);
         }

@@ -93,14 +93,15 @@ def test_set_get_distributions_round_trip_bit_exact(B):
 def test_graph_replay_is_bit_identical_to_single_launches(B, cfg):
     """Small lattices replay 50-step CUDA graphs (launch-bound regime): step(120) must give
     exactly the bits of 120 x step(1), which never reaches the graph threshold."""
-    # 96^2 = 9216 nodes: above the cluster-resident limit (4096), below the graph limit (2^20)
-    w = W.c1_taylor_green(96) if cfg == "c1" else W.c5_shan_chen(24, 20, 16)
+    # 160^2 = 25600 nodes: above the cluster-resident limit (D2Q9: 16384), below the graph limit (2^20)
+    w = W.c1_taylor_green(160) if cfg == "c1" else W.c5_shan_chen(24, 20, 16)
     out = []
     for chunks in ([120], [1] * 120, [50, 7, 63]):
         sim = B.from_workload(w)
         sim.set_geometry(w.mask)
         for s in range(w.ncomp):
             sim.init_equilibrium(w.rho[s], w.u[s], comp=s)
+        assert sim.dispatch()["graph_replay"] == 50 and sim.dispatch()["resident_nodes_per_cta"] == 0
         for n in chunks:
             sim.step(n)
         assert sim.counters()[0] == 120
@@ -181,25 +182,30 @@ def test_full_size_sampled_against_oracle(B, orc, cfg, n):
         assert abs(m1 - m0[s]) <= (2e-7 if w.precision == W.F32 else 1e-13) * m0[s]
 
 
-@pytest.mark.parametrize("lattice,shape,model", [(W.D2Q9, (64, 64, 1), W.BGK), (W.D2Q9, (50, 37, 1), W.MRT),
-                                                 (W.D3Q19, (16, 16, 16), W.BGK), (W.D3Q19, (13, 9, 7), W.LES)])
-def test_cluster_resident_path_matches_single_launches_and_oracle(B, orc, lattice, shape, model):
-    """Lattices of up to 4096 nodes run lbm_step(n) as ONE launch of a thread-block cluster that keeps
-    both buffers in distributed shared memory: must equal n single-step launches bit for bit (same
-    arithmetic, same streaming rule) and the oracle within tolerance; all node types included."""
+@pytest.mark.parametrize("lattice,shape,model,ctas", [
+    (W.D2Q9, (64, 64, 1), W.BGK, 8), (W.D2Q9, (50, 37, 1), W.MRT, 8), (W.D3Q19, (16, 16, 16), W.BGK, 8),
+    (W.D3Q19, (13, 9, 7), W.LES, 8), (W.D2Q9, (128, 128, 1), W.BGK, 16), (W.D2Q9, (96, 70, 1), W.MRT, 16),
+    (W.D2Q9, (101, 150, 1), W.REG, 16)])
+def test_cluster_resident_path_matches_single_launches_and_oracle(B, orc, lattice, shape, model, ctas):
+    """Lattices of up to 4096 nodes (D2Q9: 16384, in a 16-CTA cluster) run lbm_step(n) as ONE launch of a
+    thread-block cluster that keeps both buffers in distributed shared memory: must equal n single-step
+    launches bit for bit (same arithmetic, same streaming rule) and the oracle within tolerance; all
+    node types included."""
     import torch
     nx, ny, nz = shape
     mask, rho, u = W.random_types(lattice, nx, ny, nz, seed=91)
     D = 2 if lattice == W.D2Q9 else 3
     rates = (W.mrt_rates_d3q19(0.7) if lattice == W.D3Q19 else W.mrt_rates_d2q9(0.7)) if model == W.MRT else None
     w = W.Workload("resident", lattice, model, W.F64, nx, ny, nz, (0.7, 0.7), 60, rates=rates, smagorinsky_cs=0.15,
-                   force=(1e-5, -2e-5, 3e-5 if D == 3 else 0.0), bc_velocity=(0.02, -0.01, 0.0))
+                   force=(1e-5, -2e-5, 3e-5 if D == 3 else 0.0), bc_velocity=(0.02, -0.01, 0.0),
+                   force_scheme=W.FORCE_EDM if model == W.REG else W.FORCE_GUO)
     w.mask, w.rho, w.u = mask, rho, u
     out = []
     for chunks in ([60], [1] * 60, [7, 53]):
         sim = B.from_workload(w)
         sim.set_geometry(w.mask)
         sim.init_equilibrium(w.rho[0], w.u[0])
+        assert sim.dispatch()["resident_ctas"] == ctas and sim.dispatch()["graph_replay"] == 0
         l0 = sim.counters()[1]
         for n in chunks:
             sim.step(n)
@@ -219,10 +225,11 @@ def test_cluster_resident_path_matches_single_launches_and_oracle(B, orc, lattic
 
 def test_runs_on_a_caller_stream(B, orc):
     """All work goes to the cudaStream_t given to lbm_create (lbm.h): a non-default torch stream,
-    including the graph-replay path (96^2 D2Q9) and a full-kernel path (40 x 24 x 12 D3Q19)."""
+    including the cluster-resident path (96^2 D2Q9), the graph-replay path (160^2) and a full-kernel path
+    (40 x 24 x 12 D3Q19)."""
     import torch
     side = torch.cuda.Stream()
-    for w in (W.c1_taylor_green(96), W.c2_channel(40, 24, 12)):
+    for w in (W.c1_taylor_green(96), W.c1_taylor_green(160), W.c2_channel(40, 24, 12)):
         ref = orc.Oracle(**w.params())
         ref.set_geometry(w.mask)
         ref.init_equilibrium(w.rho[0], w.u[0])

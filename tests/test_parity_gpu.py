@@ -87,6 +87,57 @@ def test_c5_shan_chen(B, orc, shape, precision):
     check_parity(B, orc, W.c5_shan_chen(*shape, precision=precision))
 
 
+# ---- the five recipes at sizes where the TIMED kernels are the default dispatch ---------------------
+# Below 2^20 sites lbm_create narrows the packs and replays CUDA graphs, so the cases above never run
+# step_kernel<V = 4>, step_rows_kernel or the plain launch loop unless forced.  128 x 96 x 96 = 1 179 648
+# sites is above that limit: no environment override, lbm_get_dispatch states which variant ran, every
+# non-SOLID slot is compared after 100 steps (north_star's tolerance clause; P:498 benchmarks at 254^3
+# because small boxes are another regime).
+BIG = (128, 96, 96)
+
+
+def check_big(B, orc, w, want, steps=100):
+    sim, ref = make_pair(B, orc, w)
+    d = sim.dispatch()
+    assert d["graph_replay"] == 0 and d["resident_nodes_per_cta"] == 0 and d["index_bits"] == 32, d
+    for k, v in want.items():
+        assert d[k] == v, (k, d)
+    sim.step(steps)
+    ref.step(steps)
+    errs = [max_err(sim, ref, w, s) for s in range(w.ncomp)]
+    print("max |f_gpu - f_oracle| after %d steps, %s %dx%dx%d, dispatch %s: %s" % (steps, w.name, w.nx, w.ny, w.nz, d, errs))
+    assert max(errs) <= TOL[w.precision], errs
+    sim.close()
+
+
+def test_big_c2_default_dispatch_is_the_timed_v4_kernel(B, orc):
+    check_big(B, orc, W.c2_channel(*BIG), dict(nodes_per_thread=4, rows_per_block=0))
+
+
+@pytest.mark.parametrize("precision", [W.F32, W.F64])
+def test_big_c3_default_dispatch_is_the_row_walking_kernel(B, orc, precision):
+    check_big(B, orc, W.c3_mrt_obstacles(*BIG, precision=precision), dict(nodes_per_thread=2, rows_per_block=2))
+
+
+def test_big_c4_default_dispatch_fp64_v2(B, orc):
+    check_big(B, orc, W.c4_duct(*BIG), dict(nodes_per_thread=2, rows_per_block=0))
+
+
+def test_big_c5_default_dispatch_shan_chen(B, orc):
+    check_big(B, orc, W.c5_shan_chen(*BIG), dict(rows_per_block=0))
+
+
+def test_big_cavity_default_dispatch(B, orc):
+    check_big(B, orc, W.ldc_cavity(*BIG), dict(nodes_per_thread=4, rows_per_block=0))
+
+
+@pytest.mark.slow
+def test_c2_full_size_256_cubed_100_steps_every_slot(B, orc):
+    """The headline configuration exactly as bench.py times it (256^3, V = 4, plain launch loop), all
+    non-SOLID slots after 100 steps.  The oracle needs ~5 GB and under a minute on the GPU box's host cores."""
+    check_big(B, orc, W.c2_channel(), dict(nodes_per_thread=4, rows_per_block=0))
+
+
 # ---- combinations outside the configs -------------------------------------------------------------
 def generic(lattice, model, precision, shape, seed, solid=0.1, **kw):
     nx, ny, nz = shape

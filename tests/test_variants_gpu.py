@@ -1,7 +1,8 @@
-"""Every kernel variant the library can pick (pack width 1/2/4, 32- and 64-bit slot indices, link words
-fetched eagerly or lazily, graph replay on/off, cluster-resident path on/off) against the oracle.  The
-variants are normally chosen from the lattice size and geometry; the tuning environment variables
-(read at lbm_create / first lbm_step) force each one here so that none ships untested."""
+"""Every kernel variant the library can pick (pack width 1/2/4, 32- and 64-bit slot indices, the row-walking
+kernel for obstacle-rich geometries on/off, graph replay on/off, cluster-resident path on/off) against the
+oracle.  The variants are normally chosen from the lattice size and geometry; the test-only tuning
+environment variables (include/lbm.h; honoured only with LBM_TUNING=1) force each one here so that none
+ships untested, and lbm_get_dispatch confirms that the forced variant is the one that ran."""
 import itertools
 
 import numpy as np
@@ -11,8 +12,8 @@ from paper_1311_2404_b200 import workloads as W
 
 pytestmark = pytest.mark.gpu
 
-ENVS = [dict(LBM_VEC=v, LBM_IDX64=i, LBM_EAGER_LINKS=e, LBM_NO_GRAPH=g, LBM_NO_RESIDENT=g)
-        for v, i, e, g in itertools.product(("1", "2", "4"), ("0", "1"), ("0", "1"), ("0", "1"))]
+ENVS = [dict(LBM_TUNING="1", LBM_VEC=v, LBM_IDX64=i, LBM_ROWS=r, LBM_NO_GRAPH=g, LBM_NO_RESIDENT=g)
+        for v, i, r, g in itertools.product(("1", "2", "4"), ("0", "1"), ("0", "3"), ("0", "1"))]
 
 
 def cases():
@@ -30,7 +31,7 @@ def cases():
     yield w
 
 
-@pytest.mark.parametrize("env", ENVS, ids=lambda e: "v%s_i64%s_eager%s_nograph%s" % (e["LBM_VEC"], e["LBM_IDX64"], e["LBM_EAGER_LINKS"], e["LBM_NO_GRAPH"]))
+@pytest.mark.parametrize("env", ENVS, ids=lambda e: "v%s_i64%s_rows%s_nograph%s" % (e["LBM_VEC"], e["LBM_IDX64"], e["LBM_ROWS"], e["LBM_NO_GRAPH"]))
 def test_forced_variant_matches_oracle(orc, monkeypatch, env):
     import torch
     assert torch.cuda.is_available()
@@ -43,6 +44,14 @@ def test_forced_variant_matches_oracle(orc, monkeypatch, env):
             ref = orc.Oracle(**w.params())
             sim.set_geometry(w.mask)
             ref.set_geometry(w.mask)
+            d = sim.dispatch()
+            assert d["index_bits"] == (64 if env["LBM_IDX64"] == "1" else 32)
+            assert (d["graph_replay"] == 0) == (env["LBM_NO_GRAPH"] == "1")
+            if w.model != W.SC2:
+                if int(env["LBM_VEC"]) <= (4 if w.precision == W.F32 else 2):   # a width the precision has no pack for is ignored
+                    assert d["nodes_per_thread"] == int(env["LBM_VEC"])
+                rows_ok = store == B.LBM_STORE_AB and env["LBM_IDX64"] == "0" and d["nodes_per_thread"] <= 2
+                assert d["rows_per_block"] == (int(env["LBM_ROWS"]) if rows_ok else 0)
             for s in range(w.ncomp):
                 sim.init_equilibrium(w.rho[s], w.u[s], comp=s)
                 ref.init_equilibrium(w.rho[s], w.u[s], comp=s)
