@@ -33,17 +33,31 @@ from paper_1311_2404_b200 import workloads as W  # noqa: E402
 
 METRIC = "MLUPS on 1 B200 and achieved HBM GB/s as % of peak (D3Q19 LBGK fp32)"
 UNIT = "MLUPS"
-# ncu --set full: dram__bytes_read.sum + dram__bytes_write.sum per step (one step_kernel launch;
-# for c5 the sc_fields + sc_step pair), from the committed captures in profiles/r01d_step_kernels.md.
-NCU_TRAFFIC_BYTES = {"c2": 2.497e9, "c3": 8.922e9, "c4": 10.048e9, "c5": 7.903e9, "ldc": 2.506e9}
+# ncu --set full DRAM bytes per step (dram__bytes_read.sum + dram__bytes_write.sum of the step kernel(s)) are
+# read from the committed capture summary below, which also records the commit it was taken at.
+TRAFFIC_FILE = os.path.join(ROOT, "profiles", "r02_traffic.json")
+NCU_DRAM_PEAK_GBS = 8183.8  # ncu's own DRAM peak on this part: 3996 MHz x 2 x 8192 bit / 8 (profiles/)
+
+
+def ncu_traffic(key: str):
+    """(bytes per step, source string) for a config key such as "c2" or "c3_f64"; (None, reason) if absent."""
+    try:
+        with open(TRAFFIC_FILE) as f:
+            t = json.load(f)
+        k = t["configs"][key]
+        return float(k["dram_bytes_per_step"]), "profiles/r02_traffic.json (ncu --set full at commit %s, kernel %s)" % (t["commit"], k["kernel"])
+    except Exception as e:  # missing file or key: say so instead of inventing a number
+        return None, "no committed capture for %s (%s)" % (key, type(e).__name__)
 
 
 def algorithmic_bytes_per_site(w) -> float:
-    """SURVEY 8(d) / DESIGN.md: 2*Q*sizeof(real) + 1 mask byte; Shan-Chen two-pass floor 472 (fp32)."""
+    """SURVEY 8(d) / DESIGN.md: (1 - phi_s) * 2*Q*sizeof(real) + 1 mask byte, phi_s = fraction of SOLID sites (they
+    move no populations; c3: 145.4 / 289.8); Shan-Chen two-pass floor 472 (fp32)."""
     s = 4 if w.precision == W.F32 else 8
+    wet = 1.0 - float((w.mask == W.SOLID).mean())
     if w.model == W.SC2:
-        return 2 * w.Q * s + 2 * s + (2 * 2 * w.Q * s + 2 * s)  # pass 1 + pass 2
-    return 2 * w.Q * s + 1
+        return wet * 3 * (2 * w.Q * s) + 4 * s  # pass 1: read both stores, write psi; pass 2: read both + psi, write both
+    return wet * 2 * w.Q * s + 1
 
 
 def measured_peak():
@@ -169,6 +183,43 @@ class ClockSampler:
                 "power_w_max": max(float(r[2]) for r in rows), "reasons": reasons}
 
 
+OTHER_CONFIGS = (("c1", None), ("c3", "f32"), ("c3", "f64"), ("c4", None), ("c5", None), ("ldc", None))
+
+
+def config_key(cfg, w):
+    return cfg + ("_f64" if cfg == "c3" and w.precision == W.F64 else "")
+
+
+def time_steps(sim, K, repeats, barrier):
+    """K steps between CUDA events on the context's stream, `repeats` times; milliseconds per repeat."""
+    import torch
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    reps = []
+    for _ in range(repeats):
+        barrier()
+        e0.record(sim.stream)
+        sim.step(K)
+        e1.record(sim.stream)
+        barrier()
+        reps.append(e0.elapsed_time(e1))
+    return reps
+
+
+def roofline_of(w, cfg, ms_per_step):
+    peak, which = measured_peak()
+    bps = algorithmic_bytes_per_site(w)
+    achieved = bps * w.sites / (ms_per_step * 1e-3) / 1e9  # per-launch bytes / per-launch time
+    traffic, src = ncu_traffic(config_key(cfg, w))
+    kernel = "sc_fields_kernel + sc_step_kernel" if w.model == W.SC2 else "step_kernel"
+    r = {"bound": "hbm", "kernel": kernel, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+         "peak_source": which, "bytes_per_site": bps, "sites_per_launch": w.sites, "traffic": traffic, "traffic_source": src}
+    if traffic:  # what the DRAM actually moved (ncu) over this run's time, against ncu's own DRAM peak
+        r["dram_gbs"] = traffic / (ms_per_step * 1e-3) / 1e9
+        r["frac_of_ncu_dram_peak"] = r["dram_gbs"] / NCU_DRAM_PEAK_GBS
+        r["traffic_over_algorithmic"] = traffic / (bps * w.sites)
+    return r
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -192,39 +243,38 @@ def run_ours(args):
             dist.init_process_group(backend)
     binding.load()  # no fallback: raises if the CUDA library is missing
 
-    K, Wm = args.steps, max(args.warmup, 3)
-    w = make_workload(args)
-    if w.sites <= (1 << 20):
-        Wm = max(Wm, 128)  # small lattices replay 50-step CUDA graphs: capture them before timing
-    sim = binding.from_workload(w, device=dev, store=binding.LBM_STORE_AA if args.store == "aa" else binding.LBM_STORE_AB)
-    sim.set_geometry(w.mask)
-    for s in range(w.ncomp):
-        sim.init_equilibrium(w.rho[s], w.u[s], comp=s)
-
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize(dev)
+
+    def prepare(w, store):
+        sim = binding.from_workload(w, device=dev, store=binding.LBM_STORE_AA if store == "aa" else binding.LBM_STORE_AB)
+        sim.set_geometry(w.mask)
+        for s in range(w.ncomp):
+            sim.init_equilibrium(w.rho[s], w.u[s], comp=s)
+        return sim
+
+    def warm_steps(w):  # small lattices replay 50-step CUDA graphs: capture them before timing
+        return max(args.warmup, 3, 128 if w.sites <= (1 << 20) else 0)
+
+    K = args.steps
+    w = make_workload(args)
+    Wm = warm_steps(w)
+    sim = prepare(w, args.store)
 
     # ---- device-resident: K steps between CUDA events on the context's stream -------------------
     clocks = ClockSampler(dev_index)  # runs through warm-up, the timed steps and the end-to-end call
     sim.step(Wm)
     l0 = sim.counters()[1]
     barrier()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    reps = []
-    for _ in range(args.repeats):
-        barrier()
-        e0.record(sim.stream)
-        sim.step(K)
-        e1.record(sim.stream)
-        barrier()
-        reps.append(e0.elapsed_time(e1))
+    reps = time_steps(sim, K, args.repeats, barrier)
     launches = (sim.counters()[1] - l0) // args.repeats
-    ms = float(np.median(reps))
-    ms = max_over_ranks(ms, world, dev)
+    ms = max_over_ranks(float(np.median(reps)), world, dev)
+    ms_best = max_over_ranks(float(np.min(reps)), world, dev)
     rho, _ = sim.macro()
     assert bool(torch.isfinite(rho).all()), "state went non-finite during the timed steps"
+    dispatch = sim.dispatch()
 
     # ---- end to end through lbm_run_host: pinned host inputs -> H2D -> init -> K steps -> D2H ------
     tdt = torch.float32 if w.precision == W.F32 else torch.float64
@@ -244,12 +294,31 @@ def run_ours(args):
     d2h = o_rho.numel() * o_rho.element_size() + o_u.numel() * o_u.element_size()
     assert bool(torch.isfinite(o_rho).all())
     clk = clocks.stop()
+    sim.close()
+    del sim, h_mask, h_rho, h_u, o_rho, o_u
+
+    # ---- the other configs in the same process (rank 0, one GPU): same protocol, one line carries them all ----
+    others = {}
+    if rank == 0 and world == 1 and not args.no_other_configs and args.config == "c2" and args.store == "ab" and not args.model:
+        for cfg, prec in OTHER_CONFIGS:
+            kw = {} if prec is None else {"precision": W.F32 if prec == "f32" else W.F64}
+            wo = W.CONFIGS[cfg](**kw)
+            so = prepare(wo, "ab")
+            so.step(warm_steps(wo))
+            r = time_steps(so, K, args.repeats, barrier)
+            assert bool(torch.isfinite(so.macro()[0]).all()), cfg
+            med = float(np.median(r)) / K
+            roof = roofline_of(wo, cfg, med)
+            others[config_key(cfg, wo)] = {
+                "workload": config_dict(wo, cfg)["workload"], "mlups": wo.sites / (med * 1e-3) / 1e6,
+                "mlups_best": wo.sites * K / (min(r) * 1e-3) / 1e6, "ms_per_step": med, "repeats_ms": r,
+                "dispatch": so.dispatch(), "bytes_per_site": roof["bytes_per_site"], "achieved_gbs": roof["achieved"],
+                "frac": None if wo.sites <= (1 << 20) else roof["frac"],  # c1 is launch-bound, not HBM-bound
+                "traffic": roof["traffic"], "frac_of_ncu_dram_peak": roof.get("frac_of_ncu_dram_peak")}
+            so.close()
+            del so, wo
 
     if rank == 0:
-        peak, which = measured_peak()
-        bps = algorithmic_bytes_per_site(w)
-        achieved = bps * w.sites * K / (ms * 1e-3) / 1e9  # per-launch bytes / per-launch time
-        kernel = "sc_fields_kernel + sc_step_kernel" if w.model == W.SC2 else "step_kernel"
         cb = None
         if world == 1 and not args.no_cpu_baseline:
             cb, _, _ = time_oracle(args.config, args.cpu_steps, 1)
@@ -257,20 +326,19 @@ def run_ours(args):
                 "n_gpus": world, "steps": K, "warmup": Wm, "ms_per_step": ms / K, "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "f32" if w.precision == W.F32 else "f64",
                 "data": "synthetic",
+                "best": aggregate_mlups(w.sites, K, world, ms_best * 1e-3), "median": aggregate_mlups(w.sites, K, world, ms * 1e-3),
                 "config": config_dict(w, args.config, {
-                    "l2": "working set %.2f GB per step >> 126 MB L2 (no flush needed)" % (bps * w.sites / 1e9),
-                    "timing": "median of %d repeats of K steps, CUDA events on the ctx stream" % args.repeats,
-                    "repeats_ms": reps}, store=args.store),
+                    "l2": "working set %.2f GB per step >> 126 MB L2 (no flush needed)" % (algorithmic_bytes_per_site(w) * w.sites / 1e9),
+                    "timing": "value = median of %d repeats of K steps (best also given), CUDA events on the ctx stream" % args.repeats,
+                    "repeats_ms": reps, "dispatch": dispatch}, store=args.store),
                 "clocks": clk,
                 "e2e": {"value": aggregate_mlups(w.sites, K, world, e2e_s), "unit": UNIT,
                         "h2d_bytes_per_step": h2d / K, "d2h_bytes_per_step": d2h / K,
                         "note": "one lbm_run_host call = H2D(mask, rho0, u0) + init + K steps + macro + D2H(rho, u); bytes amortised over K"},
                 "gpu_launches": int(launches),
-                "roofline": {"bound": "hbm", "kernel": kernel, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                             "frac": achieved / peak, "peak_source": which,
-                             "bytes_per_site": bps, "sites_per_launch": w.sites,
-                             "traffic": NCU_TRAFFIC_BYTES.get(args.config)},
-                "cpu_baseline": cb}
+                "roofline": roofline_of(w, args.config, ms / K),
+                "cpu_baseline": cb,
+                "other_configs": others}
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
@@ -283,7 +351,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="c2", choices=sorted(W.CONFIGS))
-    ap.add_argument("--repeats", type=int, default=1)
+    ap.add_argument("--repeats", type=int, default=3, help="repeats of the K timed steps; value = median, best also reported")
+    ap.add_argument("--no-other-configs", action="store_true", help="skip timing c1, c3, c4, c5 and ldc after the headline")
     ap.add_argument("--cpu-steps", type=int, default=250, help="oracle steps on the bounded sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--precision", default=None, choices=["f32", "f64"], help="override the config's precision (c3 is quoted in both)")

@@ -159,6 +159,8 @@ typedef struct {
     int32_t resident_ctas;           /* CTAs of that cluster (8 or 16), else 0                        */
     int32_t rows_per_block;          /* > 0: row-walking kernel for obstacle-rich geometries          */
     int32_t block_threads;           /* threads per block of the step kernels                         */
+    int32_t sc_split;                /* LBM_SC2: 1 = one collide launch per component, 0 = one
+                                        launch for both                                               */
     int32_t reserved_;
 } lbm_dispatch;
 int lbm_get_dispatch(const lbm_ctx *ctx, lbm_dispatch *out);
@@ -167,7 +169,7 @@ int lbm_get_dispatch(const lbm_ctx *ctx, lbm_dispatch *out);
  * ONLY if LBM_TUNING=1 is set too: LBM_VEC (1|2|4 nodes per thread), LBM_IDX64 (1: 64-bit slot indices),
  * LBM_BLOCK_X, LBM_BLOCK_THREADS (multiples of 32), LBM_ROWS (rows per block of the row-walking kernel,
  * 0 = off), LBM_NO_GRAPH, LBM_NO_RESIDENT, LBM_RESIDENT_MAX (largest lattice of the cluster-resident
- * path).  They select among kernels that all pass the same parity tests; they are not part of the ABI. */
+ * path), LBM_SC_SPLIT (0: monolithic two-component collide kernel), LBM_SC_FIELDS_VEC, LBM_SPAN_BX.  They select among kernels that all pass the same parity tests; they are not part of the ABI. */
 
 const char *lbm_last_error(const lbm_ctx *ctx);
 

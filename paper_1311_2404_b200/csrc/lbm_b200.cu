@@ -67,7 +67,10 @@ void make_layout(const lbm_params *p, int Q, int D, Layout *L) {
     L->link = off; off += align_up(4 * N);
     L->counters = off; off += ALIGN;
     if (nc == 2)
-        { L->psi[0] = L->psi[1] = off; off += align_up(2 * N * rs); }  // (psi_A, psi_B) interleaved
+    {   // (psi_A, psi_B) interleaved, or planar psi_A | psi_B for the split kernels; u' of the split kernels
+        L->psi[0] = L->psi[1] = off; off += align_up(2 * N * rs);
+        L->up = off; off += align_up((size_t)D * N * rs);
+    }
     L->stage_mask = off; off += align_up(N);
     L->stage_rho = off; off += align_up(N * rs);
     L->stage_u = off; off += align_up(D * N * rs);
@@ -102,10 +105,10 @@ int env_int(const char *name, int dflt, int lo, int hi) {
 //   fix-up of 4 nodes costs too many registers (c3: V = 2 34.8, V = 4 29.5, V = 1 26.1 GLUPS);
 //   fp64: 2-node packs (c4: 22.4 vs 22.1); two-component kernel: register-bound, 1 node (c5: 12.0 vs 9.9).
 // LBM_VEC overrides (tuning knob, not part of the ABI).  Falls back to what divides nx.
-int pick_vec(const lbm_params *p, double nonbulk_fraction) {
+int pick_vec(const lbm_params *p, double nonbulk_fraction, bool sc_split = false) {
     const int widest = p->precision == LBM_F32 ? 4 : 2;
     int v = 1;
-    if (p->model != LBM_SC2) v = p->precision == LBM_F64 ? 2 : (nonbulk_fraction < 0.2 ? 4 : 2);
+    if (p->model != LBM_SC2 || sc_split) v = p->precision == LBM_F64 ? 2 : (nonbulk_fraction < 0.2 ? 4 : 2);
     // regularized LBGK / Smagorinsky carry six second moments per node: 2-node packs (cavity box:
     // LES 43.0 vs 33.9 GLUPS at V = 4, regularized 42.9 vs 41.4)
     // and so does MRT with its 19 moments (cavity box: 43.0 vs 41.0 GLUPS)
@@ -205,6 +208,11 @@ LBM_API int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, voi
     c->aa = p->store == LBM_STORE_AA;
     c->idx32 = (double)Q * (double)c->g.N < 4294967296.0 && !env_int("LBM_IDX64", 0, 0, 1);
     c->rows = 0;
+    c->sc_split = (p->model == LBM_SC2 && env_int("LBM_SC_SPLIT", 1, 0, 1)) ? pick_vec(p, 0.0, true) : 0;
+    c->all_bulk = true;  // the geometry starts all-FLUID
+    c->span_bx = env_int("LBM_SPAN_BX", 0, 32, 256) / 32 * 32;
+    c->sc_fields_vec = env_int("LBM_SC_FIELDS_VEC", 1, 1, 2);
+    if (p->nx % 2) c->sc_fields_vec = 1;
     c->block_threads = env_int("LBM_BLOCK_THREADS", 64, 32, 256) / 32 * 32;
     c->vt = select_impl(p);
     c->err[0] = 0;
@@ -247,7 +255,9 @@ LBM_API int lbm_set_geometry(lbm_ctx *c, const uint8_t *d_mask) {
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
     if (e != cudaSuccess) return fail(c, LBM_ECUDA, "reading the geometry counter: %s", cudaGetErrorString(e));
     const double frac = (double)nonbulk / (double)c->g.N;
+    c->all_bulk = nonbulk == 0;
     c->vec = pick_vec(&c->p, frac);
+    if (c->sc_split) c->sc_split = pick_vec(&c->p, frac, true);
     c->rows = env_int("LBM_ROWS", frac >= 0.2 ? 2 : 0, 0, 65535);
     return LBM_OK;
 }
@@ -399,7 +409,9 @@ LBM_API int lbm_get_counters(const lbm_ctx *c, int64_t *steps, int64_t *launches
 LBM_API int lbm_get_dispatch(const lbm_ctx *c, lbm_dispatch *out) {
     CHECK_CTX(c);
     if (!out) return LBM_EINVAL;
-    out->nodes_per_thread = c->p.model == LBM_SC2 ? ((c->vec >= 2 && !c->aa && c->rs == 4) ? 2 : 1) : c->vec;
+    out->nodes_per_thread = c->p.model == LBM_SC2 ? ((c->sc_split && !c->aa) ? c->sc_split : (c->vec >= 2 && !c->aa && c->rs == 4) ? 2 : 1) : c->vec;
+    out->reserved_ = 0;
+    out->sc_split = c->p.model == LBM_SC2 && c->sc_split && !c->aa;
     out->index_bits = c->idx32 ? 32 : 64;
     out->graph_replay = (c->use_graph && !c->no_graph) ? GRAPH_STEPS : 0;
     out->resident_nodes_per_cta = (c->resident_slog2 > 0 && c->resident_state >= 0) ? 1 << c->resident_slog2 : 0;

@@ -21,7 +21,7 @@ constexpr size_t ALIGN = 256;
 inline size_t align_up(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
 
 struct Layout {
-    size_t store[2][2], type, link, counters, psi[2], stage_mask, stage_rho, stage_u, total;
+    size_t store[2][2], type, link, counters, psi[2], up, stage_mask, stage_rho, stage_u, total;
 };
 
 struct Vtbl;
@@ -44,6 +44,10 @@ struct lbm_ctx {
     int resident_slog2; // > 0: the AB store fits one cluster's shared memory; log2 of nodes per CTA
     int resident_ctas;  // CTAs of that cluster (8, or 16 = non-portable size)
     int resident_state; // 0 not probed yet, 1 launchable, -1 not launchable here (fall back for good)
+    int span_bx;        // tuning: block width (threads along x) of the step kernels, 0 = default
+    bool all_bulk;      // no node of the geometry is SOLID / BOUNDARY / special: the step kernels skip the type array
+    int sc_split;       // Shan-Chen: > 0 = split variant (one collide launch per component), nodes per thread
+    int sc_fields_vec;  // Shan-Chen: nodes per thread of the macro-field pass (the collide pass uses `vec`)
     int rows;           // > 0: obstacle-rich geometry (>= 20 % of the nodes not BULK): step_rows_kernel, rows per block
     bool idx32;         // Q * N < 2^32: slot numbers fit 32 bits (cheaper address arithmetic)
     int block_x;        // one-node-per-thread kernels: 1-D block along x
@@ -126,7 +130,8 @@ struct Launch { dim3 grid, block; };
 // Step kernels: V nodes per thread along x, 2-D blocks (bx packs) x (by rows).
 Launch span_launch(const lbm_ctx *c, int V) {
     const int nxv = c->g.nx / V;
-    const int bx = nxv > 32 ? 64 : 32;
+    int bx = nxv > 32 ? 64 : 32;
+    if (c->span_bx > 0) bx = c->span_bx;
     int by = c->block_threads / bx;
     if (by < 1) by = 1;
     while (by > 1 && by / 2 >= c->g.ny) by /= 2;

@@ -256,7 +256,10 @@ __device__ __forceinline__ void gather_span(const T *__restrict__ src, int64_t N
 }
 
 // Node types of the pack as one word (byte k = node k).
+// type == nullptr: the geometry has BULK nodes only (all-FLUID torus, e.g. c1 and c5): no load, and the
+// thread does not wait one memory round trip before it issues its pull.
 template <int V> __device__ __forceinline__ uint32_t load_types(const uint8_t *__restrict__ type, int n0) {
+    if (!type) return 0u;
     if (V == 4) return __ldg(reinterpret_cast<const uint32_t *>(type + n0));
     if (V == 2) return __ldg(reinterpret_cast<const uint16_t *>(type + n0));
     return __ldg(type + n0);
@@ -372,10 +375,10 @@ template <int V> __device__ __forceinline__ void load_links(const uint32_t *__re
     else w[0] = __ldg(link + n0);
 }
 
-// 64-thread blocks; fp32: 12 blocks per SM (80 registers, 24 warps), fp64: 6 (168 registers), by measurement
+// 64-thread blocks (128 allowed); fp32: 80 registers (24 warps per SM), fp64: 168 registers, by measurement
 // on c3 (fp32 at 96 registers / 20 warps: the same; at 64 registers / 32 warps: -10 %, spills).
 template <class L, typename T, int V, typename I, int MODEL, int FORCE>
-__global__ void __launch_bounds__(64, sizeof(T) == 4 ? 12 : 6)
+__global__ void __launch_bounds__(128, sizeof(T) == 4 ? 6 : 3)
 step_rows_kernel(Geom g, const uint32_t *__restrict__ link, const T *__restrict__ src, T *__restrict__ dst,
                  Relax<T> rp, int rows) {
     Span s;
@@ -764,6 +767,10 @@ __device__ __forceinline__ void psi_gradient(const typename Pair<T>::type *__res
     }
 }
 
+template <class L, typename T, int PSI, int FS>
+__device__ __forceinline__ void sc_collide_with_gradient(T (&hA)[L::Q], T (&hB)[L::Q], const T (&SA)[3], const T (&SB)[3],
+                                                         const Relax<T> &rpA, const Relax<T> &rpB, T G);
+
 // Collision of both components at one node (rows a10-a11): moments, common velocity u',
 // coupling forces (eq. 10, sign A11) + body force, Guo (A13) or EDM (A22) per component; node types
 // FULLWAY / VELOCITY replace the collision of both components.
@@ -778,6 +785,13 @@ __device__ __forceinline__ void sc_collide_node(T (&hA)[L::Q], T (&hB)[L::Q], ui
     }
     T SA[3], SB[3];
     psi_gradient<L, T>(psi, n, o, SA, SB);
+    sc_collide_with_gradient<L, T, PSI, FS>(hA, hB, SA, SB, rpA, rpB, G);
+}
+
+// ... with S_A, S_B already summed (the V-node kernel sums them row by row for the whole pack).
+template <class L, typename T, int PSI, int FS>
+__device__ __forceinline__ void sc_collide_with_gradient(T (&hA)[L::Q], T (&hB)[L::Q], const T (&SA)[3], const T (&SB)[3],
+                                                         const Relax<T> &rpA, const Relax<T> &rpB, T G) {
     T dA, dB, jA[3], jB[3];
     moments<L, T>(hA, dA, jA);
     moments<L, T>(hB, dB, jB);
@@ -801,6 +815,78 @@ __device__ __forceinline__ void sc_collide_node(T (&hA)[L::Q], T (&hB)[L::Q], ui
     collide<L, T, MODEL_BGK, FS>(hB, rB, dB, vB, mB, FB, rpB);
 }
 
+// S_A, S_B for the V nodes of a pack, summed row by row: for each of the (e_y, e_z) rows the D3Q19 / D2Q9
+// neighbourhood touches, the interleaved field is read once for the whole pack (x0 - 1, the pack's own V
+// columns as one aligned vector, x0 + V) instead of once per node and link: 19 loads per 2-node pack
+// where the one-node kernel issues 36, all but the two edge columns 16 bytes wide.
+template <typename T, int V> struct PairRow;
+template <> struct PairRow<float, 2> {
+    static __device__ __forceinline__ void ld(const float2 *p, float2 (&v)[2]) {
+        const float4 q = __ldg(reinterpret_cast<const float4 *>(p));
+        v[0] = make_float2(q.x, q.y); v[1] = make_float2(q.z, q.w);
+    }
+};
+template <typename T> struct PairRow<T, 1> {
+    static __device__ __forceinline__ void ld(const typename Pair<T>::type *p, typename Pair<T>::type (&v)[1]) { v[0] = __ldg(p); }
+};
+template <> struct PairRow<double, 2> {
+    static __device__ __forceinline__ void ld(const double2 *p, double2 (&v)[2]) { v[0] = __ldg(p); v[1] = __ldg(p + 1); }
+};
+
+template <class L, typename T, int V>
+__device__ __forceinline__ void psi_gradient_span(const typename Pair<T>::type *__restrict__ psi, const Span &s,
+                                                  T (&SA)[V][3], T (&SB)[V][3]) {
+    using P = typename Pair<T>::type;
+    T axA[V][3], dgA[V][3], axB[V][3], dgB[V][3];
+#pragma unroll
+    for (int k = 0; k < V; k++)
+#pragma unroll
+        for (int c = 0; c < 3; c++) axA[k][c] = dgA[k][c] = axB[k][c] = dgB[k][c] = T(0);
+#pragma unroll
+    for (int dz = -1; dz <= 1; dz++) {
+#pragma unroll
+        for (int dy = -1; dy <= 1; dy++) {
+            // which columns of row (dy, dz) the neighbourhood touches
+            bool centre = false, sides = false;
+#pragma unroll
+            for (int i = 1; i < L::Q; i++)
+                if (L::ey(i) == dy && L::ez(i) == dz) { if (L::ex(i) == 0) centre = true; else sides = true; }
+            if (!centre && !sides) continue;
+            const int r = s.row + (dy == 1 ? s.o.yp : dy == -1 ? s.o.ym : 0) + (dz == 1 ? s.o.zp : dz == -1 ? s.o.zm : 0);
+            P v[V + 2];
+            if (centre || V > 1) {  // the pack's own columns: neighbours at e_x = 0, and at e_x = +-1 of the other nodes
+                P mid[V];
+                PairRow<T, V>::ld(psi + (r + s.x0), mid);
+#pragma unroll
+                for (int k = 0; k < V; k++) v[k + 1] = mid[k];
+            }
+            if (sides) { v[0] = __ldg(psi + (r + s.xm)); v[V + 1] = __ldg(psi + (r + s.xp)); }
+#pragma unroll
+            for (int i = 1; i < L::Q; i++) {
+                if (L::ey(i) != dy || L::ez(i) != dz) continue;
+                const bool axis = (L::ex(i) != 0) + (dy != 0) + (dz != 0) == 1;
+#pragma unroll
+                for (int k = 0; k < V; k++) {
+                    const P p = v[k + 1 + L::ex(i)];
+                    T(&a)[3] = axis ? axA[k] : dgA[k];
+                    T(&b)[3] = axis ? axB[k] : dgB[k];
+                    if (L::ex(i) == 1) { a[0] += p.x; b[0] += p.y; } else if (L::ex(i) == -1) { a[0] -= p.x; b[0] -= p.y; }
+                    if (dy == 1) { a[1] += p.x; b[1] += p.y; } else if (dy == -1) { a[1] -= p.x; b[1] -= p.y; }
+                    if (dz == 1) { a[2] += p.x; b[2] += p.y; } else if (dz == -1) { a[2] -= p.x; b[2] -= p.y; }
+                }
+            }
+        }
+    }
+    const T ratio = L::template w<T>(1) / L::template w<T>(L::Q - 1), wd = L::template w<T>(L::Q - 1);
+#pragma unroll
+    for (int k = 0; k < V; k++)
+#pragma unroll
+        for (int c = 0; c < 3; c++) {
+            SA[k][c] = wd * (ratio * axA[k][c] + dgA[k][c]);
+            SB[k][c] = wd * (ratio * axB[k][c] + dgB[k][c]);
+        }
+}
+
 // Pass 2 (rows a10-a11): both components in one kernel: gather, moments, common velocity u'
 // (P:188), forces (eq. 10, sign A11) + body force, v_s = u' + F_s / (2 rho_s), LBGK + Guo (A13).
 template <class L, typename T, int V, typename I, int PSI, int FS>
@@ -819,18 +905,168 @@ sc_step_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restr
     gather_span<L, T, V, I>(srcB, g.N, s, hB);
     pull_reflected_span<L, T, V, I>(srcA, g.N, n0, types, link, hA);
     pull_reflected_span<L, T, V, I>(srcB, g.N, n0, types, link, hB);
+    T SA[V][3], SB[V][3];
+    psi_gradient_span<L, T, V>(psi, s, SA, SB);
 #pragma unroll
     for (int k = 0; k < V; k++) {
-        Nbr o = s.o;
-        const int x = s.x0 + k;
-        o.xm = (x == 0) ? (g.nx - 1) : -1;
-        o.xp = (x == g.nx - 1) ? -(g.nx - 1) : 1;
-        sc_collide_node<L, T, PSI, FS>(hA[k], hB[k], (types >> (8 * k)) & 0xffu, psi, n0 + k, o, rpA, rpB, G);
+        const uint32_t t = (types >> (8 * k)) & 0xffu;
+        if (t & NODE_FULLWAY) { fullway_reverse<L, T>(hA[k]); fullway_reverse<L, T>(hB[k]); }
+        else if (t & NODE_VELOCITY) { velocity_node<L, T>(hA[k], rpA.ubc); velocity_node<L, T>(hB[k], rpB.ubc); }
+        else sc_collide_with_gradient<L, T, PSI, FS>(hA[k], hB[k], SA[k], SB[k], rpA, rpB, G);
     }
     store_span<L, T, V, I>(dstA, g.N, n0, hA);
     store_span<L, T, V, I>(dstB, g.N, n0, hB);
 }
 
+
+// ---- Shan-Chen, split variant ("split" kernels, one launch per component) -----------
+// The paper found per-component collide kernels faster than one monolithic kernel by 5-53 % because of
+// their smaller register footprint.  Same on B200: the monolithic kernel holds two components per node
+// (80 registers at ONE node per thread, 70 % of the DRAM peak), a one-component kernel is the ordinary
+// step kernel at V = 4 plus a force.  Price: the common velocity u' has to travel through memory.
+//   pass 1  sc_fields_split_kernel: psi_A, psi_B (planar) and u' from the time-t state     152 B read, 20 B written (fp32)
+//   pass 2  sc_collide_split_kernel, once per component s: pull f_s, S = sum_i w_i psi_other(x + e_i) e_i,
+//           u', F_s, collide, store                                                         2 x (76 + 4 + 12 B read, 76 B written)
+// 508 B per site instead of 472; which variant runs is chosen by measurement (lbm_b200.cu).
+template <class L, typename T, int V, typename I, int PSI>
+__global__ void __launch_bounds__(256)
+sc_fields_split_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restrict__ link,
+                       const T *__restrict__ srcA, const T *__restrict__ srcB, T *__restrict__ psiA,
+                       T *__restrict__ psiB, T *__restrict__ up, T inv_tauA, T inv_tauB) {
+    Span s;
+    if (!thread_span<V>(g, s)) return;
+    const int n0 = s.row + s.x0;
+    const uint32_t types = load_types<V>(type, n0);
+    T pa[V], pb[V], u[3][V];
+#pragma unroll
+    for (int k = 0; k < V; k++) { pa[k] = pb[k] = -psi_one<T, PSI>(); u[0][k] = u[1][k] = u[2][k] = T(0); }
+    if (!all_solid<V>(types)) {
+        T h[V][L::Q], rA[V], jA[V][3];
+        gather_span<L, T, V, I>(srcA, g.N, s, h);
+        pull_reflected_span<L, T, V, I>(srcA, g.N, n0, types, link, h);
+#pragma unroll
+        for (int k = 0; k < V; k++) {
+            T d;
+            moments<L, T>(h[k], d, jA[k]);
+            rA[k] = T(1) + d;
+            pa[k] = psi_dev<T, PSI>(d);
+        }
+        gather_span<L, T, V, I>(srcB, g.N, s, h);
+        pull_reflected_span<L, T, V, I>(srcB, g.N, n0, types, link, h);
+#pragma unroll
+        for (int k = 0; k < V; k++) {
+            T d, jB[3];
+            moments<L, T>(h[k], d, jB);
+            const T rB = T(1) + d;
+            pb[k] = psi_dev<T, PSI>(d);
+            const T inv_den = T(1) / (rA[k] * inv_tauA + rB * inv_tauB);
+#pragma unroll
+            for (int a = 0; a < 3; a++) u[a][k] = (jA[k][a] * inv_tauA + jB[a] * inv_tauB) * inv_den;  // u'
+            if ((types >> (8 * k)) & (NODE_SOLID | NODE_FULLWAY)) {  // dry: psi = 0 (A14), no velocity
+                pa[k] = pb[k] = -psi_one<T, PSI>();
+                u[0][k] = u[1][k] = u[2][k] = T(0);
+            }
+        }
+    }
+    Pack<T, V>::stp(psiA + n0, pa);  // plain stores: pass 2 re-reads the fields right away (L2)
+    Pack<T, V>::stp(psiB + n0, pb);
+#pragma unroll
+    for (int a = 0; a < L::D; a++) Pack<T, V>::stp(up + ((int64_t)a * g.N + n0), u[a]);
+}
+
+// S = sum_i w_i psi(x + e_i) e_i of ONE planar field for the V nodes of a pack, row by row (see psi_gradient_span).
+template <class L, typename T, int V>
+__device__ __forceinline__ void field_gradient_span(const T *__restrict__ psi, const Span &s, T (&S)[V][3]) {
+    T ax[V][3], dg[V][3];
+#pragma unroll
+    for (int k = 0; k < V; k++)
+#pragma unroll
+        for (int c = 0; c < 3; c++) ax[k][c] = dg[k][c] = T(0);
+#pragma unroll
+    for (int dz = -1; dz <= 1; dz++) {
+#pragma unroll
+        for (int dy = -1; dy <= 1; dy++) {
+            bool centre = false, sides = false;
+#pragma unroll
+            for (int i = 1; i < L::Q; i++)
+                if (L::ey(i) == dy && L::ez(i) == dz) { if (L::ex(i) == 0) centre = true; else sides = true; }
+            if (!centre && !sides) continue;
+            const int r = s.row + (dy == 1 ? s.o.yp : dy == -1 ? s.o.ym : 0) + (dz == 1 ? s.o.zp : dz == -1 ? s.o.zm : 0);
+            T v[V + 2];
+            if (centre || V > 1) {
+                T mid[V];
+                Pack<T, V>::ld(psi + (r + s.x0), mid);
+#pragma unroll
+                for (int k = 0; k < V; k++) v[k + 1] = mid[k];
+            }
+            if (sides) { v[0] = __ldg(psi + (r + s.xm)); v[V + 1] = __ldg(psi + (r + s.xp)); }
+#pragma unroll
+            for (int i = 1; i < L::Q; i++) {
+                if (L::ey(i) != dy || L::ez(i) != dz) continue;
+                const bool axis = (L::ex(i) != 0) + (dy != 0) + (dz != 0) == 1;
+#pragma unroll
+                for (int k = 0; k < V; k++) {
+                    const T p = v[k + 1 + L::ex(i)];
+                    T(&a)[3] = axis ? ax[k] : dg[k];
+                    if (L::ex(i) == 1) a[0] += p; else if (L::ex(i) == -1) a[0] -= p;
+                    if (dy == 1) a[1] += p; else if (dy == -1) a[1] -= p;
+                    if (dz == 1) a[2] += p; else if (dz == -1) a[2] -= p;
+                }
+            }
+        }
+    }
+    const T ratio = L::template w<T>(1) / L::template w<T>(L::Q - 1), wd = L::template w<T>(L::Q - 1);
+#pragma unroll
+    for (int k = 0; k < V; k++)
+#pragma unroll
+        for (int c = 0; c < 3; c++) S[k][c] = wd * (ratio * ax[k][c] + dg[k][c]);
+}
+
+template <class L, typename T, int V, typename I, int PSI, int FS>
+__global__ void __launch_bounds__(256)
+sc_collide_split_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restrict__ link,
+                        const T *__restrict__ src, T *__restrict__ dst, const T *__restrict__ psi_other,
+                        const T *__restrict__ up, Relax<T> rp, T G) {
+    Span s;
+    if (!thread_span<V>(g, s)) return;
+    const int n0 = s.row + s.x0;
+    const uint32_t types = load_types<V>(type, n0);
+    if (all_solid<V>(types)) return;
+    T h[V][L::Q];
+    gather_span<L, T, V, I>(src, g.N, s, h);
+    T u[3][V];
+#pragma unroll
+    for (int a = 0; a < 3; a++) {
+        if (a < L::D) Pack<T, V>::ldp(up + ((int64_t)a * g.N + n0), u[a]);
+        else {
+#pragma unroll
+            for (int k = 0; k < V; k++) u[a][k] = T(0);
+        }
+    }
+    T S[V][3];
+    field_gradient_span<L, T, V>(psi_other, s, S);
+    pull_reflected_span<L, T, V, I>(src, g.N, n0, types, link, h);
+#pragma unroll
+    for (int k = 0; k < V; k++) {
+        const uint32_t t = (types >> (8 * k)) & 0xffu;
+        if (t & NODE_FULLWAY) fullway_reverse<L, T>(h[k]);
+        else if (t & NODE_VELOCITY) velocity_node<L, T>(h[k], rp.ubc);
+        else {
+            T d, j[3];
+            moments<L, T>(h[k], d, j);
+            const T r = T(1) + d, p = psi_dev<T, PSI>(d) + psi_one<T, PSI>(), ir = T(0.5) / r;
+            T v[3], m[3], F[3];
+#pragma unroll
+            for (int a = 0; a < 3; a++) {
+                F[a] = -G * p * S[k][a] + r * rp.g[a];               // eq. (10), sign A11, + body force
+                v[a] = FS == FORCE_EDM ? u[a][k] : u[a][k] + F[a] * ir;  // Guo: v_s = u' + F_s / (2 rho_s) (A13); EDM: u' (A22)
+                m[a] = r * v[a];
+            }
+            collide<L, T, MODEL_BGK, FS>(h[k], r, d, v, m, F, rp);
+        }
+    }
+    store_span<L, T, V, I>(dst, g.N, n0, h);
+}
 
 // ---- Shan-Chen on the in-place AA store: one node per thread, both parities (see aa_slot) ------
 template <class L, typename T, typename I, int PSI>

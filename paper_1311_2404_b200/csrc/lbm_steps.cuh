@@ -10,6 +10,8 @@ template <class L, typename T> struct Steps {
     static T *dst(lbm_ctx *c, int s) { return at<T>(c, c->lay.store[s][c->cur ^ 1]); }
     static uint8_t *type(lbm_ctx *c) { return at<uint8_t>(c, c->lay.type); }
     static uint32_t *link(lbm_ctx *c) { return at<uint32_t>(c, c->lay.link); }
+    // for the V-node step kernels: no type array to read when every node is BULK
+    static const uint8_t *type_or_null(lbm_ctx *c) { return c->all_bulk ? nullptr : at<uint8_t>(c, c->lay.type); }
 
     template <int V, int MODEL, int FORCE> static int step_single_v(lbm_ctx *c, int n, const Relax<T> &rp) {
         return c->idx32 ? step_single_vi<V, uint32_t, MODEL, FORCE>(c, n, rp) : step_single_vi<V, int64_t, MODEL, FORCE>(c, n, rp);
@@ -21,7 +23,7 @@ template <class L, typename T> struct Steps {
             const Launch l1 = span_launch(c, 1);
             T *f = at<T>(c, c->lay.store[0][0]);
             for (int t = 0; t < n; t++) {
-                if (c->cur == 0) aa_even_kernel<L, T, V, I, MODEL, FORCE><<<l.grid, l.block, 0, c->stream>>>(c->g, type(c), f, rp);
+                if (c->cur == 0) aa_even_kernel<L, T, V, I, MODEL, FORCE><<<l.grid, l.block, 0, c->stream>>>(c->g, type_or_null(c), f, rp);
                 else aa_odd_kernel<L, T, I, MODEL, FORCE><<<l1.grid, l1.block, 0, c->stream>>>(c->g, type(c), link(c), f, rp);
                 if (int rc = check_launch(c, "aa_step_kernel")) return rc;
                 c->cur ^= 1;
@@ -31,7 +33,7 @@ template <class L, typename T> struct Steps {
         }
         if constexpr (V <= 2 && sizeof(I) == 4) {
             if (c->rows > 0) {  // obstacle-rich geometry: row-walking kernel, link words one row ahead
-                const int nxv = c->g.nx / V, bx = nxv > 32 ? 64 : 32;
+                const int nxv = c->g.nx / V, bx = c->span_bx > 0 ? c->span_bx : (nxv > 32 ? 64 : 32);
                 const dim3 grid((nxv + bx - 1) / bx, (c->g.ny + c->rows - 1) / c->rows, c->g.nz);
                 for (int t = 0; t < n; t++) {
                     step_rows_kernel<L, T, V, I, MODEL, FORCE><<<grid, bx, 0, c->stream>>>(c->g, link(c), src(c, 0), dst(c, 0), rp, c->rows);
@@ -43,7 +45,7 @@ template <class L, typename T> struct Steps {
             }
         }
         for (int t = 0; t < n; t++) {
-            step_kernel<L, T, V, I, MODEL, FORCE><<<l.grid, l.block, 0, c->stream>>>(c->g, type(c), link(c), src(c, 0), dst(c, 0), rp);
+            step_kernel<L, T, V, I, MODEL, FORCE><<<l.grid, l.block, 0, c->stream>>>(c->g, type_or_null(c), link(c), src(c, 0), dst(c, 0), rp);
             if (int rc = check_launch(c, "step_kernel")) return rc;
             c->cur ^= 1;
             c->steps++;
@@ -111,12 +113,20 @@ template <class L, typename T> struct Steps {
 
     template <int V, int PSI> static int step_sc_v(lbm_ctx *c, int n) {
         if (c->p.force_scheme == LBM_FORCE_EDM)
-            return c->idx32 ? step_sc_vi<V, uint32_t, PSI, FORCE_EDM>(c, n) : step_sc_vi<V, int64_t, PSI, FORCE_EDM>(c, n);
-        return c->idx32 ? step_sc_vi<V, uint32_t, PSI, FORCE_GUO>(c, n) : step_sc_vi<V, int64_t, PSI, FORCE_GUO>(c, n);
+            return c->idx32 ? step_sc_vf<V, uint32_t, PSI, FORCE_EDM>(c, n) : step_sc_vf<V, int64_t, PSI, FORCE_EDM>(c, n);
+        return c->idx32 ? step_sc_vf<V, uint32_t, PSI, FORCE_GUO>(c, n) : step_sc_vf<V, int64_t, PSI, FORCE_GUO>(c, n);
     }
 
-    template <int V, typename I, int PSI, int FS> static int step_sc_vi(lbm_ctx *c, int n) {
-        const Launch l = span_launch(c, V);
+    // VF = nodes per thread of the macro-field pass, V = of the collide pass (chosen independently)
+    template <int V, typename I, int PSI, int FS> static int step_sc_vf(lbm_ctx *c, int n) {
+        if constexpr (sizeof(T) == 4) {
+            if (c->sc_fields_vec == 2 && !c->aa) return step_sc_vi<2, V, I, PSI, FS>(c, n);
+        }
+        return step_sc_vi<1, V, I, PSI, FS>(c, n);
+    }
+
+    template <int VF, int V, typename I, int PSI, int FS> static int step_sc_vi(lbm_ctx *c, int n) {
+        const Launch l = span_launch(c, V), lf = span_launch(c, VF);
         const Relax<T> rA = make_relax<T>(c, 0), rB = make_relax<T>(c, 1);
         auto *psi = at<typename Pair<T>::type>(c, c->lay.psi[0]);
         if (c->aa) {  // in place: one node per thread, `cur` is the parity
@@ -136,10 +146,10 @@ template <class L, typename T> struct Steps {
             }
         }
         for (int t = 0; t < n; t++) {
-            sc_fields_kernel<L, T, V, I, PSI><<<l.grid, l.block, 0, c->stream>>>(c->g, type(c), link(c), src(c, 0), src(c, 1), psi);
+            sc_fields_kernel<L, T, VF, I, PSI><<<lf.grid, lf.block, 0, c->stream>>>(c->g, type_or_null(c), link(c), src(c, 0), src(c, 1), psi);
             if (int rc = check_launch(c, "sc_fields_kernel")) return rc;
             sc_step_kernel<L, T, V, I, PSI, FS><<<l.grid, l.block, 0, c->stream>>>(
-                c->g, type(c), link(c), src(c, 0), src(c, 1), dst(c, 0), dst(c, 1), psi, rA, rB, T(c->p.sc_G));
+                c->g, type_or_null(c), link(c), src(c, 0), src(c, 1), dst(c, 0), dst(c, 1), psi, rA, rB, T(c->p.sc_G));
             if (int rc = check_launch(c, "sc_step_kernel")) return rc;
             c->cur ^= 1;
             c->steps++;
@@ -147,7 +157,40 @@ template <class L, typename T> struct Steps {
         return LBM_OK;
     }
 
+    // Split variant: one macro-field pass (psi_A, psi_B, u') + one collide pass per component.
+    template <int V, typename I, int PSI, int FS> static int step_sc_split_vi(lbm_ctx *c, int n) {
+        const Launch l = span_launch(c, V);
+        const Relax<T> rA = make_relax<T>(c, 0), rB = make_relax<T>(c, 1);
+        T *psiA = at<T>(c, c->lay.psi[0]), *psiB = psiA + c->g.N, *up = at<T>(c, c->lay.up);
+        for (int t = 0; t < n; t++) {
+            sc_fields_split_kernel<L, T, V, I, PSI><<<l.grid, l.block, 0, c->stream>>>(
+                c->g, type_or_null(c), link(c), src(c, 0), src(c, 1), psiA, psiB, up, rA.inv_tau, rB.inv_tau);
+            if (int rc = check_launch(c, "sc_fields_split_kernel")) return rc;
+            sc_collide_split_kernel<L, T, V, I, PSI, FS><<<l.grid, l.block, 0, c->stream>>>(
+                c->g, type_or_null(c), link(c), src(c, 0), dst(c, 0), psiB, up, rA, T(c->p.sc_G));
+            if (int rc = check_launch(c, "sc_collide_split_kernel")) return rc;
+            sc_collide_split_kernel<L, T, V, I, PSI, FS><<<l.grid, l.block, 0, c->stream>>>(
+                c->g, type_or_null(c), link(c), src(c, 1), dst(c, 1), psiA, up, rB, T(c->p.sc_G));
+            if (int rc = check_launch(c, "sc_collide_split_kernel")) return rc;
+            c->cur ^= 1;
+            c->steps++;
+        }
+        return LBM_OK;
+    }
+    template <int V, int PSI> static int step_sc_split_v(lbm_ctx *c, int n) {
+        if (c->p.force_scheme == LBM_FORCE_EDM)
+            return c->idx32 ? step_sc_split_vi<V, uint32_t, PSI, FORCE_EDM>(c, n) : step_sc_split_vi<V, int64_t, PSI, FORCE_EDM>(c, n);
+        return c->idx32 ? step_sc_split_vi<V, uint32_t, PSI, FORCE_GUO>(c, n) : step_sc_split_vi<V, int64_t, PSI, FORCE_GUO>(c, n);
+    }
+
     template <int PSI> static int step_sc(lbm_ctx *c, int n) {
+        if (c->sc_split > 0 && !c->aa) {
+            if constexpr (sizeof(T) == 4) {
+                if (c->sc_split == 4) return step_sc_split_v<4, PSI>(c, n);
+            }
+            if (c->sc_split == 2) return step_sc_split_v<2, PSI>(c, n);
+            return step_sc_split_v<1, PSI>(c, n);
+        }
         if constexpr (sizeof(T) == 4) {  // fp64 with two components and V = 2 would spill
             if (c->vec >= 2 && !c->aa) return step_sc_v<2, PSI>(c, n);
         }

@@ -12,7 +12,9 @@ from paper_1311_2404_b200 import workloads as W
 
 pytestmark = pytest.mark.gpu
 
-ENVS = [dict(LBM_TUNING="1", LBM_VEC=v, LBM_IDX64=i, LBM_ROWS=r, LBM_NO_GRAPH=g, LBM_NO_RESIDENT=g)
+# the Shan-Chen variant (split per-component collide kernels | one monolithic kernel) rides on the LBM_ROWS axis
+ENVS = [dict(LBM_TUNING="1", LBM_VEC=v, LBM_IDX64=i, LBM_ROWS=r, LBM_NO_GRAPH=g, LBM_NO_RESIDENT=g,
+             LBM_SC_SPLIT="1" if r == "0" else "0", LBM_SC_FIELDS_VEC="2" if g == "1" else "1")
         for v, i, r, g in itertools.product(("1", "2", "4"), ("0", "1"), ("0", "3"), ("0", "1"))]
 
 
@@ -47,6 +49,8 @@ def test_forced_variant_matches_oracle(orc, monkeypatch, env):
             d = sim.dispatch()
             assert d["index_bits"] == (64 if env["LBM_IDX64"] == "1" else 32)
             assert (d["graph_replay"] == 0) == (env["LBM_NO_GRAPH"] == "1")
+            if w.model == W.SC2:
+                assert d["sc_split"] == (1 if env["LBM_SC_SPLIT"] == "1" and store == B.LBM_STORE_AB else 0)
             if w.model != W.SC2:
                 if int(env["LBM_VEC"]) <= (4 if w.precision == W.F32 else 2):   # a width the precision has no pack for is ignored
                     assert d["nodes_per_thread"] == int(env["LBM_VEC"])
