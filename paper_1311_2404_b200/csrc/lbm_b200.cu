@@ -208,7 +208,7 @@ LBM_API int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, voi
     c->aa = p->store == LBM_STORE_AA;
     c->idx32 = (double)Q * (double)c->g.N < 4294967296.0 && !env_int("LBM_IDX64", 0, 0, 1);
     c->rows = 0;
-    c->sc_split = (p->model == LBM_SC2 && env_int("LBM_SC_SPLIT", 1, 0, 1)) ? pick_vec(p, 0.0, true) : 0;
+    c->sc_split = (p->model == LBM_SC2 && (env_int("LBM_SC_SPLIT", 1, 0, 1) || p->store == LBM_STORE_AA)) ? pick_vec(p, 0.0, true) : 0;
     c->all_bulk = true;  // the geometry starts all-FLUID
     c->span_bx = env_int("LBM_SPAN_BX", 0, 32, 256) / 32 * 32;
     c->sc_fields_vec = env_int("LBM_SC_FIELDS_VEC", 1, 1, 2);
@@ -409,9 +409,9 @@ LBM_API int lbm_get_counters(const lbm_ctx *c, int64_t *steps, int64_t *launches
 LBM_API int lbm_get_dispatch(const lbm_ctx *c, lbm_dispatch *out) {
     CHECK_CTX(c);
     if (!out) return LBM_EINVAL;
-    out->nodes_per_thread = c->p.model == LBM_SC2 ? ((c->sc_split && !c->aa) ? c->sc_split : (c->vec >= 2 && !c->aa && c->rs == 4) ? 2 : 1) : c->vec;
+    out->nodes_per_thread = c->p.model == LBM_SC2 ? (c->sc_split ? c->sc_split : (c->vec >= 2 && c->rs == 4) ? 2 : 1) : c->vec;
     out->reserved_ = 0;
-    out->sc_split = c->p.model == LBM_SC2 && c->sc_split && !c->aa;
+    out->sc_split = c->p.model == LBM_SC2 && c->sc_split;
     out->index_bits = c->idx32 ? 32 : 64;
     out->graph_replay = (c->use_graph && !c->no_graph) ? GRAPH_STEPS : 0;
     out->resident_nodes_per_cta = (c->resident_slog2 > 0 && c->resident_state >= 0) ? 1 << c->resident_slog2 : 0;

@@ -128,11 +128,11 @@ namespace {
 struct Launch { dim3 grid, block; };
 
 // Step kernels: V nodes per thread along x, 2-D blocks (bx packs) x (by rows).
-Launch span_launch(const lbm_ctx *c, int V) {
+Launch span_launch(const lbm_ctx *c, int V, int max_threads = 256) {
     const int nxv = c->g.nx / V;
     int bx = nxv > 32 ? 64 : 32;
-    if (c->span_bx > 0) bx = c->span_bx;
-    int by = c->block_threads / bx;
+    if (c->span_bx > 0 && c->span_bx <= max_threads) bx = c->span_bx;
+    int by = (c->block_threads < max_threads ? c->block_threads : max_threads) / bx;
     if (by < 1) by = 1;
     while (by > 1 && by / 2 >= c->g.ny) by /= 2;
     Launch l;

@@ -607,26 +607,175 @@ aa_even_kernel(Geom g, const uint8_t *__restrict__ type, T *f, Relax<T> rp) {
     }
 }
 
-template <class L, typename T, typename I, int MODEL, int FORCE>
-__global__ void __launch_bounds__(256)
-aa_odd_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restrict__ link, T *f, Relax<T> rp) {
-    Span s;
-    if (!thread_span<1>(g, s)) return;
-    const int n = s.row + s.x0;
-    const uint8_t t = type[n];
-    if (t & NODE_SOLID) return;
-    const uint32_t w = (t & NODE_LINKS) ? __ldg(link + n) : 0u;
-    const Nbr o = neighbours(g, s.x0, s.y, s.z);
-    I slot[L::Q];
-    T h[L::Q];
+// ---- odd AA step with V-node packs --------------------------------------------------------------
+// Packs whose nodes are all wet with no SOLID pull source ("plain") move whole vectors: the reads are
+// the pull of step_kernel from the opposite planes (aligned vector + one scalar for e_x = +-1); the
+// writes go to (i, x + e_i), which for e_x = +-1 is the pack's own aligned vector shifted by one node:
+// the element that falls on the pack's first (last) column comes from the left (right) neighbour
+// thread through shared memory, so that every thread still issues one aligned 16-byte store per plane;
+// only the first / last thread of a block row stores its edge elements one by one.  A thread that
+// writes on behalf of its neighbour does so after the barrier, i.e. after the neighbour's collision and
+// hence after the neighbour has read that slot: the in-place update stays race-free.  Other packs (a SOLID
+// node, a reflected link) take the one-node-at-a-time path with link-dependent slots (aa_slot).
+template <int V> __device__ __forceinline__ bool pack_plain(uint32_t types) { return (types & (PACK_SOLID | PACK_LINKS)) == 0; }
+
+__device__ __forceinline__ Nbr span_node_neighbours(const Geom &g, const Span &s, int k) {
+    Nbr o = s.o;
+    const int x = s.x0 + k;
+    o.xm = (x == 0) ? (g.nx - 1) : -1;
+    o.xp = (x == g.nx - 1) ? -(g.nx - 1) : 1;
+    return o;
+}
+
+template <int V> __device__ __forceinline__ bool thread_span_all(const Geom &g, Span &s) {
+    s.x0 = (blockIdx.x * blockDim.x + threadIdx.x) * V;
+    s.y = blockIdx.y * blockDim.y + threadIdx.y;
+    s.z = blockIdx.z;
+    const bool valid = s.x0 < g.nx && s.y < g.ny;
+    const int y = valid ? s.y : 0;
+    s.row = (s.z * g.ny + y) * g.nx;
+    s.xm = (s.x0 == 0) ? g.nx - 1 : s.x0 - 1;
+    s.xp = (s.x0 + V == g.nx) ? 0 : s.x0 + V;
+    s.o = neighbours(g, 1, y, s.z);
+    return valid;
+}
+
+// f_i(x, t) before an odd step: slot (ibar, x - e_i), or the node's own (i, x) for a reflected link.
+template <class L, typename T, int V, typename I>
+__device__ __forceinline__ void aa_gather_odd_span(const T *f, const Geom &g, const Span &s, uint32_t types,
+                                                   const uint32_t *__restrict__ link, T (&h)[V][L::Q]) {
+    const int64_t N = g.N;
+    if (pack_plain<V>(types)) {
+#pragma unroll
+        for (int i = 0; i < L::Q; i++) {
+            const int r = s.row + shift_yz<L>(i, -1, s.o);
+            const I plane = I(L::opp(i)) * I(N);
+            if (L::ex(i) == 0) {
+                T a[V];
+                Pack<T, V>::ldp(f + (plane + I(r + s.x0)), a);
+#pragma unroll
+                for (int k = 0; k < V; k++) h[k][i] = a[k];
+            } else if (L::ex(i) == 1) {
+                h[0][i] = f[plane + I(r + s.xm)];
+                if (V > 1) {
+                    T a[V];
+                    Pack<T, V>::ldp(f + (plane + I(r + s.x0)), a);
+#pragma unroll
+                    for (int k = 1; k < V; k++) h[k][i] = a[k - 1];
+                }
+            } else {
+                h[V - 1][i] = f[plane + I(r + s.xp)];
+                if (V > 1) {
+                    T a[V];
+                    Pack<T, V>::ldp(f + (plane + I(r + s.x0)), a);
+#pragma unroll
+                    for (int k = 0; k < V - 1; k++) h[k][i] = a[k + 1];
+                }
+            }
+        }
+    } else {
+#pragma unroll
+        for (int k = 0; k < V; k++) {
+            const uint32_t t = (types >> (8 * k)) & 0xffu;
+            const int n = s.row + s.x0 + k;
+            const uint32_t w = (t & NODE_LINKS) ? __ldg(link + n) : 0u;
+            const Nbr o = span_node_neighbours(g, s, k);
+#pragma unroll
+            for (int i = 0; i < L::Q; i++) h[k][i] = (t & NODE_SOLID) ? T(0) : f[aa_slot<L, I>(1, i, n, N, o, w)];
+        }
+    }
+}
+
+// h*_i(x) after an odd step: slot (i, x + e_i), or (ibar, x) when x + e_i is SOLID.  Called by EVERY
+// thread of the block (`live` = the thread has nodes to write): edge elements travel through shared memory.
+constexpr int AA_MAX_BLOCK = 128;  // threads per block of the odd-step AA kernels (lbm_steps.cuh clamps the launch)
+template <class L> __device__ __forceinline__ constexpr int edge_slot(int i) {  // rank of link i among those with e_x != 0
+    int e = 0;
+    for (int j = 1; j < i; j++) e += L::ex(j) != 0;
+    return e;
+}
+template <class L> __device__ __forceinline__ constexpr int edge_count() { return edge_slot<L>(L::Q); }
+
+template <class L, typename T, int V, typename I>
+__device__ __forceinline__ void aa_scatter_odd_span(T *f, const Geom &g, const Span &s, uint32_t types, bool live,
+                                                    const uint32_t *__restrict__ link, const T (&h)[V][L::Q]) {
+    __shared__ T edge[edge_count<L>()][AA_MAX_BLOCK];
+    __shared__ uint8_t plain_of[AA_MAX_BLOCK];
+    const int64_t N = g.N;
+    const int tid = threadIdx.y * blockDim.x + threadIdx.x;
+    const bool plain = live && pack_plain<V>(types);
+#pragma unroll
+    for (int i = 1; i < L::Q; i++) {  // what the neighbour thread stores on this thread's behalf
+        if (L::ex(i) == 1) edge[edge_slot<L>(i)][tid] = h[V - 1][i];
+        else if (L::ex(i) == -1) edge[edge_slot<L>(i)][tid] = h[0][i];
+    }
+    plain_of[tid] = plain;
+    __syncthreads();
+    const bool has_left = threadIdx.x > 0, has_right = threadIdx.x + 1 < blockDim.x && s.x0 + V < g.nx;
+    const bool left_plain = has_left && plain_of[tid - 1], right_plain = has_right && plain_of[tid + 1];
 #pragma unroll
     for (int i = 0; i < L::Q; i++) {
-        slot[i] = aa_slot<L, I>(1, i, n, g.N, o, w);
-        h[i] = f[slot[i]];
-    }
-    update_typed<L, T, MODEL, FORCE>(h, t, rp);
+        if (!plain) break;
+        const int r = s.row + shift_yz<L>(i, +1, s.o);
+        const I plane = I(i) * I(N);
+        if (L::ex(i) == 0) {
+            T a[V];
 #pragma unroll
-    for (int i = 0; i < L::Q; i++) f[slot[L::opp(i)]] = h[i];
+            for (int k = 0; k < V; k++) a[k] = h[k][i];
+            Pack<T, V>::stp(f + (plane + I(r + s.x0)), a);
+        } else if (L::ex(i) == 1) {  // targets x0 + 1 .. x0 + V
+            if (has_left) {
+                T a[V];
+                a[0] = edge[edge_slot<L>(i)][tid - 1];
+#pragma unroll
+                for (int k = 1; k < V; k++) a[k] = h[k - 1][i];
+                Pack<T, V>::stp(f + (plane + I(r + s.x0)), a);
+            } else {
+#pragma unroll
+                for (int k = 1; k < V; k++) f[plane + I(r + s.x0 + k)] = h[k - 1][i];
+            }
+            if (!right_plain) f[plane + I(r + s.xp)] = h[V - 1][i];
+        } else {  // targets x0 - 1 .. x0 + V - 2
+            if (has_right) {
+                T a[V];
+#pragma unroll
+                for (int k = 0; k < V - 1; k++) a[k] = h[k + 1][i];
+                a[V - 1] = edge[edge_slot<L>(i)][tid + 1];
+                Pack<T, V>::stp(f + (plane + I(r + s.x0)), a);
+            } else {
+#pragma unroll
+                for (int k = 0; k < V - 1; k++) f[plane + I(r + s.x0 + k)] = h[k + 1][i];
+            }
+            if (!left_plain) f[plane + I(r + s.xm)] = h[0][i];
+        }
+    }
+    if (live && !plain) {
+#pragma unroll
+        for (int k = 0; k < V; k++) {
+            const uint32_t t = (types >> (8 * k)) & 0xffu;
+            if (t & NODE_SOLID) continue;
+            const int n = s.row + s.x0 + k;
+            const uint32_t w = (t & NODE_LINKS) ? __ldg(link + n) : 0u;
+            const Nbr o = span_node_neighbours(g, s, k);
+#pragma unroll
+            for (int i = 0; i < L::Q; i++) f[aa_slot<L, I>(1, L::opp(i), n, N, o, w)] = h[k][i];  // where the read of ibar came from
+        }
+    }
+}
+
+template <class L, typename T, int V, typename I, int MODEL, int FORCE>
+__global__ void __launch_bounds__(AA_MAX_BLOCK)
+aa_odd_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restrict__ link, T *f, Relax<T> rp) {
+    Span s;
+    const bool valid = thread_span_all<V>(g, s);
+    const uint32_t types = valid ? load_types<V>(type, s.row + s.x0) : PACK_SOLID;
+    const bool live = valid && !all_solid<V>(types);
+    T h[V][L::Q];
+    if (live) {
+        aa_gather_odd_span<L, T, V, I>(f, g, s, types, link, h);
+        update_span<L, T, V, MODEL, FORCE>(h, types, rp);
+    }
+    aa_scatter_odd_span<L, T, V, I>(f, g, s, types, live, link, h);
 }
 
 // Conversions for the AA store (parity 0: before an even step, 1: before an odd step).
@@ -1022,30 +1171,11 @@ __device__ __forceinline__ void field_gradient_span(const T *__restrict__ psi, c
         for (int c = 0; c < 3; c++) S[k][c] = wd * (ratio * ax[k][c] + dg[k][c]);
 }
 
-template <class L, typename T, int V, typename I, int PSI, int FS>
-__global__ void __launch_bounds__(256)
-sc_collide_split_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restrict__ link,
-                        const T *__restrict__ src, T *__restrict__ dst, const T *__restrict__ psi_other,
-                        const T *__restrict__ up, Relax<T> rp, T G) {
-    Span s;
-    if (!thread_span<V>(g, s)) return;
-    const int n0 = s.row + s.x0;
-    const uint32_t types = load_types<V>(type, n0);
-    if (all_solid<V>(types)) return;
-    T h[V][L::Q];
-    gather_span<L, T, V, I>(src, g.N, s, h);
-    T u[3][V];
-#pragma unroll
-    for (int a = 0; a < 3; a++) {
-        if (a < L::D) Pack<T, V>::ldp(up + ((int64_t)a * g.N + n0), u[a]);
-        else {
-#pragma unroll
-            for (int k = 0; k < V; k++) u[a][k] = T(0);
-        }
-    }
-    T S[V][3];
-    field_gradient_span<L, T, V>(psi_other, s, S);
-    pull_reflected_span<L, T, V, I>(src, g.N, n0, types, link, h);
+// One component's collision for the V nodes of a pack: S = gradient sum of the OTHER component's psi,
+// u = common velocity u' (component planes).  Node types FULLWAY / VELOCITY replace the collision.
+template <class L, typename T, int V, int PSI, int FS>
+__device__ __forceinline__ void sc_component_update_span(T (&h)[V][L::Q], uint32_t types, const T (&S)[V][3],
+                                                         const T (&u)[3][V], const Relax<T> &rp, T G) {
 #pragma unroll
     for (int k = 0; k < V; k++) {
         const uint32_t t = (types >> (8 * k)) & 0xffu;
@@ -1065,60 +1195,133 @@ sc_collide_split_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t
             collide<L, T, MODEL_BGK, FS>(h[k], r, d, v, m, F, rp);
         }
     }
+}
+
+template <class L, typename T, int V>
+__device__ __forceinline__ void load_common_velocity(const T *__restrict__ up, int64_t N, int n0, T (&u)[3][V]) {
+#pragma unroll
+    for (int a = 0; a < 3; a++) {
+        if (a < L::D) Pack<T, V>::ldp(up + ((int64_t)a * N + n0), u[a]);
+        else {
+#pragma unroll
+            for (int k = 0; k < V; k++) u[a][k] = T(0);
+        }
+    }
+}
+
+template <class L, typename T, int V, typename I, int PSI, int FS>
+__global__ void __launch_bounds__(256)
+sc_collide_split_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restrict__ link,
+                        const T *__restrict__ src, T *__restrict__ dst, const T *__restrict__ psi_other,
+                        const T *__restrict__ up, Relax<T> rp, T G) {
+    Span s;
+    if (!thread_span<V>(g, s)) return;
+    const int n0 = s.row + s.x0;
+    const uint32_t types = load_types<V>(type, n0);
+    if (all_solid<V>(types)) return;
+    T h[V][L::Q];
+    gather_span<L, T, V, I>(src, g.N, s, h);
+    T u[3][V];
+    load_common_velocity<L, T, V>(up, g.N, n0, u);
+    T S[V][3];
+    field_gradient_span<L, T, V>(psi_other, s, S);
+    pull_reflected_span<L, T, V, I>(src, g.N, n0, types, link, h);
+    sc_component_update_span<L, T, V, PSI, FS>(h, types, S, u, rp, G);
     store_span<L, T, V, I>(dst, g.N, n0, h);
 }
 
-// ---- Shan-Chen on the in-place AA store: one node per thread, both parities (see aa_slot) ------
-template <class L, typename T, typename I, int PSI>
-__global__ void __launch_bounds__(256)
-aa_sc_fields_kernel(Geom g, int parity, const uint8_t *__restrict__ type, const uint32_t *__restrict__ link,
-                    const T *fA, const T *fB, typename Pair<T>::type *__restrict__ psi) {
-    Span s;
-    if (!thread_span<1>(g, s)) return;
-    const int n = s.row + s.x0;
-    const uint8_t t = type[n];
-    typename Pair<T>::type p;
-    p.x = p.y = -psi_one<T, PSI>();  // dry nodes: psi = 0 (A14)
-    if (!(t & (NODE_SOLID | NODE_FULLWAY))) {
-        const uint32_t w = (t & NODE_LINKS) ? __ldg(link + n) : 0u;
-        const Nbr o = neighbours(g, s.x0, s.y, s.z);
-        T sA = T(0), sB = T(0);
+// ---- Shan-Chen on the in-place AA store: the split variant on both parities ---------------------
+// Pass 1 reads f_A, f_B where the current parity keeps them (even: (i, x); odd: see aa_gather_odd_span)
+// and writes psi_A, psi_B, u'; pass 2 is the AA even / odd step of ONE component with the coupling force.
+template <class L, typename T, int V, typename I>
+__device__ __forceinline__ void aa_gather_span(int parity, const T *f, const Geom &g, const Span &s, uint32_t types,
+                                               const uint32_t *__restrict__ link, T (&h)[V][L::Q]) {
+    if (parity == 0) {
 #pragma unroll
         for (int i = 0; i < L::Q; i++) {
-            const I sl = aa_slot<L, I>(parity, i, n, g.N, o, w);
-            sA += fA[sl];
-            sB += fB[sl];
+            T a[V];
+            Pack<T, V>::ldp(f + (I(i) * I(g.N) + I(s.row + s.x0)), a);
+#pragma unroll
+            for (int k = 0; k < V; k++) h[k][i] = a[k];
         }
-        p.x = psi_dev<T, PSI>(sA);
-        p.y = psi_dev<T, PSI>(sB);
+    } else {
+        aa_gather_odd_span<L, T, V, I>(f, g, s, types, link, h);
     }
-    psi[n] = p;
 }
 
-template <class L, typename T, typename I, int PSI, int FS>
+template <class L, typename T, int V, typename I, int PSI>
 __global__ void __launch_bounds__(256)
-aa_sc_step_kernel(Geom g, int parity, const uint8_t *__restrict__ type, const uint32_t *__restrict__ link, T *fA,
-                  T *fB, const typename Pair<T>::type *__restrict__ psi, Relax<T> rpA, Relax<T> rpB, T G) {
+aa_sc_fields_split_kernel(Geom g, int parity, const uint8_t *__restrict__ type, const uint32_t *__restrict__ link,
+                          const T *fA, const T *fB, T *__restrict__ psiA, T *__restrict__ psiB, T *__restrict__ up,
+                          T inv_tauA, T inv_tauB) {
     Span s;
-    if (!thread_span<1>(g, s)) return;
-    const int n = s.row + s.x0;
-    const uint8_t t = type[n];
-    if (t & NODE_SOLID) return;
-    const uint32_t w = (t & NODE_LINKS) ? __ldg(link + n) : 0u;
-    const Nbr o = neighbours(g, s.x0, s.y, s.z);
-    I slot[L::Q];
-    T hA[L::Q], hB[L::Q];
+    if (!thread_span<V>(g, s)) return;
+    const int n0 = s.row + s.x0;
+    const uint32_t types = load_types<V>(type, n0);
+    T pa[V], pb[V], u[3][V];
 #pragma unroll
-    for (int i = 0; i < L::Q; i++) {
-        slot[i] = aa_slot<L, I>(parity, i, n, g.N, o, w);
-        hA[i] = fA[slot[i]];
-        hB[i] = fB[slot[i]];
+    for (int k = 0; k < V; k++) { pa[k] = pb[k] = -psi_one<T, PSI>(); u[0][k] = u[1][k] = u[2][k] = T(0); }
+    if (!all_solid<V>(types)) {
+        T h[V][L::Q], rA[V], jA[V][3];
+        aa_gather_span<L, T, V, I>(parity, fA, g, s, types, link, h);
+#pragma unroll
+        for (int k = 0; k < V; k++) {
+            T d;
+            moments<L, T>(h[k], d, jA[k]);
+            rA[k] = T(1) + d;
+            pa[k] = psi_dev<T, PSI>(d);
+        }
+        aa_gather_span<L, T, V, I>(parity, fB, g, s, types, link, h);
+#pragma unroll
+        for (int k = 0; k < V; k++) {
+            T d, jB[3];
+            moments<L, T>(h[k], d, jB);
+            const T rB = T(1) + d;
+            pb[k] = psi_dev<T, PSI>(d);
+            const T inv_den = T(1) / (rA[k] * inv_tauA + rB * inv_tauB);
+#pragma unroll
+            for (int a = 0; a < 3; a++) u[a][k] = (jA[k][a] * inv_tauA + jB[a] * inv_tauB) * inv_den;
+            if ((types >> (8 * k)) & (NODE_SOLID | NODE_FULLWAY)) {
+                pa[k] = pb[k] = -psi_one<T, PSI>();
+                u[0][k] = u[1][k] = u[2][k] = T(0);
+            }
+        }
     }
-    sc_collide_node<L, T, PSI, FS>(hA, hB, t, psi, n, o, rpA, rpB, G);
+    Pack<T, V>::stp(psiA + n0, pa);
+    Pack<T, V>::stp(psiB + n0, pb);
 #pragma unroll
-    for (int i = 0; i < L::Q; i++) {  // the slot the read of ibar came from (even: (ibar, x); odd: (i, x + e_i) ...)
-        fA[slot[L::opp(i)]] = hA[i];
-        fB[slot[L::opp(i)]] = hB[i];
+    for (int a = 0; a < L::D; a++) Pack<T, V>::stp(up + ((int64_t)a * g.N + n0), u[a]);
+}
+
+template <class L, typename T, int V, typename I, int PSI, int FS>
+__global__ void __launch_bounds__(AA_MAX_BLOCK)
+aa_sc_collide_split_kernel(Geom g, int parity, const uint8_t *__restrict__ type, const uint32_t *__restrict__ link, T *f,
+                           const T *__restrict__ psi_other, const T *__restrict__ up, Relax<T> rp, T G) {
+    Span s;
+    const bool valid = thread_span_all<V>(g, s);
+    const int n0 = s.row + s.x0;
+    const uint32_t types = valid ? load_types<V>(type, n0) : PACK_SOLID;
+    const bool live = valid && !all_solid<V>(types);
+    T h[V][L::Q];
+    if (live) {
+        aa_gather_span<L, T, V, I>(parity, f, g, s, types, link, h);
+        T u[3][V], S[V][3];
+        load_common_velocity<L, T, V>(up, g.N, n0, u);
+        field_gradient_span<L, T, V>(psi_other, s, S);
+        sc_component_update_span<L, T, V, PSI, FS>(h, types, S, u, rp, G);
+    }
+    if (parity == 0) {  // even: local, h*_i to (ibar, x)
+        if (live) {
+#pragma unroll
+            for (int i = 0; i < L::Q; i++) {
+                T a[V];
+#pragma unroll
+                for (int k = 0; k < V; k++) a[k] = h[k][i];
+                Pack<T, V>::stp(f + (I(L::opp(i)) * I(g.N) + I(n0)), a);
+            }
+        }
+    } else {
+        aa_scatter_odd_span<L, T, V, I>(f, g, s, types, live, link, h);
     }
 }
 

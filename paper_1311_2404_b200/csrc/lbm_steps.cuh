@@ -18,13 +18,12 @@ template <class L, typename T> struct Steps {
     }
 
     template <int V, typename I, int MODEL, int FORCE> static int step_single_vi(lbm_ctx *c, int n, const Relax<T> &rp) {
-        const Launch l = span_launch(c, V);
-        if (c->aa) {  // in place: even steps are local (V-node packs), odd steps move data (one node per thread)
-            const Launch l1 = span_launch(c, 1);
+        const Launch l = span_launch(c, V, c->aa ? AA_MAX_BLOCK : 256);
+        if (c->aa) {  // in place: even steps are local, odd steps move data; V-node packs on both
             T *f = at<T>(c, c->lay.store[0][0]);
             for (int t = 0; t < n; t++) {
                 if (c->cur == 0) aa_even_kernel<L, T, V, I, MODEL, FORCE><<<l.grid, l.block, 0, c->stream>>>(c->g, type_or_null(c), f, rp);
-                else aa_odd_kernel<L, T, I, MODEL, FORCE><<<l1.grid, l1.block, 0, c->stream>>>(c->g, type(c), link(c), f, rp);
+                else aa_odd_kernel<L, T, V, I, MODEL, FORCE><<<l.grid, l.block, 0, c->stream>>>(c->g, type_or_null(c), link(c), f, rp);
                 if (int rc = check_launch(c, "aa_step_kernel")) return rc;
                 c->cur ^= 1;
                 c->steps++;
@@ -129,22 +128,6 @@ template <class L, typename T> struct Steps {
         const Launch l = span_launch(c, V), lf = span_launch(c, VF);
         const Relax<T> rA = make_relax<T>(c, 0), rB = make_relax<T>(c, 1);
         auto *psi = at<typename Pair<T>::type>(c, c->lay.psi[0]);
-        if (c->aa) {  // in place: one node per thread, `cur` is the parity
-            if constexpr (V != 1) return fail(c, LBM_EUNSUPPORTED, "internal: AA Shan-Chen runs one node per thread");
-            else {
-                T *fA = at<T>(c, c->lay.store[0][0]), *fB = at<T>(c, c->lay.store[1][0]);
-                for (int t = 0; t < n; t++) {
-                    aa_sc_fields_kernel<L, T, I, PSI><<<l.grid, l.block, 0, c->stream>>>(c->g, c->cur, type(c), link(c), fA, fB, psi);
-                    if (int rc = check_launch(c, "aa_sc_fields_kernel")) return rc;
-                    aa_sc_step_kernel<L, T, I, PSI, FS><<<l.grid, l.block, 0, c->stream>>>(
-                        c->g, c->cur, type(c), link(c), fA, fB, psi, rA, rB, T(c->p.sc_G));
-                    if (int rc = check_launch(c, "aa_sc_step_kernel")) return rc;
-                    c->cur ^= 1;
-                    c->steps++;
-                }
-                return LBM_OK;
-            }
-        }
         for (int t = 0; t < n; t++) {
             sc_fields_kernel<L, T, VF, I, PSI><<<lf.grid, lf.block, 0, c->stream>>>(c->g, type_or_null(c), link(c), src(c, 0), src(c, 1), psi);
             if (int rc = check_launch(c, "sc_fields_kernel")) return rc;
@@ -159,9 +142,26 @@ template <class L, typename T> struct Steps {
 
     // Split variant: one macro-field pass (psi_A, psi_B, u') + one collide pass per component.
     template <int V, typename I, int PSI, int FS> static int step_sc_split_vi(lbm_ctx *c, int n) {
-        const Launch l = span_launch(c, V);
+        const Launch l = span_launch(c, V, c->aa ? AA_MAX_BLOCK : 256);
         const Relax<T> rA = make_relax<T>(c, 0), rB = make_relax<T>(c, 1);
         T *psiA = at<T>(c, c->lay.psi[0]), *psiB = psiA + c->g.N, *up = at<T>(c, c->lay.up);
+        if (c->aa) {  // in place: `cur` is the parity
+            T *fA = at<T>(c, c->lay.store[0][0]), *fB = at<T>(c, c->lay.store[1][0]);
+            for (int t = 0; t < n; t++) {
+                aa_sc_fields_split_kernel<L, T, V, I, PSI><<<l.grid, l.block, 0, c->stream>>>(
+                    c->g, c->cur, type_or_null(c), link(c), fA, fB, psiA, psiB, up, rA.inv_tau, rB.inv_tau);
+                if (int rc = check_launch(c, "aa_sc_fields_split_kernel")) return rc;
+                aa_sc_collide_split_kernel<L, T, V, I, PSI, FS><<<l.grid, l.block, 0, c->stream>>>(
+                    c->g, c->cur, type_or_null(c), link(c), fA, psiB, up, rA, T(c->p.sc_G));
+                if (int rc = check_launch(c, "aa_sc_collide_split_kernel")) return rc;
+                aa_sc_collide_split_kernel<L, T, V, I, PSI, FS><<<l.grid, l.block, 0, c->stream>>>(
+                    c->g, c->cur, type_or_null(c), link(c), fB, psiA, up, rB, T(c->p.sc_G));
+                if (int rc = check_launch(c, "aa_sc_collide_split_kernel")) return rc;
+                c->cur ^= 1;
+                c->steps++;
+            }
+            return LBM_OK;
+        }
         for (int t = 0; t < n; t++) {
             sc_fields_split_kernel<L, T, V, I, PSI><<<l.grid, l.block, 0, c->stream>>>(
                 c->g, type_or_null(c), link(c), src(c, 0), src(c, 1), psiA, psiB, up, rA.inv_tau, rB.inv_tau);
@@ -184,11 +184,11 @@ template <class L, typename T> struct Steps {
     }
 
     template <int PSI> static int step_sc(lbm_ctx *c, int n) {
-        if (c->sc_split > 0 && !c->aa) {
+        if (c->sc_split > 0 || c->aa) {  // the in-place store has the split variant only
             if constexpr (sizeof(T) == 4) {
                 if (c->sc_split == 4) return step_sc_split_v<4, PSI>(c, n);
             }
-            if (c->sc_split == 2) return step_sc_split_v<2, PSI>(c, n);
+            if (c->sc_split == 2 || (c->sc_split == 4 && sizeof(T) == 8)) return step_sc_split_v<2, PSI>(c, n);
             return step_sc_split_v<1, PSI>(c, n);
         }
         if constexpr (sizeof(T) == 4) {  // fp64 with two components and V = 2 would spill

@@ -50,7 +50,7 @@ def test_forced_variant_matches_oracle(orc, monkeypatch, env):
             assert d["index_bits"] == (64 if env["LBM_IDX64"] == "1" else 32)
             assert (d["graph_replay"] == 0) == (env["LBM_NO_GRAPH"] == "1")
             if w.model == W.SC2:
-                assert d["sc_split"] == (1 if env["LBM_SC_SPLIT"] == "1" and store == B.LBM_STORE_AB else 0)
+                assert d["sc_split"] == (1 if env["LBM_SC_SPLIT"] == "1" or store == B.LBM_STORE_AA else 0)  # in place: split only
             if w.model != W.SC2:
                 if int(env["LBM_VEC"]) <= (4 if w.precision == W.F32 else 2):   # a width the precision has no pack for is ignored
                     assert d["nodes_per_thread"] == int(env["LBM_VEC"])
