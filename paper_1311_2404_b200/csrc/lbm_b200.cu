@@ -206,9 +206,18 @@ LBM_API int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, voi
     c->block_x = pick_block_x(p->nx);
     c->vec = pick_vec(p, 0.0);
     c->aa = p->store == LBM_STORE_AA;
-    c->idx32 = (double)Q * (double)c->g.N < 4294967296.0 && !env_int("LBM_IDX64", 0, 0, 1);
+    // slot numbers i * N + node: 32 bits whenever Q * N < 2^32; the 64-bit kernels exist for the AB store of
+    // D3Q19 LBGK / MRT / (split) Shan-Chen, which is what a lattice of that size (> 226 M nodes) would run
+    const bool idx64_built = p->lattice == LBM_D3Q19 && p->store == LBM_STORE_AB &&
+                             (p->model == LBM_BGK || p->model == LBM_MRT || p->model == LBM_SC2);
+    c->idx32 = (double)Q * (double)c->g.N < 4294967296.0;
+    if (!c->idx32 && !idx64_built) {
+        delete c;
+        return fail(nullptr, LBM_EUNSUPPORTED, "Q*nx*ny*nz >= 2^32 is built for D3Q19 with the AB store and LBM_BGK / LBM_MRT / LBM_SC2 only");
+    }
+    if (idx64_built && env_int("LBM_IDX64", 0, 0, 1)) c->idx32 = false;
     c->rows = 0;
-    c->sc_split = (p->model == LBM_SC2 && (env_int("LBM_SC_SPLIT", 1, 0, 1) || p->store == LBM_STORE_AA)) ? pick_vec(p, 0.0, true) : 0;
+    c->sc_split = (p->model == LBM_SC2 && (env_int("LBM_SC_SPLIT", 1, 0, 1) || p->store == LBM_STORE_AA || !c->idx32)) ? pick_vec(p, 0.0, true) : 0;
     c->all_bulk = true;  // the geometry starts all-FLUID
     c->span_bx = env_int("LBM_SPAN_BX", 0, 32, 256) / 32 * 32;
     c->sc_fields_vec = env_int("LBM_SC_FIELDS_VEC", 1, 1, 2);

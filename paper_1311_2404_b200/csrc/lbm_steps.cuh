@@ -14,11 +14,17 @@ template <class L, typename T> struct Steps {
     static const uint8_t *type_or_null(lbm_ctx *c) { return c->all_bulk ? nullptr : at<uint8_t>(c, c->lay.type); }
 
     template <int V, int MODEL, int FORCE> static int step_single_v(lbm_ctx *c, int n, const Relax<T> &rp) {
-        return c->idx32 ? step_single_vi<V, uint32_t, MODEL, FORCE>(c, n, rp) : step_single_vi<V, int64_t, MODEL, FORCE>(c, n, rp);
+        // 64-bit slot indices (Q * N >= 2^32: more than 226 M D3Q19 nodes) are built for the AB kernels of
+        // D3Q19 LBGK / MRT / split Shan-Chen only (lbm_create rejects other combinations at that size)
+        if constexpr (L::Q == 19 && (MODEL == MODEL_BGK || MODEL == MODEL_MRT)) {
+            if (!c->idx32) return step_single_vi<V, int64_t, MODEL, FORCE>(c, n, rp);
+        }
+        return step_single_vi<V, uint32_t, MODEL, FORCE>(c, n, rp);
     }
 
     template <int V, typename I, int MODEL, int FORCE> static int step_single_vi(lbm_ctx *c, int n, const Relax<T> &rp) {
         const Launch l = span_launch(c, V, c->aa ? AA_MAX_BLOCK : 256);
+        if constexpr (sizeof(I) == 4) {
         if (c->aa) {  // in place: even steps are local, odd steps move data; V-node packs on both
             T *f = at<T>(c, c->lay.store[0][0]);
             for (int t = 0; t < n; t++) {
@@ -29,6 +35,7 @@ template <class L, typename T> struct Steps {
                 c->steps++;
             }
             return LBM_OK;
+        }
         }
         if constexpr (V <= 2 && sizeof(I) == 4) {
             if (c->rows > 0) {  // obstacle-rich geometry: row-walking kernel, link words one row ahead
@@ -112,8 +119,8 @@ template <class L, typename T> struct Steps {
 
     template <int V, int PSI> static int step_sc_v(lbm_ctx *c, int n) {
         if (c->p.force_scheme == LBM_FORCE_EDM)
-            return c->idx32 ? step_sc_vf<V, uint32_t, PSI, FORCE_EDM>(c, n) : step_sc_vf<V, int64_t, PSI, FORCE_EDM>(c, n);
-        return c->idx32 ? step_sc_vf<V, uint32_t, PSI, FORCE_GUO>(c, n) : step_sc_vf<V, int64_t, PSI, FORCE_GUO>(c, n);
+            return step_sc_vf<V, uint32_t, PSI, FORCE_EDM>(c, n);
+        return step_sc_vf<V, uint32_t, PSI, FORCE_GUO>(c, n);
     }
 
     // VF = nodes per thread of the macro-field pass, V = of the collide pass (chosen independently)
@@ -145,6 +152,7 @@ template <class L, typename T> struct Steps {
         const Launch l = span_launch(c, V, c->aa ? AA_MAX_BLOCK : 256);
         const Relax<T> rA = make_relax<T>(c, 0), rB = make_relax<T>(c, 1);
         T *psiA = at<T>(c, c->lay.psi[0]), *psiB = psiA + c->g.N, *up = at<T>(c, c->lay.up);
+        if constexpr (sizeof(I) == 4) {
         if (c->aa) {  // in place: `cur` is the parity
             T *fA = at<T>(c, c->lay.store[0][0]), *fB = at<T>(c, c->lay.store[1][0]);
             for (int t = 0; t < n; t++) {
@@ -161,6 +169,7 @@ template <class L, typename T> struct Steps {
                 c->steps++;
             }
             return LBM_OK;
+        }
         }
         for (int t = 0; t < n; t++) {
             sc_fields_split_kernel<L, T, V, I, PSI><<<l.grid, l.block, 0, c->stream>>>(
@@ -179,8 +188,13 @@ template <class L, typename T> struct Steps {
     }
     template <int V, int PSI> static int step_sc_split_v(lbm_ctx *c, int n) {
         if (c->p.force_scheme == LBM_FORCE_EDM)
-            return c->idx32 ? step_sc_split_vi<V, uint32_t, PSI, FORCE_EDM>(c, n) : step_sc_split_vi<V, int64_t, PSI, FORCE_EDM>(c, n);
-        return c->idx32 ? step_sc_split_vi<V, uint32_t, PSI, FORCE_GUO>(c, n) : step_sc_split_vi<V, int64_t, PSI, FORCE_GUO>(c, n);
+        if constexpr (L::Q == 19) {
+            if (!c->idx32)
+                return c->p.force_scheme == LBM_FORCE_EDM ? step_sc_split_vi<V, int64_t, PSI, FORCE_EDM>(c, n)
+                                                          : step_sc_split_vi<V, int64_t, PSI, FORCE_GUO>(c, n);
+        }
+        if (c->p.force_scheme == LBM_FORCE_EDM) return step_sc_split_vi<V, uint32_t, PSI, FORCE_EDM>(c, n);
+        return step_sc_split_vi<V, uint32_t, PSI, FORCE_GUO>(c, n);
     }
 
     template <int PSI> static int step_sc(lbm_ctx *c, int n) {

@@ -47,14 +47,15 @@ def test_forced_variant_matches_oracle(orc, monkeypatch, env):
             sim.set_geometry(w.mask)
             ref.set_geometry(w.mask)
             d = sim.dispatch()
-            assert d["index_bits"] == (64 if env["LBM_IDX64"] == "1" else 32)
+            idx64 = env["LBM_IDX64"] == "1" and store == B.LBM_STORE_AB and w.model in (W.BGK, W.MRT, W.SC2)  # where built
+            assert d["index_bits"] == (64 if idx64 else 32)
             assert (d["graph_replay"] == 0) == (env["LBM_NO_GRAPH"] == "1")
             if w.model == W.SC2:
-                assert d["sc_split"] == (1 if env["LBM_SC_SPLIT"] == "1" or store == B.LBM_STORE_AA else 0)  # in place: split only
+                assert d["sc_split"] == (1 if env["LBM_SC_SPLIT"] == "1" or store == B.LBM_STORE_AA or idx64 else 0)
             if w.model != W.SC2:
                 if int(env["LBM_VEC"]) <= (4 if w.precision == W.F32 else 2):   # a width the precision has no pack for is ignored
                     assert d["nodes_per_thread"] == int(env["LBM_VEC"])
-                rows_ok = store == B.LBM_STORE_AB and env["LBM_IDX64"] == "0" and d["nodes_per_thread"] <= 2
+                rows_ok = store == B.LBM_STORE_AB and not idx64 and d["nodes_per_thread"] <= 2
                 assert d["rows_per_block"] == (int(env["LBM_ROWS"]) if rows_ok else 0)
             for s in range(w.ncomp):
                 sim.init_equilibrium(w.rho[s], w.u[s], comp=s)
