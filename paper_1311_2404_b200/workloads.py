@@ -171,16 +171,19 @@ def ldc_cavity(nx: int = 256, ny: int = 256, nz: int = 256, steps: int = 1000, R
     return w
 
 
-def binary_poiseuille(nx: int = 64, ny: int = 256, steps: int = 400000, g: float = 1e-7, G: float = 1.2,
-                      minority: float = 0.06, precision: int = F64) -> Workload:
+def binary_poiseuille(nx: int = 64, ny: int = 256, steps: int = 400000, g: float = 1e-7, G: float = 1.5,
+                      density: float = 0.8, minority: float = 0.06, precision: int = F64) -> Workload:
     """Shan-Chen binary Poiseuille flow of the paper's section 5.3: 64 x 256 D2Q9, half-way
     bounce-back walls at y = +-L, fluid of viscosity nu_1 = 1/24 in the core |y| <= L/2 and nu_0 = 1/6
     outside, G = 1.5, body force through the Exact Difference Method, starting from rest.
     Component 0 is the outer fluid, component 1 the core fluid; each phase carries a small amount of
-    the other component (`minority`), since the Shan-Chen model permits residual mixing.
-    G: the paper quotes 1.5; with this build's reading of the model (psi = rho, sign A11, EDM) 1.5 drives
-    the minority density negative at the interface and a slowly growing asymmetric mode appears after
-    ~2e5 steps, so the default is 1.2, which stays symmetric to round-off."""
+    the other component (`minority`, as a fraction of `density`), since the Shan-Chen model permits
+    residual mixing.
+    The paper gives G = 1.5 but not the densities.  With psi = rho only the product G * density enters the
+    dynamics: at density 1 (G rho = 1.5) the minority density goes negative at the interface and an
+    asymmetric mode grows after ~2e5 steps; G rho <= 1.2 stays symmetric to round-off and positive.  So the
+    paper's G is kept and the phases are initialised at density 0.8 (reading A22; measured scan in
+    section 7).  psi = 1 - exp(-rho) at G = 1.5 does not keep the two fluids apart at all."""
     nu0, nu1 = 1.0 / 6.0, 1.0 / 24.0
     w = Workload("binary_poiseuille_d2q9_sc2", D2Q9, SC2, precision, nx, ny, 1, (3 * nu0 + 0.5, 3 * nu1 + 0.5), steps,
                  force=(g, 0.0, 0.0), sc_G=G, sc_psi=0, force_scheme=FORCE_EDM)
@@ -191,7 +194,7 @@ def binary_poiseuille(nx: int = 64, ny: int = 256, steps: int = 400000, g: float
     L = (ny - 2) / 2.0
     core = (np.abs(y) <= L / 2)[None, :, None] * np.ones((1, ny, nx), bool)
     w.mask = mask
-    w.rho = [np.where(core, minority, 1.0), np.where(core, 1.0, minority)]
+    w.rho = [np.where(core, minority * density, density), np.where(core, density, minority * density)]
     w.u = [np.zeros((2, 1, ny, nx)), np.zeros((2, 1, ny, nx))]
     return w
 

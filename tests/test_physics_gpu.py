@@ -129,12 +129,13 @@ def test_poiseuille_profile_parabola_plus_constant(B):
 
 
 def test_shan_chen_binary_poiseuille(B):
-    """Section 5.3 of the paper (eq. 21), its own sizes: 64 x 256, nu_0 = 1/6 outside,
-    nu_1 = 1/24 in the core, EDM, G = 1.2 (the paper's 1.5 is marginally unstable here, see workloads.py).  The paper reports "good agreement" from a figure and
+    """Section 5.3 of the paper (eq. 21), its own sizes and parameters: 64 x 256, nu_0 = 1/6
+    outside, nu_1 = 1/24 in the core, EDM, G = 1.5 (phases at density 0.8: the paper gives no densities and with
+    psi = rho only G * density matters, reading A22).  The paper reports "good agreement" from a figure and
     computes the effective density and viscosity as rho = rho_0 + rho_1, nu rho = rho_0 nu_0 +
-    rho_1 nu_1 because the components mix a little; so the check is (a) eq. (21) within 8 % and
-    (b) the 1-D momentum balance d/dy(rho nu du/dy) = -rho g with the simulated densities within
-    4 % (measured on B200, fp64: 5.9 % and 2.2 %), plus symmetry about the centre line."""
+    rho_1 nu_1 because the components mix a little; so the check is (a) eq. (21) and (b) the 1-D momentum
+    balance d/dy(rho nu du/dy) = -rho g with the simulated densities, plus symmetry about the centre
+    line.  Bars = what the run gives on B200 in fp64 (5.90 % and 2.17 %) + 20 %."""
     w = W.binary_poiseuille()
     sim = start(B, w)
     sim.step(w.steps)
@@ -150,7 +151,7 @@ def test_shan_chen_binary_poiseuille(B):
     exact = np.where(np.abs(y) > L / 2, g / (2 * nu0) * (L * L - y * y),
                      g * L * L / 8 * (3 / nu0 + (1 - 4 * y * y / (L * L)) / nu1))
     err_exact = np.abs(ux - exact).max() / exact.max()
-    assert err_exact < 0.08, err_exact
+    assert err_exact < 0.071, err_exact
     mu = r0 * nu0 + r1 * nu1
     n = len(y)
     A = np.zeros((n, n))
@@ -167,9 +168,10 @@ def test_shan_chen_binary_poiseuille(B):
     balance = np.linalg.solve(A, -rho * g)
     err_balance = np.abs(ux - balance).max() / balance.max()
     print("binary Poiseuille: vs eq. (21) %.4f, vs 1-D momentum balance %.4f" % (err_exact, err_balance))
-    assert err_balance < 0.04, err_balance
+    assert err_balance < 0.026, err_balance
     # the two fluids stay where they were put
-    assert r1[n // 2] > 0.9 and r0[n // 2] < 0.1 and r0[3] > 0.9 and r1[3] < 0.1
+    assert r1[n // 2] > 0.72 and r0[n // 2] < 0.08 and r0[3] > 0.72 and r1[3] < 0.08   # of density 0.8
+    assert min(r0.min(), r1.min()) > 0.0
 
 
 def test_regularized_smagorinsky_and_mrt_survive_where_lbgk_diverges(B):
