@@ -145,6 +145,20 @@ int lbm_get_stream_map(lbm_ctx *ctx, int64_t *d_map);
 int lbm_run_host(lbm_ctx *ctx, const uint8_t *h_mask, const void *const *h_rho0, const void *const *h_u0,
                  int n, void *h_rho_out, void *h_u_out);
 
+/* z-slab decomposition of one lattice over several contexts (section 3.6 of the paper).
+ * Each slab is an ordinary context whose local lattice is its share of the global z-planes PLUS one ghost
+ * plane below (local z = 0) and one above (local z = nz - 1): the caller slices mask, rho0 and u0 of the
+ * global lattice accordingly (ghost planes = copies of the neighbour's boundary planes, through the
+ * periodic seam if periodic_z) and initialises every slab with the usual calls.  lbm_step_slabs then
+ * advances all slabs n steps in lockstep: after every step each ghost plane receives, from the
+ * neighbouring slab's boundary interior plane, the 5 of 19 populations that stream across the face
+ * (P:464); for LBM_SC2 the psi planes are exchanged between the macro-field pass and the collide pass.
+ * slabs[0] is the lowest slab; periodic_z != 0 also links slabs[count-1] to slabs[0].  Interior planes
+ * then hold exactly the bits of a single context running the whole lattice; ghost planes are scratch.
+ * Contexts may use different streams (ordered by events) and, with peer access enabled, different
+ * devices; D3Q19, AB store.  Errors: LBM_EINVAL (mismatching slabs), LBM_EUNSUPPORTED, LBM_ESTATE. */
+int lbm_step_slabs(lbm_ctx *const *slabs, int count, int periodic_z, int n);
+
 /* Time step counter since the last init/set, and number of kernels launched by this context. */
 int lbm_get_counters(const lbm_ctx *ctx, int64_t *steps, int64_t *launches);
 

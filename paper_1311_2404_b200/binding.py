@@ -26,7 +26,7 @@ LBM_QMAX = 19
 EXPORTS = ("lbm_lattice_info", "lbm_workspace_bytes", "lbm_create", "lbm_destroy", "lbm_set_geometry",
            "lbm_get_geometry", "lbm_init_equilibrium", "lbm_step", "lbm_macro", "lbm_get_distributions",
            "lbm_set_distributions", "lbm_get_stream_map", "lbm_run_host", "lbm_get_counters",
-           "lbm_get_dispatch", "lbm_last_error")
+           "lbm_get_dispatch", "lbm_step_slabs", "lbm_last_error")
 
 
 class lbm_params(C.Structure):
@@ -81,6 +81,7 @@ def load():
     L.lbm_run_host.argtypes = [vp, vp, C.POINTER(vp), C.POINTER(vp), C.c_int, vp, vp]
     L.lbm_get_counters.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
     L.lbm_get_dispatch.argtypes = [vp, C.POINTER(lbm_dispatch)]
+    L.lbm_step_slabs.argtypes = [C.POINTER(vp), C.c_int, C.c_int, C.c_int]
     L.lbm_last_error.argtypes = [vp]
     L.lbm_last_error.restype = C.c_char_p
     for name in EXPORTS:
@@ -170,6 +171,11 @@ def lbm_get_counters(ctx):
     s, l = C.c_int64(), C.c_int64()
     _check(load().lbm_get_counters(ctx, C.byref(s), C.byref(l)), ctx)
     return s.value, l.value
+
+
+def lbm_step_slabs(ctxs, periodic_z: bool, n: int):
+    arr = (C.c_void_p * len(ctxs))(*ctxs)
+    _check(load().lbm_step_slabs(arr, len(ctxs), 1 if periodic_z else 0, int(n)), ctxs[0])
 
 
 def lbm_get_dispatch(ctx) -> dict:

@@ -217,6 +217,8 @@ LBM_API int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, voi
     }
     if (idx64_built && env_int("LBM_IDX64", 0, 0, 1)) c->idx32 = false;
     c->rows = 0;
+    c->sc_phase = 0;
+    c->slab_event = nullptr;
     c->sc_split = (p->model == LBM_SC2 && (env_int("LBM_SC_SPLIT", 1, 0, 1) || p->store == LBM_STORE_AA || !c->idx32)) ? pick_vec(p, 0.0, true) : 0;
     c->all_bulk = true;  // the geometry starts all-FLUID
     c->span_bx = env_int("LBM_SPAN_BX", 0, 32, 256) / 32 * 32;
@@ -248,6 +250,7 @@ LBM_API int lbm_destroy(lbm_ctx *c) {
     CHECK_CTX(c);
     drop_graphs(c);
     if (c->capture_stream) cudaStreamDestroy(c->capture_stream);
+    if (c->slab_event) cudaEventDestroy(c->slab_event);
     delete c;
     return LBM_OK;
 }
@@ -405,6 +408,129 @@ LBM_API int lbm_run_host(lbm_ctx *c, const uint8_t *h_mask, const void *const *h
         if (h_u_out) CUDA_TRY(c, cudaMemcpyAsync(h_u_out, d_u, c->D * N * rs, cudaMemcpyDeviceToHost, c->stream));
     }
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    return LBM_OK;
+}
+
+// ---- z-slab decomposition --------------------------------------------------------------
+namespace {
+
+template <typename T>
+int copy_planes(lbm_ctx *to, const T *src, T *dst, int64_t Nsrc, int64_t Ndst, int from_plane, int to_plane,
+                int ndir, const PlaneList &dirs) {
+    const int plane = to->g.nx * to->g.ny;
+    const dim3 grid((plane + 255) / 256, ndir);
+    slab_copy_planes_kernel<T><<<grid, 256, 0, to->stream>>>(src, dst, Nsrc, Ndst, (int64_t)from_plane * plane, (int64_t)to_plane * plane,
+                                                            plane, dirs);
+    return check_launch(to, "slab_copy_planes_kernel");
+}
+
+// Fill the ghost plane `to_plane` of `to` from the interior plane `from_plane` of `from`.
+// what = 0: the populations with e_z = ez of the current buffer of every component; 1: the psi fields.
+template <typename T> int fill_ghost(lbm_ctx *to, lbm_ctx *from, int from_plane, int to_plane, int ez, int what) {
+    if (what == 1) {
+        PlaneList one = {{0}};
+        T *pa = at<T>(to, to->lay.psi[0]);
+        const T *qa = at<T>(from, from->lay.psi[0]);
+        for (int s = 0; s < 2; s++)  // planar psi_A | psi_B (split kernels)
+            if (int rc = copy_planes<T>(to, qa + s * from->g.N, pa + s * to->g.N, from->g.N, to->g.N, from_plane, to_plane, 1, one)) return rc;
+        return LBM_OK;
+    }
+    PlaneList dirs = {{0}};
+    int32_t e[3 * LBM_QMAX];
+    int nd = 0;
+    lbm_lattice_info(to->p.lattice, nullptr, nullptr, e, nullptr, nullptr);
+    for (int i = 0; i < to->Q; i++)
+        if (e[3 * i + 2] == ez) dirs.dir[nd++] = i;
+    for (int s = 0; s < to->ncomp; s++)
+        if (int rc = copy_planes<T>(to, at<T>(from, from->lay.store[s][from->cur]), at<T>(to, to->lay.store[s][to->cur]),
+                                    from->g.N, to->g.N, from_plane, to_plane, nd, dirs)) return rc;
+    return LBM_OK;
+}
+
+int fill_ghost_any(lbm_ctx *to, lbm_ctx *from, int from_plane, int to_plane, int ez, int what) {
+    return to->rs == 4 ? fill_ghost<float>(to, from, from_plane, to_plane, ez, what)
+                       : fill_ghost<double>(to, from, from_plane, to_plane, ez, what);
+}
+
+// All ghost planes of all slabs from their neighbours' boundary interior planes.  Streams: each slab's
+// copies run on its own stream after the neighbour's work enqueued so far (event), so slabs on different
+// streams / devices stay ordered; with one shared stream the events are skipped.
+int exchange_ghosts(lbm_ctx *const *slabs, int count, int periodic_z, int what) {
+    bool one_stream = true;
+    for (int k = 1; k < count; k++) one_stream = one_stream && slabs[k]->stream == slabs[0]->stream;
+    if (!one_stream)
+        for (int k = 0; k < count; k++) {
+            lbm_ctx *c = slabs[k];
+            if (!c->slab_event && cudaEventCreateWithFlags(&c->slab_event, cudaEventDisableTiming) != cudaSuccess)
+                return fail(c, LBM_ECUDA, "cudaEventCreate failed");
+            if (cudaEventRecord(c->slab_event, c->stream) != cudaSuccess) return fail(c, LBM_ECUDA, "cudaEventRecord failed");
+        }
+    for (int k = 0; k < count; k++) {
+        lbm_ctx *c = slabs[k];
+        lbm_ctx *below = k > 0 ? slabs[k - 1] : (periodic_z ? slabs[count - 1] : nullptr);
+        lbm_ctx *above = k + 1 < count ? slabs[k + 1] : (periodic_z ? slabs[0] : nullptr);
+        for (lbm_ctx *nb : {below, above})
+            if (nb && !one_stream && nb != c && cudaStreamWaitEvent(c->stream, nb->slab_event, 0) != cudaSuccess)
+                return fail(c, LBM_ECUDA, "cudaStreamWaitEvent failed");
+        // lower ghost (plane 0) <- top interior plane of the slab below: what moves up (e_z = +1)
+        if (below) if (int rc = fill_ghost_any(c, below, below->g.nz - 2, 0, +1, what)) return rc;
+        // upper ghost (plane nz-1) <- bottom interior plane (1) of the slab above: what moves down (e_z = -1)
+        if (above) if (int rc = fill_ghost_any(c, above, 1, c->g.nz - 1, -1, what)) return rc;
+    }
+    if (!one_stream)  // a slab must not run ahead and overwrite planes a neighbour's copy is still reading
+        for (int k = 0; k < count; k++)
+            if (cudaEventRecord(slabs[k]->slab_event, slabs[k]->stream) != cudaSuccess) return fail(slabs[k], LBM_ECUDA, "cudaEventRecord failed");
+    if (!one_stream)
+        for (int k = 0; k < count; k++) {
+            lbm_ctx *c = slabs[k];
+            lbm_ctx *below = k > 0 ? slabs[k - 1] : (periodic_z ? slabs[count - 1] : nullptr);
+            lbm_ctx *above = k + 1 < count ? slabs[k + 1] : (periodic_z ? slabs[0] : nullptr);
+            for (lbm_ctx *nb : {below, above})
+                if (nb && nb != c && cudaStreamWaitEvent(c->stream, nb->slab_event, 0) != cudaSuccess)
+                    return fail(c, LBM_ECUDA, "cudaStreamWaitEvent failed");
+        }
+    return LBM_OK;
+}
+
+}  // namespace
+
+static int check_state(lbm_ctx *c);
+
+LBM_API int lbm_step_slabs(lbm_ctx *const *slabs, int count, int periodic_z, int n) {
+    if (!slabs || count < 1) return fail(nullptr, LBM_EINVAL, "slabs is NULL or count < 1");
+    for (int k = 0; k < count; k++) {
+        lbm_ctx *c = slabs[k];
+        CHECK_CTX(c);
+        if (n < 0) return fail(c, LBM_EINVAL, "n < 0");
+        if (int rc = check_state(c)) return rc;
+        if (c->p.lattice != LBM_D3Q19 || c->aa) return fail(c, LBM_EUNSUPPORTED, "slabs: D3Q19 with the AB store only");
+        if (c->p.model == LBM_SC2 && !c->sc_split) return fail(c, LBM_EUNSUPPORTED, "slabs: Shan-Chen needs the split kernels");
+        if (c->g.nz < 3) return fail(c, LBM_EINVAL, "slabs: a slab needs two ghost planes and at least one interior plane");
+        const lbm_ctx *a = slabs[0];
+        if (c->g.nx != a->g.nx || c->g.ny != a->g.ny || c->p.model != a->p.model || c->rs != a->rs || c->cur != a->cur || c->steps != a->steps)
+            return fail(c, LBM_EINVAL, "slabs: contexts differ in nx, ny, model, precision or time step");
+    }
+    for (int t = 0; t < n; t++) {
+        if (slabs[0]->p.model == LBM_SC2) {
+            for (int k = 0; k < count; k++) {
+                slabs[k]->sc_phase = 1;
+                const int rc = slabs[k]->vt->step(slabs[k], 1);
+                slabs[k]->sc_phase = 0;
+                if (rc) return rc;
+            }
+            if (int rc = exchange_ghosts(slabs, count, periodic_z, 1)) return rc;  // psi planes (eq. 10 reads neighbours)
+            for (int k = 0; k < count; k++) {
+                slabs[k]->sc_phase = 2;
+                const int rc = slabs[k]->vt->step(slabs[k], 1);
+                slabs[k]->sc_phase = 0;
+                if (rc) return rc;
+            }
+        } else {
+            for (int k = 0; k < count; k++)
+                if (int rc = slabs[k]->vt->step(slabs[k], 1)) return rc;
+        }
+        if (int rc = exchange_ghosts(slabs, count, periodic_z, 0)) return rc;  // the crossing populations of the new state
+    }
     return LBM_OK;
 }
 

@@ -46,6 +46,8 @@ struct lbm_ctx {
     int resident_state; // 0 not probed yet, 1 launchable, -1 not launchable here (fall back for good)
     int span_bx;        // tuning: block width (threads along x) of the step kernels, 0 = default
     bool all_bulk;      // no node of the geometry is SOLID / BOUNDARY / special: the step kernels skip the type array
+    int sc_phase;       // lbm_step_slabs only: which part of a Shan-Chen step the next vt->step call runs (see lbm_steps.cuh)
+    cudaEvent_t slab_event;  // lbm_step_slabs only: "this slab's kernels up to here are enqueued", created on first use
     int sc_split;       // Shan-Chen: > 0 = split variant (one collide launch per component), nodes per thread
     int sc_fields_vec;  // Shan-Chen: nodes per thread of the macro-field pass (the collide pass uses `vec`)
     int rows;           // > 0: obstacle-rich geometry (>= 20 % of the nodes not BULK): step_rows_kernel, rows per block

@@ -407,6 +407,24 @@ step_rows_kernel(Geom g, const uint32_t *__restrict__ link, const T *__restrict_
     }
 }
 
+// ---- z-slab decomposition: ghost-plane exchange ------------------------------------
+// A slab context holds its share of the lattice as local planes 1 .. nz-2 plus one ghost plane below
+// (0) and above (nz-1).  After a step the ghost planes receive, from the neighbouring slab's boundary
+// interior plane, the populations that will stream across the face ("only the mass fractions that
+// actually need to be sent"): in the SoA store a population's z-plane is one contiguous run of
+// nx*ny values, so the "pack" is a plane copy per crossing direction (5 of 19 for D3Q19).  The same
+// kernel moves the psi planes of the Shan-Chen fields (ndir = 1 per field).  src and dst may live on
+// different devices with peer access enabled (plain stores over NVLink); tested on one device.
+struct PlaneList { int dir[8]; };
+template <typename T>
+__global__ void slab_copy_planes_kernel(const T *__restrict__ src, T *__restrict__ dst, int64_t Nsrc, int64_t Ndst,
+                                        int64_t src_off, int64_t dst_off, int plane_nodes, PlaneList dirs) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= plane_nodes) return;
+    const int i = dirs.dir[blockIdx.y];
+    dst[(int64_t)i * Ndst + dst_off + j] = src[(int64_t)i * Nsrc + src_off + j];
+}
+
 // ---- canonical <-> internal conversions (off the hot loop; reading A9) ----------------------
 // canonical f_i(x,t) -> store: S[source_slot(i, x)] = f_i(x) - w_i, the inverse of the pull.  The
 // pull is a permutation of FLUID slots (A8), so every FLUID slot is written exactly once.

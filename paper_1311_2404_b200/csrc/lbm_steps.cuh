@@ -172,9 +172,14 @@ template <class L, typename T> struct Steps {
         }
         }
         for (int t = 0; t < n; t++) {
-            sc_fields_split_kernel<L, T, V, I, PSI><<<l.grid, l.block, 0, c->stream>>>(
-                c->g, type_or_null(c), link(c), src(c, 0), src(c, 1), psiA, psiB, up, rA.inv_tau, rB.inv_tau);
-            if (int rc = check_launch(c, "sc_fields_split_kernel")) return rc;
+            // sc_phase (lbm_step_slabs): 1 = macro-field pass only, 2 = collide passes only (the psi planes of the
+            // slab's ghost layers are exchanged in between), 0 = the whole step
+            if (c->sc_phase != 2) {
+                sc_fields_split_kernel<L, T, V, I, PSI><<<l.grid, l.block, 0, c->stream>>>(
+                    c->g, type_or_null(c), link(c), src(c, 0), src(c, 1), psiA, psiB, up, rA.inv_tau, rB.inv_tau);
+                if (int rc = check_launch(c, "sc_fields_split_kernel")) return rc;
+            }
+            if (c->sc_phase == 1) continue;
             sc_collide_split_kernel<L, T, V, I, PSI, FS><<<l.grid, l.block, 0, c->stream>>>(
                 c->g, type_or_null(c), link(c), src(c, 0), dst(c, 0), psiB, up, rA, T(c->p.sc_G));
             if (int rc = check_launch(c, "sc_collide_split_kernel")) return rc;
