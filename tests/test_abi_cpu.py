@@ -112,6 +112,27 @@ def test_null_ctx_calls_return_einval(lib):
     assert lib.lbm_step(None, 1) == binding.LBM_EINVAL
     assert lib.lbm_destroy(None) == binding.LBM_EINVAL
     assert lib.lbm_macro(None, 0, None, None) == binding.LBM_EINVAL
+    assert lib.lbm_get_dispatch(None, None) == binding.LBM_EINVAL
+    assert lib.lbm_step_slabs(None, 0, 1, 1) == binding.LBM_EINVAL
+    arr = (C.c_void_p * 2)(None, None)
+    assert lib.lbm_step_slabs(arr, 2, 1, 1) == binding.LBM_EINVAL
+
+
+def test_reserved_field_and_node_count_limit(lib):
+    """lbm.h: reserved_ must be 0 (so the field can be given a meaning later); nx*ny*nz <= 2^31 - 512 (node
+    indices are ints and padded threads index up to one block beyond the last node)."""
+    p = binding.make_params(1, 0, 0, 8, 8, 8, tau=0.8)
+    p.reserved_ = 1
+    with pytest.raises(binding.LbmError) as e:
+        binding.lbm_workspace_bytes(p)
+    assert e.value.code == binding.LBM_EINVAL and "reserved_" in str(e.value)
+    ok = binding.make_params(1, 0, 0, 2 ** 15, 2 ** 15, 1, tau=0.8)            # 2^30 nodes
+    assert binding.lbm_workspace_bytes(ok) > 2 * 19 * 4 * 2 ** 30
+    for nx, ny, nz in ((2 ** 16, 2 ** 15, 1), (2 ** 15, 2 ** 15, 2), (2 ** 31 - 511, 1, 1)):   # > 2^31 - 512
+        with pytest.raises(binding.LbmError) as e:
+            binding.lbm_workspace_bytes(binding.make_params(1, 0, 0, nx, ny, nz, tau=0.8))
+        assert e.value.code == binding.LBM_EINVAL
+    assert C.sizeof(binding.lbm_dispatch) == 36
 
 
 def test_product_does_not_import_oracle():
