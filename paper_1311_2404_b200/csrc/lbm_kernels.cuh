@@ -13,6 +13,7 @@
 #pragma once
 #include <cooperative_groups.h>
 #include <cuda_runtime.h>
+#include <type_traits>
 #include "lbm_node.cuh"
 
 namespace lbm {
@@ -519,27 +520,21 @@ __global__ void macro_kernel(Geom g, const uint8_t *__restrict__ type, const uin
 // once and kept in registers.  Same arithmetic and streaming rule as step_kernel: bit-identical.
 constexpr int RESIDENT_MAX_CTAS = 16;
 
-__device__ __forceinline__ uint32_t dsmem_address(const void *smem_ptr, unsigned cta_rank) {
-    uint32_t local = (uint32_t)__cvta_generic_to_shared(smem_ptr), remote;
-    asm("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(local), "r"(cta_rank));
-    return remote;
-}
-template <typename T> __device__ __forceinline__ T dsmem_load(uint32_t addr);
-template <> __device__ __forceinline__ float dsmem_load<float>(uint32_t addr) {
-    float v; asm volatile("ld.shared::cluster.f32 %0, [%1];" : "=f"(v) : "r"(addr) : "memory"); return v;
-}
-template <> __device__ __forceinline__ double dsmem_load<double>(uint32_t addr) {
-    double v; asm volatile("ld.shared::cluster.f64 %0, [%1];" : "=d"(v) : "r"(addr) : "memory"); return v;
-}
-
-template <class L, typename T, int MODEL, int FORCE, int THREADS>
+// SFIX: the CTA's share S equals THREADS (a compile-time constant).  Then the step loop is unrolled by two
+// (one body per buffer parity) and every shared-memory address is a register that never changes plus an
+// immediate: 9 LD + 9 STS + the collision per D2Q9 node and step, no address arithmetic (the generic-S loop
+// spends half of its issue slots on it, and at 1024 nodes per SM the kernel is issue-bound).
+template <class L, typename T, int MODEL, int FORCE, int THREADS, bool SFIX>
 __global__ void __launch_bounds__(THREADS)
-resident_kernel(Geom g, int s_log2, const uint8_t *__restrict__ type, const uint32_t *__restrict__ link,
+resident_kernel(Geom g, int s_log2_arg, const uint8_t *__restrict__ type, const uint32_t *__restrict__ link,
                 const T *src, T *dst, Relax<T> rp, int nsteps) {
     extern __shared__ __align__(16) unsigned char resident_smem[];
     T *buf = reinterpret_cast<T *>(resident_smem);  // [2][Q][S]
     namespace cg = cooperative_groups;
     cg::cluster_group cluster = cg::this_cluster();
+    constexpr int LOG2_THREADS = THREADS == 1024 ? 10 : THREADS == 512 ? 9 : THREADS == 256 ? 8 : 7;
+    static_assert((1 << LOG2_THREADS) == THREADS, "THREADS must be 128 .. 1024, a power of two");
+    const int s_log2 = SFIX ? LOG2_THREADS : s_log2_arg;
     const int S = 1 << s_log2, mask = S - 1, N = (int)g.N;
     const int base = (int)cluster.block_rank() * S;
     const int tid = threadIdx.x;
@@ -547,10 +542,13 @@ resident_kernel(Geom g, int s_log2, const uint8_t *__restrict__ type, const uint
         const int i = idx >> s_log2, n = base + (idx & mask);
         buf[idx] = n < N ? src[(int64_t)i * N + n] : T(0);
     }
-    // this thread's node: type and the Q source addresses (buffer 0) stay in registers for all steps
+    // this thread's node: type and the Q source addresses (buffer 0; generic pointers into the cluster's
+    // distributed shared memory, reflected links resolved) stay in registers for all steps
     const int n = base + tid;
     uint32_t t = NODE_SOLID;  // threads beyond the lattice or beyond S do nothing
-    uint32_t from[L::Q];
+    const T *from[L::Q];
+#pragma unroll
+    for (int i = 0; i < L::Q; i++) from[i] = buf;
     if (tid < S && n < N) {
         t = type[n];
         const uint32_t w = (t & NODE_LINKS) ? link[n] : 0u;
@@ -561,24 +559,47 @@ resident_kernel(Geom g, int s_log2, const uint8_t *__restrict__ type, const uint
             const bool refl = reflected(w, i);
             const int m = refl ? n : n + shift<L>(i, -1, o);  // source node
             const int plane = refl ? L::opp(i) : i;
-            from[i] = dsmem_address(buf + plane * S + (m & mask), (unsigned)(m >> s_log2));
+            from[i] = cluster.map_shared_rank(buf + plane * S + (m & mask), m >> s_log2);
         }
     }
+    T *mine = buf + tid;
     cluster.sync();
-    const uint32_t flip = (uint32_t)(L::Q * S * sizeof(T));  // byte distance between the two buffers
     int cur = 0;
-    for (int step = 0; step < nsteps; step++) {
-        if (!(t & NODE_SOLID)) {
-            T h[L::Q];
+    if constexpr (SFIX) {
+        constexpr int FLIP = L::Q * THREADS;  // elements between the two buffers
+        auto one_step = [&](auto parity) {
+            constexpr int c = decltype(parity)::value;
+            if (!(t & NODE_SOLID)) {
+                T h[L::Q];
 #pragma unroll
-            for (int i = 0; i < L::Q; i++) h[i] = dsmem_load<T>(from[i] + (cur ? flip : 0u));
-            update_typed<L, T, MODEL, FORCE>(h, t, rp);
-            T *B = buf + (cur ^ 1) * L::Q * S;
+                for (int i = 0; i < L::Q; i++) h[i] = from[i][c * FLIP];
+                update_typed<L, T, MODEL, FORCE>(h, t, rp);
 #pragma unroll
-            for (int i = 0; i < L::Q; i++) B[i * S + tid] = h[i];
+                for (int i = 0; i < L::Q; i++) mine[(c ^ 1) * FLIP + i * THREADS] = h[i];
+            }
+            cluster.sync();  // every CTA has written step t+1 before anyone pulls from it
+        };
+        int step = 0;
+        for (; step + 1 < nsteps; step += 2) {
+            one_step(std::integral_constant<int, 0>{});
+            one_step(std::integral_constant<int, 1>{});
         }
-        cluster.sync();  // every CTA has written step t+1 before anyone pulls from it
-        cur ^= 1;
+        if (step < nsteps) { one_step(std::integral_constant<int, 0>{}); cur = 1; }
+    } else {
+        const int flip = L::Q * S;
+        for (int step = 0; step < nsteps; step++) {
+            if (!(t & NODE_SOLID)) {
+                T h[L::Q];
+#pragma unroll
+                for (int i = 0; i < L::Q; i++) h[i] = from[i][cur ? flip : 0];
+                update_typed<L, T, MODEL, FORCE>(h, t, rp);
+                T *B = mine + (cur ^ 1) * flip;
+#pragma unroll
+                for (int i = 0; i < L::Q; i++) B[i * S] = h[i];
+            }
+            cluster.sync();
+            cur ^= 1;
+        }
     }
     for (int idx = tid; idx < L::Q * S; idx += THREADS) {
         const int i = idx >> s_log2, m = base + (idx & mask);

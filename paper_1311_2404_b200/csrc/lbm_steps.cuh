@@ -63,8 +63,8 @@ template <class L, typename T> struct Steps {
     // The first call probes the launch (shared-memory opt-in, non-portable cluster size, at least one
     // co-schedulable cluster: a MIG/MPS slice may have too few SMs); if it cannot run, the context falls
     // back to the ordinary step kernels with graph replay for good.
-    template <int MODEL, int FORCE, int THREADS> static int launch_resident(lbm_ctx *c, int n, const Relax<T> &rp, bool *unavailable) {
-        auto kernel = resident_kernel<L, T, MODEL, FORCE, THREADS>;
+    template <int MODEL, int FORCE, int THREADS, bool SFIX> static int launch_resident(lbm_ctx *c, int n, const Relax<T> &rp, bool *unavailable) {
+        auto kernel = resident_kernel<L, T, MODEL, FORCE, THREADS, SFIX>;
         const size_t smem = 2 * (size_t)L::Q * ((size_t)1 << c->resident_slog2) * sizeof(T);
         cudaLaunchConfig_t cfg = {};
         cudaLaunchAttribute attr[1];
@@ -96,10 +96,11 @@ template <class L, typename T> struct Steps {
     }
 
     template <int MODEL, int FORCE> static int step_resident(lbm_ctx *c, int n, const Relax<T> &rp, bool *unavailable) {
-        if constexpr (L::Q == 9) {
-            if (c->resident_slog2 == 10) return launch_resident<MODEL, FORCE, 1024>(c, n, rp, unavailable);
+        if constexpr (L::Q == 9) {  // nodes per CTA == threads per CTA: the unrolled loop with immediate addresses
+            if (c->resident_slog2 == 10) return launch_resident<MODEL, FORCE, 1024, true>(c, n, rp, unavailable);
         }
-        return launch_resident<MODEL, FORCE, 512>(c, n, rp, unavailable);
+        if (c->resident_slog2 == 9) return launch_resident<MODEL, FORCE, 512, true>(c, n, rp, unavailable);
+        return launch_resident<MODEL, FORCE, 512, false>(c, n, rp, unavailable);
     }
 
     template <int MODEL, int FORCE> static int step_single(lbm_ctx *c, int n, const Relax<T> &rp) {
