@@ -538,9 +538,17 @@ resident_kernel(Geom g, int s_log2_arg, const uint8_t *__restrict__ type, const 
     const int S = 1 << s_log2, mask = S - 1, N = (int)g.N;
     const int base = (int)cluster.block_rank() * S;
     const int tid = threadIdx.x;
-    for (int idx = tid; idx < L::Q * S; idx += THREADS) {
-        const int i = idx >> s_log2, n = base + (idx & mask);
-        buf[idx] = n < N ? src[(int64_t)i * N + n] : T(0);
+    if constexpr (SFIX) {  // S == THREADS: one slot of every plane per thread, all Q loads in flight at once
+        T v[L::Q];
+#pragma unroll
+        for (int i = 0; i < L::Q; i++) v[i] = base + tid < N ? src[(int64_t)i * N + base + tid] : T(0);
+#pragma unroll
+        for (int i = 0; i < L::Q; i++) buf[i * THREADS + tid] = v[i];
+    } else {
+        for (int idx = tid; idx < L::Q * S; idx += THREADS) {
+            const int i = idx >> s_log2, n = base + (idx & mask);
+            buf[idx] = n < N ? src[(int64_t)i * N + n] : T(0);
+        }
     }
     // this thread's node: type and the Q source addresses (buffer 0; generic pointers into the cluster's
     // distributed shared memory, reflected links resolved) stay in registers for all steps
