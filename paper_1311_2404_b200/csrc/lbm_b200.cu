@@ -201,6 +201,7 @@ LBM_API int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, voi
     c->rs = p->precision == LBM_F32 ? 4 : 8;
     c->g.nx = p->nx; c->g.ny = p->ny; c->g.nz = p->nz; c->g.N = (int64_t)p->nx * p->ny * p->nz;
     c->stream = static_cast<cudaStream_t>(cuda_stream);
+    if (cudaGetDevice(&c->device) != cudaSuccess) { cudaGetLastError(); c->device = 0; }
     c->ws = static_cast<char *>(d_workspace);
     c->lay = lay;
     c->block_x = pick_block_x(p->nx);
@@ -452,15 +453,27 @@ int fill_ghost_any(lbm_ctx *to, lbm_ctx *from, int from_plane, int to_plane, int
                        : fill_ghost<double>(to, from, from_plane, to_plane, ez, what);
 }
 
+// Slabs may live on different devices: launches and event calls for a slab run with its device current.
+struct DeviceGuard {
+    int saved = -1;
+    DeviceGuard() { if (cudaGetDevice(&saved) != cudaSuccess) saved = -1; }
+    void use(const lbm_ctx *c) { if (c->device != current()) cudaSetDevice(c->device); }
+    static int current() { int d = -1; cudaGetDevice(&d); return d; }
+    ~DeviceGuard() { if (saved >= 0 && saved != current()) cudaSetDevice(saved); }
+};
+
 // All ghost planes of all slabs from their neighbours' boundary interior planes.  Streams: each slab's
 // copies run on its own stream after the neighbour's work enqueued so far (event), so slabs on different
 // streams / devices stay ordered; with one shared stream the events are skipped.
 int exchange_ghosts(lbm_ctx *const *slabs, int count, int periodic_z, int what) {
+    DeviceGuard dev;
     bool one_stream = true;
-    for (int k = 1; k < count; k++) one_stream = one_stream && slabs[k]->stream == slabs[0]->stream;
+    for (int k = 1; k < count; k++)
+        one_stream = one_stream && slabs[k]->stream == slabs[0]->stream && slabs[k]->device == slabs[0]->device;
     if (!one_stream)
         for (int k = 0; k < count; k++) {
             lbm_ctx *c = slabs[k];
+            dev.use(c);
             if (!c->slab_event && cudaEventCreateWithFlags(&c->slab_event, cudaEventDisableTiming) != cudaSuccess)
                 return fail(c, LBM_ECUDA, "cudaEventCreate failed");
             if (cudaEventRecord(c->slab_event, c->stream) != cudaSuccess) return fail(c, LBM_ECUDA, "cudaEventRecord failed");
@@ -469,6 +482,7 @@ int exchange_ghosts(lbm_ctx *const *slabs, int count, int periodic_z, int what) 
         lbm_ctx *c = slabs[k];
         lbm_ctx *below = k > 0 ? slabs[k - 1] : (periodic_z ? slabs[count - 1] : nullptr);
         lbm_ctx *above = k + 1 < count ? slabs[k + 1] : (periodic_z ? slabs[0] : nullptr);
+        dev.use(c);
         for (lbm_ctx *nb : {below, above})
             if (nb && !one_stream && nb != c && cudaStreamWaitEvent(c->stream, nb->slab_event, 0) != cudaSuccess)
                 return fail(c, LBM_ECUDA, "cudaStreamWaitEvent failed");
@@ -478,11 +492,14 @@ int exchange_ghosts(lbm_ctx *const *slabs, int count, int periodic_z, int what) 
         if (above) if (int rc = fill_ghost_any(c, above, 1, c->g.nz - 1, -1, what)) return rc;
     }
     if (!one_stream)  // a slab must not run ahead and overwrite planes a neighbour's copy is still reading
-        for (int k = 0; k < count; k++)
+        for (int k = 0; k < count; k++) {
+            dev.use(slabs[k]);
             if (cudaEventRecord(slabs[k]->slab_event, slabs[k]->stream) != cudaSuccess) return fail(slabs[k], LBM_ECUDA, "cudaEventRecord failed");
+        }
     if (!one_stream)
         for (int k = 0; k < count; k++) {
             lbm_ctx *c = slabs[k];
+            dev.use(c);
             lbm_ctx *below = k > 0 ? slabs[k - 1] : (periodic_z ? slabs[count - 1] : nullptr);
             lbm_ctx *above = k + 1 < count ? slabs[k + 1] : (periodic_z ? slabs[0] : nullptr);
             for (lbm_ctx *nb : {below, above})
@@ -510,9 +527,11 @@ LBM_API int lbm_step_slabs(lbm_ctx *const *slabs, int count, int periodic_z, int
         if (c->g.nx != a->g.nx || c->g.ny != a->g.ny || c->p.model != a->p.model || c->rs != a->rs || c->cur != a->cur || c->steps != a->steps)
             return fail(c, LBM_EINVAL, "slabs: contexts differ in nx, ny, model, precision or time step");
     }
+    DeviceGuard dev;
     for (int t = 0; t < n; t++) {
         if (slabs[0]->p.model == LBM_SC2) {
             for (int k = 0; k < count; k++) {
+                dev.use(slabs[k]);
                 slabs[k]->sc_phase = 1;
                 const int rc = slabs[k]->vt->step(slabs[k], 1);
                 slabs[k]->sc_phase = 0;
@@ -520,14 +539,17 @@ LBM_API int lbm_step_slabs(lbm_ctx *const *slabs, int count, int periodic_z, int
             }
             if (int rc = exchange_ghosts(slabs, count, periodic_z, 1)) return rc;  // psi planes (eq. 10 reads neighbours)
             for (int k = 0; k < count; k++) {
+                dev.use(slabs[k]);
                 slabs[k]->sc_phase = 2;
                 const int rc = slabs[k]->vt->step(slabs[k], 1);
                 slabs[k]->sc_phase = 0;
                 if (rc) return rc;
             }
         } else {
-            for (int k = 0; k < count; k++)
+            for (int k = 0; k < count; k++) {
+                dev.use(slabs[k]);
                 if (int rc = slabs[k]->vt->step(slabs[k], 1)) return rc;
+            }
         }
         if (int rc = exchange_ghosts(slabs, count, periodic_z, 0)) return rc;  // the crossing populations of the new state
     }

@@ -34,6 +34,7 @@ struct lbm_ctx {
     size_t rs;  // sizeof(real)
     Geom g;
     cudaStream_t stream;
+    int device;  // CUDA device current at lbm_create (the workspace and the stream belong to it)
     char *ws;
     Layout lay;
     int cur;  // which of the two buffers holds the current state (AB)
