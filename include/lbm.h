@@ -150,9 +150,11 @@ int lbm_run_host(lbm_ctx *ctx, const uint8_t *h_mask, const void *const *h_rho0,
  * plane below (local z = 0) and one above (local z = nz - 1): the caller slices mask, rho0 and u0 of the
  * global lattice accordingly (ghost planes = copies of the neighbour's boundary planes, through the
  * periodic seam if periodic_z) and initialises every slab with the usual calls.  lbm_step_slabs then
- * advances all slabs n steps in lockstep: after every step each ghost plane receives, from the
- * neighbouring slab's boundary interior plane, the 5 of 19 populations that stream across the face
- * (P:464); for LBM_SC2 the psi planes are exchanged between the macro-field pass and the collide pass.
+ * advances all slabs n steps in lockstep.  Every step launches the two boundary interior planes of each
+ * slab first; as soon as they are done each ghost plane receives, from the neighbouring slab's boundary
+ * plane, the 5 of 19 populations that stream across the face -- on a side stream, concurrently with
+ * the launch over the bulk planes; ghost planes themselves are never updated.  For LBM_SC2 the
+ * macro-field pass is ordered the same way and exchanges the psi planes before the collide pass.
  * slabs[0] is the lowest slab; periodic_z != 0 also links slabs[count-1] to slabs[0].  Interior planes
  * then hold exactly the bits of a single context running the whole lattice; ghost planes are scratch.
  * Contexts may use different streams (ordered by events) and, with peer access enabled, different

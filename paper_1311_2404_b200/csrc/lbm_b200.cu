@@ -199,7 +199,8 @@ LBM_API int lbm_create(const lbm_params *p, void *d_workspace, size_t bytes, voi
     memcpy(&c->p, p, p->struct_size);  // a shorter (older) struct leaves the newer fields zero
     c->Q = Q; c->D = D; c->ncomp = p->model == LBM_SC2 ? 2 : 1;
     c->rs = p->precision == LBM_F32 ? 4 : 8;
-    c->g.nx = p->nx; c->g.ny = p->ny; c->g.nz = p->nz; c->g.N = (int64_t)p->nx * p->ny * p->nz;
+    c->g.nx = p->nx; c->g.ny = p->ny; c->g.nz = p->nz; c->g.N = (int64_t)p->nx * p->ny * p->nz; c->g.z0 = 0;
+    c->zsel0 = 0; c->zselc = p->nz; c->no_advance = false; c->slab_stream = nullptr; c->slab_event2 = nullptr;
     c->stream = static_cast<cudaStream_t>(cuda_stream);
     if (cudaGetDevice(&c->device) != cudaSuccess) { cudaGetLastError(); c->device = 0; }
     c->ws = static_cast<char *>(d_workspace);
@@ -252,6 +253,8 @@ LBM_API int lbm_destroy(lbm_ctx *c) {
     drop_graphs(c);
     if (c->capture_stream) cudaStreamDestroy(c->capture_stream);
     if (c->slab_event) cudaEventDestroy(c->slab_event);
+    if (c->slab_event2) cudaEventDestroy(c->slab_event2);
+    if (c->slab_stream) cudaStreamDestroy(c->slab_stream);
     delete c;
     return LBM_OK;
 }
@@ -416,24 +419,26 @@ LBM_API int lbm_run_host(lbm_ctx *c, const uint8_t *h_mask, const void *const *h
 namespace {
 
 template <typename T>
-int copy_planes(lbm_ctx *to, const T *src, T *dst, int64_t Nsrc, int64_t Ndst, int from_plane, int to_plane,
+int copy_planes(lbm_ctx *to, cudaStream_t stream, const T *src, T *dst, int64_t Nsrc, int64_t Ndst, int from_plane, int to_plane,
                 int ndir, const PlaneList &dirs) {
     const int plane = to->g.nx * to->g.ny;
     const dim3 grid((plane + 255) / 256, ndir);
-    slab_copy_planes_kernel<T><<<grid, 256, 0, to->stream>>>(src, dst, Nsrc, Ndst, (int64_t)from_plane * plane, (int64_t)to_plane * plane,
-                                                            plane, dirs);
+    slab_copy_planes_kernel<T><<<grid, 256, 0, stream>>>(src, dst, Nsrc, Ndst, (int64_t)from_plane * plane, (int64_t)to_plane * plane,
+                                                        plane, dirs);
     return check_launch(to, "slab_copy_planes_kernel");
 }
 
-// Fill the ghost plane `to_plane` of `to` from the interior plane `from_plane` of `from`.
-// what = 0: the populations with e_z = ez of the current buffer of every component; 1: the psi fields.
-template <typename T> int fill_ghost(lbm_ctx *to, lbm_ctx *from, int from_plane, int to_plane, int ez, int what) {
+// Fill the ghost plane `to_plane` of `to` from the interior plane `from_plane` of `from`, on `to`'s side stream.
+// what = 0: the populations with e_z = ez of buffer `buf` (the one the step in progress writes) of every
+// component; 1: the psi fields.
+template <typename T> int fill_ghost(lbm_ctx *to, lbm_ctx *from, int from_plane, int to_plane, int ez, int what, int buf) {
     if (what == 1) {
         PlaneList one = {{0}};
         T *pa = at<T>(to, to->lay.psi[0]);
         const T *qa = at<T>(from, from->lay.psi[0]);
         for (int s = 0; s < 2; s++)  // planar psi_A | psi_B (split kernels)
-            if (int rc = copy_planes<T>(to, qa + s * from->g.N, pa + s * to->g.N, from->g.N, to->g.N, from_plane, to_plane, 1, one)) return rc;
+            if (int rc = copy_planes<T>(to, to->slab_stream, qa + s * from->g.N, pa + s * to->g.N, from->g.N, to->g.N, from_plane, to_plane, 1, one))
+                return rc;
         return LBM_OK;
     }
     PlaneList dirs = {{0}};
@@ -443,14 +448,14 @@ template <typename T> int fill_ghost(lbm_ctx *to, lbm_ctx *from, int from_plane,
     for (int i = 0; i < to->Q; i++)
         if (e[3 * i + 2] == ez) dirs.dir[nd++] = i;
     for (int s = 0; s < to->ncomp; s++)
-        if (int rc = copy_planes<T>(to, at<T>(from, from->lay.store[s][from->cur]), at<T>(to, to->lay.store[s][to->cur]),
+        if (int rc = copy_planes<T>(to, to->slab_stream, at<T>(from, from->lay.store[s][buf]), at<T>(to, to->lay.store[s][buf]),
                                     from->g.N, to->g.N, from_plane, to_plane, nd, dirs)) return rc;
     return LBM_OK;
 }
 
-int fill_ghost_any(lbm_ctx *to, lbm_ctx *from, int from_plane, int to_plane, int ez, int what) {
-    return to->rs == 4 ? fill_ghost<float>(to, from, from_plane, to_plane, ez, what)
-                       : fill_ghost<double>(to, from, from_plane, to_plane, ez, what);
+int fill_ghost_any(lbm_ctx *to, lbm_ctx *from, int from_plane, int to_plane, int ez, int what, int buf) {
+    return to->rs == 4 ? fill_ghost<float>(to, from, from_plane, to_plane, ez, what, buf)
+                       : fill_ghost<double>(to, from, from_plane, to_plane, ez, what, buf);
 }
 
 // Slabs may live on different devices: launches and event calls for a slab run with its device current.
@@ -462,59 +467,70 @@ struct DeviceGuard {
     ~DeviceGuard() { if (saved >= 0 && saved != current()) cudaSetDevice(saved); }
 };
 
-// All ghost planes of all slabs from their neighbours' boundary interior planes.  Streams: each slab's
-// copies run on its own stream after the neighbour's work enqueued so far (event), so slabs on different
-// streams / devices stay ordered; with one shared stream the events are skipped.
-int exchange_ghosts(lbm_ctx *const *slabs, int count, int periodic_z, int what) {
-    DeviceGuard dev;
-    bool one_stream = true;
-    for (int k = 1; k < count; k++)
-        one_stream = one_stream && slabs[k]->stream == slabs[0]->stream && slabs[k]->device == slabs[0]->device;
-    if (!one_stream)
-        for (int k = 0; k < count; k++) {
-            lbm_ctx *c = slabs[k];
-            dev.use(c);
-            if (!c->slab_event && cudaEventCreateWithFlags(&c->slab_event, cudaEventDisableTiming) != cudaSuccess)
-                return fail(c, LBM_ECUDA, "cudaEventCreate failed");
-            if (cudaEventRecord(c->slab_event, c->stream) != cudaSuccess) return fail(c, LBM_ECUDA, "cudaEventRecord failed");
-        }
-    for (int k = 0; k < count; k++) {
-        lbm_ctx *c = slabs[k];
-        lbm_ctx *below = k > 0 ? slabs[k - 1] : (periodic_z ? slabs[count - 1] : nullptr);
-        lbm_ctx *above = k + 1 < count ? slabs[k + 1] : (periodic_z ? slabs[0] : nullptr);
+struct Slabs {
+    lbm_ctx *const *c;
+    int count, periodic;
+    lbm_ctx *below(int k) const { return k > 0 ? c[k - 1] : (periodic ? c[count - 1] : nullptr); }
+    lbm_ctx *above(int k) const { return k + 1 < count ? c[k + 1] : (periodic ? c[0] : nullptr); }
+};
+
+int slab_resources(lbm_ctx *c) {
+    if (!c->slab_stream && cudaStreamCreateWithFlags(&c->slab_stream, cudaStreamNonBlocking) != cudaSuccess) return fail(c, LBM_ECUDA, "cudaStreamCreate failed");
+    if (!c->slab_event && cudaEventCreateWithFlags(&c->slab_event, cudaEventDisableTiming) != cudaSuccess) return fail(c, LBM_ECUDA, "cudaEventCreate failed");
+    if (!c->slab_event2 && cudaEventCreateWithFlags(&c->slab_event2, cudaEventDisableTiming) != cudaSuccess) return fail(c, LBM_ECUDA, "cudaEventCreate failed");
+    return LBM_OK;
+}
+
+// One pass (a whole step, or one phase of a Shan-Chen step) over every slab, the way section 3.6 of the
+// paper orders it: the two boundary interior planes first; as soon as they are done, the ghost
+// planes of the neighbours are filled from them on a side stream, concurrently with the bulk launch.
+//   phase: sc_phase of the launches (0 whole step, 1 macro fields, 2 collide); what: 0 populations, 1 psi.
+int slab_pass(const Slabs &S, DeviceGuard &dev, int phase, int what) {
+    auto launch = [&](lbm_ctx *c, int z0, int zc) -> int {
+        if (zc <= 0) return LBM_OK;
+        c->zsel0 = z0; c->zselc = zc; c->no_advance = true; c->sc_phase = phase;
+        const int rc = c->vt->step(c, 1);
+        c->zsel0 = 0; c->zselc = c->g.nz; c->no_advance = false; c->sc_phase = 0;
+        return rc;
+    };
+    for (int k = 0; k < S.count; k++) {  // boundary planes: local z = 1 and z = nz - 2
+        lbm_ctx *c = S.c[k];
         dev.use(c);
-        for (lbm_ctx *nb : {below, above})
-            if (nb && !one_stream && nb != c && cudaStreamWaitEvent(c->stream, nb->slab_event, 0) != cudaSuccess)
-                return fail(c, LBM_ECUDA, "cudaStreamWaitEvent failed");
-        // lower ghost (plane 0) <- top interior plane of the slab below: what moves up (e_z = +1)
-        if (below) if (int rc = fill_ghost_any(c, below, below->g.nz - 2, 0, +1, what)) return rc;
-        // upper ghost (plane nz-1) <- bottom interior plane (1) of the slab above: what moves down (e_z = -1)
-        if (above) if (int rc = fill_ghost_any(c, above, 1, c->g.nz - 1, -1, what)) return rc;
+        if (int rc = launch(c, 1, 1)) return rc;
+        if (c->g.nz - 2 > 1) if (int rc = launch(c, c->g.nz - 2, 1)) return rc;
+        if (cudaEventRecord(c->slab_event, c->stream) != cudaSuccess) return fail(c, LBM_ECUDA, "cudaEventRecord failed");
     }
-    if (!one_stream)  // a slab must not run ahead and overwrite planes a neighbour's copy is still reading
-        for (int k = 0; k < count; k++) {
-            dev.use(slabs[k]);
-            if (cudaEventRecord(slabs[k]->slab_event, slabs[k]->stream) != cudaSuccess) return fail(slabs[k], LBM_ECUDA, "cudaEventRecord failed");
-        }
-    if (!one_stream)
-        for (int k = 0; k < count; k++) {
-            lbm_ctx *c = slabs[k];
-            dev.use(c);
-            lbm_ctx *below = k > 0 ? slabs[k - 1] : (periodic_z ? slabs[count - 1] : nullptr);
-            lbm_ctx *above = k + 1 < count ? slabs[k + 1] : (periodic_z ? slabs[0] : nullptr);
-            for (lbm_ctx *nb : {below, above})
-                if (nb && nb != c && cudaStreamWaitEvent(c->stream, nb->slab_event, 0) != cudaSuccess)
-                    return fail(c, LBM_ECUDA, "cudaStreamWaitEvent failed");
-        }
+    for (int k = 0; k < S.count; k++) {  // ghost planes <- the neighbours' fresh boundary planes (side stream)
+        lbm_ctx *c = S.c[k], *below = S.below(k), *above = S.above(k);
+        dev.use(c);
+        const int buf = c->cur ^ 1;  // the buffer this step writes (ignored for psi)
+        for (lbm_ctx *nb : {c, below, above})
+            if (nb && cudaStreamWaitEvent(c->slab_stream, nb->slab_event, 0) != cudaSuccess) return fail(c, LBM_ECUDA, "cudaStreamWaitEvent failed");
+        // lower ghost (plane 0) <- top interior plane of the slab below: what moves up (e_z = +1)
+        if (below) if (int rc = fill_ghost_any(c, below, below->g.nz - 2, 0, +1, what, buf)) return rc;
+        // upper ghost (plane nz-1) <- bottom interior plane (1) of the slab above: what moves down (e_z = -1)
+        if (above) if (int rc = fill_ghost_any(c, above, 1, c->g.nz - 1, -1, what, buf)) return rc;
+        if (cudaEventRecord(c->slab_event2, c->slab_stream) != cudaSuccess) return fail(c, LBM_ECUDA, "cudaEventRecord failed");
+    }
+    for (int k = 0; k < S.count; k++) {  // bulk planes 2 .. nz - 3, overlapping the copies
+        lbm_ctx *c = S.c[k];
+        dev.use(c);
+        if (int rc = launch(c, 2, c->g.nz - 4)) return rc;
+    }
+    for (int k = 0; k < S.count; k++) {  // nobody goes on before its ghosts are filled and its planes have been read
+        lbm_ctx *c = S.c[k];
+        dev.use(c);
+        for (lbm_ctx *nb : {c, S.below(k), S.above(k)})
+            if (nb && cudaStreamWaitEvent(c->stream, nb->slab_event2, 0) != cudaSuccess) return fail(c, LBM_ECUDA, "cudaStreamWaitEvent failed");
+    }
     return LBM_OK;
 }
 
 }  // namespace
 
-static int check_state(lbm_ctx *c);
-
 LBM_API int lbm_step_slabs(lbm_ctx *const *slabs, int count, int periodic_z, int n) {
     if (!slabs || count < 1) return fail(nullptr, LBM_EINVAL, "slabs is NULL or count < 1");
+    DeviceGuard dev;
     for (int k = 0; k < count; k++) {
         lbm_ctx *c = slabs[k];
         CHECK_CTX(c);
@@ -526,32 +542,18 @@ LBM_API int lbm_step_slabs(lbm_ctx *const *slabs, int count, int periodic_z, int
         const lbm_ctx *a = slabs[0];
         if (c->g.nx != a->g.nx || c->g.ny != a->g.ny || c->p.model != a->p.model || c->rs != a->rs || c->cur != a->cur || c->steps != a->steps)
             return fail(c, LBM_EINVAL, "slabs: contexts differ in nx, ny, model, precision or time step");
+        dev.use(c);
+        if (int rc = slab_resources(c)) return rc;
     }
-    DeviceGuard dev;
+    const Slabs S = {slabs, count, periodic_z};
     for (int t = 0; t < n; t++) {
         if (slabs[0]->p.model == LBM_SC2) {
-            for (int k = 0; k < count; k++) {
-                dev.use(slabs[k]);
-                slabs[k]->sc_phase = 1;
-                const int rc = slabs[k]->vt->step(slabs[k], 1);
-                slabs[k]->sc_phase = 0;
-                if (rc) return rc;
-            }
-            if (int rc = exchange_ghosts(slabs, count, periodic_z, 1)) return rc;  // psi planes (eq. 10 reads neighbours)
-            for (int k = 0; k < count; k++) {
-                dev.use(slabs[k]);
-                slabs[k]->sc_phase = 2;
-                const int rc = slabs[k]->vt->step(slabs[k], 1);
-                slabs[k]->sc_phase = 0;
-                if (rc) return rc;
-            }
+            if (int rc = slab_pass(S, dev, 1, 1)) return rc;  // macro fields; psi planes exchanged (eq. 10 reads neighbours)
+            if (int rc = slab_pass(S, dev, 2, 0)) return rc;  // collide; the crossing populations of the new state exchanged
         } else {
-            for (int k = 0; k < count; k++) {
-                dev.use(slabs[k]);
-                if (int rc = slabs[k]->vt->step(slabs[k], 1)) return rc;
-            }
+            if (int rc = slab_pass(S, dev, 0, 0)) return rc;
         }
-        if (int rc = exchange_ghosts(slabs, count, periodic_z, 0)) return rc;  // the crossing populations of the new state
+        for (int k = 0; k < count; k++) { slabs[k]->cur ^= 1; slabs[k]->steps++; }
     }
     return LBM_OK;
 }

@@ -47,6 +47,12 @@ struct lbm_ctx {
     int resident_state; // 0 not probed yet, 1 launchable, -1 not launchable here (fall back for good)
     int span_bx;        // tuning: block width (threads along x) of the step kernels, 0 = default
     bool all_bulk;      // no node of the geometry is SOLID / BOUNDARY / special: the step kernels skip the type array
+    // lbm_step_slabs only: the next vt->step call covers z-planes [zsel0, zsel0 + zselc) and, with no_advance,
+    // neither flips the buffers nor counts a step (boundary planes are launched before the bulk)
+    int zsel0, zselc;
+    bool no_advance;
+    cudaStream_t slab_stream;  // side stream of the ghost-plane copies, so that they overlap the bulk launch
+    cudaEvent_t slab_event2;   // "this slab's ghost planes are filled"
     int sc_phase;       // lbm_step_slabs only: which part of a Shan-Chen step the next vt->step call runs (see lbm_steps.cuh)
     cudaEvent_t slab_event;  // lbm_step_slabs only: "this slab's kernels up to here are enqueued", created on first use
     int sc_split;       // Shan-Chen: > 0 = split variant (one collide launch per component), nodes per thread
@@ -131,6 +137,8 @@ namespace {
 struct Launch { dim3 grid, block; };
 
 // Step kernels: V nodes per thread along x, 2-D blocks (bx packs) x (by rows).
+Geom launch_geom(const lbm_ctx *c) { Geom g = c->g; g.z0 = c->zsel0; return g; }  // Geom of a (partial) step launch
+
 Launch span_launch(const lbm_ctx *c, int V, int max_threads = 256) {
     const int nxv = c->g.nx / V;
     int bx = nxv > 32 ? 64 : 32;
@@ -140,7 +148,7 @@ Launch span_launch(const lbm_ctx *c, int V, int max_threads = 256) {
     while (by > 1 && by / 2 >= c->g.ny) by /= 2;
     Launch l;
     l.block = dim3(bx, by, 1);
-    l.grid = dim3((nxv + bx - 1) / bx, (c->g.ny + by - 1) / by, c->g.nz);
+    l.grid = dim3((nxv + bx - 1) / bx, (c->g.ny + by - 1) / by, c->zselc);
     return l;
 }
 

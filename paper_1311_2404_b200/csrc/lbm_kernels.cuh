@@ -31,6 +31,7 @@ __device__ __forceinline__ bool mask_is_solid(uint8_t m) { return m != MASK_FLUI
 struct Geom {
     int nx, ny, nz;
     int64_t N;
+    int z0;  // first z-plane this launch covers (blockIdx.z counts from it): 0 except in lbm_step_slabs
 };
 
 // Element offsets from node n to its periodic neighbours along each axis: m = coordinate - 1,
@@ -100,7 +101,7 @@ __device__ __forceinline__ void gather(const T *__restrict__ src, int n, int64_t
 __device__ __forceinline__ bool thread_node(const Geom &g, int &x, int &y, int &z, int &n) {
     x = blockIdx.x * blockDim.x + threadIdx.x;
     y = blockIdx.y;
-    z = blockIdx.z;
+    z = blockIdx.z + g.z0;
     n = (z * g.ny + y) * g.nx + x;
     return x < g.nx;
 }
@@ -213,7 +214,7 @@ struct Span {
 template <int V> __device__ __forceinline__ bool thread_span(const Geom &g, Span &s) {
     s.x0 = (blockIdx.x * blockDim.x + threadIdx.x) * V;
     s.y = blockIdx.y * blockDim.y + threadIdx.y;
-    s.z = blockIdx.z;
+    s.z = blockIdx.z + g.z0;
     if (s.x0 >= g.nx || s.y >= g.ny) return false;
     s.row = (s.z * g.ny + s.y) * g.nx;
     s.xm = (s.x0 == 0) ? g.nx - 1 : s.x0 - 1;
@@ -385,7 +386,7 @@ step_rows_kernel(Geom g, const uint32_t *__restrict__ link, const T *__restrict_
     Span s;
     s.x0 = (blockIdx.x * blockDim.x + threadIdx.x) * V;
     if (s.x0 >= g.nx) return;
-    s.z = blockIdx.z;
+    s.z = blockIdx.z + g.z0;
     s.xm = (s.x0 == 0) ? g.nx - 1 : s.x0 - 1;
     s.xp = (s.x0 + V == g.nx) ? 0 : s.x0 + V;
     const int y0 = blockIdx.y * rows, y1 = min(y0 + rows, g.ny);
@@ -677,7 +678,7 @@ __device__ __forceinline__ Nbr span_node_neighbours(const Geom &g, const Span &s
 template <int V> __device__ __forceinline__ bool thread_span_all(const Geom &g, Span &s) {
     s.x0 = (blockIdx.x * blockDim.x + threadIdx.x) * V;
     s.y = blockIdx.y * blockDim.y + threadIdx.y;
-    s.z = blockIdx.z;
+    s.z = blockIdx.z + g.z0;
     const bool valid = s.x0 < g.nx && s.y < g.ny;
     const int y = valid ? s.y : 0;
     s.row = (s.z * g.ny + y) * g.nx;

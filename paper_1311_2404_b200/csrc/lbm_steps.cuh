@@ -40,10 +40,11 @@ template <class L, typename T> struct Steps {
         if constexpr (V <= 2 && sizeof(I) == 4) {
             if (c->rows > 0) {  // obstacle-rich geometry: row-walking kernel, link words one row ahead
                 const int nxv = c->g.nx / V, bx = c->span_bx > 0 ? c->span_bx : (nxv > 32 ? 64 : 32);
-                const dim3 grid((nxv + bx - 1) / bx, (c->g.ny + c->rows - 1) / c->rows, c->g.nz);
+                const dim3 grid((nxv + bx - 1) / bx, (c->g.ny + c->rows - 1) / c->rows, c->zselc);
                 for (int t = 0; t < n; t++) {
-                    step_rows_kernel<L, T, V, I, MODEL, FORCE><<<grid, bx, 0, c->stream>>>(c->g, link(c), src(c, 0), dst(c, 0), rp, c->rows);
+                    step_rows_kernel<L, T, V, I, MODEL, FORCE><<<grid, bx, 0, c->stream>>>(launch_geom(c), link(c), src(c, 0), dst(c, 0), rp, c->rows);
                     if (int rc = check_launch(c, "step_rows_kernel")) return rc;
+                    if (c->no_advance) continue;
                     c->cur ^= 1;
                     c->steps++;
                 }
@@ -51,8 +52,9 @@ template <class L, typename T> struct Steps {
             }
         }
         for (int t = 0; t < n; t++) {
-            step_kernel<L, T, V, I, MODEL, FORCE><<<l.grid, l.block, 0, c->stream>>>(c->g, type_or_null(c), link(c), src(c, 0), dst(c, 0), rp);
+            step_kernel<L, T, V, I, MODEL, FORCE><<<l.grid, l.block, 0, c->stream>>>(launch_geom(c), type_or_null(c), link(c), src(c, 0), dst(c, 0), rp);
             if (int rc = check_launch(c, "step_kernel")) return rc;
+            if (c->no_advance) continue;
             c->cur ^= 1;
             c->steps++;
         }
@@ -177,16 +179,17 @@ template <class L, typename T> struct Steps {
             // slab's ghost layers are exchanged in between), 0 = the whole step
             if (c->sc_phase != 2) {
                 sc_fields_split_kernel<L, T, V, I, PSI><<<l.grid, l.block, 0, c->stream>>>(
-                    c->g, type_or_null(c), link(c), src(c, 0), src(c, 1), psiA, psiB, up, rA.inv_tau, rB.inv_tau);
+                    launch_geom(c), type_or_null(c), link(c), src(c, 0), src(c, 1), psiA, psiB, up, rA.inv_tau, rB.inv_tau);
                 if (int rc = check_launch(c, "sc_fields_split_kernel")) return rc;
             }
             if (c->sc_phase == 1) continue;
             sc_collide_split_kernel<L, T, V, I, PSI, FS><<<l.grid, l.block, 0, c->stream>>>(
-                c->g, type_or_null(c), link(c), src(c, 0), dst(c, 0), psiB, up, rA, T(c->p.sc_G));
+                launch_geom(c), type_or_null(c), link(c), src(c, 0), dst(c, 0), psiB, up, rA, T(c->p.sc_G));
             if (int rc = check_launch(c, "sc_collide_split_kernel")) return rc;
             sc_collide_split_kernel<L, T, V, I, PSI, FS><<<l.grid, l.block, 0, c->stream>>>(
-                c->g, type_or_null(c), link(c), src(c, 1), dst(c, 1), psiA, up, rB, T(c->p.sc_G));
+                launch_geom(c), type_or_null(c), link(c), src(c, 1), dst(c, 1), psiA, up, rB, T(c->p.sc_G));
             if (int rc = check_launch(c, "sc_collide_split_kernel")) return rc;
+            if (c->no_advance) continue;
             c->cur ^= 1;
             c->steps++;
         }
