@@ -139,16 +139,15 @@ struct Launch { dim3 grid, block; };
 // Step kernels: V nodes per thread along x, 2-D blocks (bx packs) x (by rows).
 Geom launch_geom(const lbm_ctx *c) { Geom g = c->g; g.z0 = c->zsel0; return g; }  // Geom of a (partial) step launch
 
+// Step kernels: V nodes per thread along x; 1-D blocks over the packs of a z-plane (rows back to back).
 Launch span_launch(const lbm_ctx *c, int V, int max_threads = 256) {
-    const int nxv = c->g.nx / V;
-    int bx = nxv > 32 ? 64 : 32;
-    if (c->span_bx > 0 && c->span_bx <= max_threads) bx = c->span_bx;
-    int by = (c->block_threads < max_threads ? c->block_threads : max_threads) / bx;
-    if (by < 1) by = 1;
-    while (by > 1 && by / 2 >= c->g.ny) by /= 2;
+    const int64_t packs = (int64_t)(c->g.nx / V) * c->g.ny;
+    int threads = c->block_threads < max_threads ? c->block_threads : max_threads;
+    if (c->span_bx > 0 && c->span_bx <= max_threads) threads = c->span_bx;
+    while (threads > 32 && threads / 2 >= packs) threads /= 2;
     Launch l;
-    l.block = dim3(bx, by, 1);
-    l.grid = dim3((nxv + bx - 1) / bx, (c->g.ny + by - 1) / by, c->zselc);
+    l.block = dim3(threads, 1, 1);
+    l.grid = dim3((unsigned)((packs + threads - 1) / threads), 1, c->zselc);
     return l;
 }
 

@@ -39,8 +39,9 @@ template <class L, typename T> struct Steps {
         }
         if constexpr (V <= 2 && sizeof(I) == 4) {
             if (c->rows > 0) {  // obstacle-rich geometry: row-walking kernel, link words one row ahead
-                const int nxv = c->g.nx / V, bx = c->span_bx > 0 ? c->span_bx : (nxv > 32 ? 64 : 32);
-                const dim3 grid((nxv + bx - 1) / bx, (c->g.ny + c->rows - 1) / c->rows, c->zselc);
+                const int bx = (c->span_bx > 0 && c->span_bx <= 128) ? c->span_bx : 64;
+                const int64_t spans = (int64_t)(c->g.nx / V) * ((c->g.ny + c->rows - 1) / c->rows);  // (x-pack, y-chunk) pairs per z-plane
+                const dim3 grid((unsigned)((spans + bx - 1) / bx), 1, c->zselc);
                 for (int t = 0; t < n; t++) {
                     step_rows_kernel<L, T, V, I, MODEL, FORCE><<<grid, bx, 0, c->stream>>>(launch_geom(c), link(c), src(c, 0), dst(c, 0), rp, c->rows);
                     if (int rc = check_launch(c, "step_rows_kernel")) return rc;
