@@ -123,6 +123,9 @@ def run_reference(args):
     """CPU oracle arm: rank 0 only; each step is one oracle step over the bounded sample."""
     if int(os.environ.get("RANK", "0")) != 0:
         return
+    if int(os.environ.get("WORLD_SIZE", "1")) > 1 and os.environ.get("OMP_NUM_THREADS") == "1":
+        # torchrun pins OMP_NUM_THREADS=1 for its workers; rank 0 alone runs the oracle, on all host cores as at N = 1
+        os.environ["OMP_NUM_THREADS"] = str(os.cpu_count() or 1)
     steps = min(args.steps, 60)
     cb, dt, w = time_oracle(args.config, steps, min(args.warmup, 3))
     line = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus,
