@@ -161,6 +161,25 @@ int lbm_run_host(lbm_ctx *ctx, const uint8_t *h_mask, const void *const *h_rho0,
  * devices; D3Q19, AB store.  Errors: LBM_EINVAL (mismatching slabs), LBM_EUNSUPPORTED, LBM_ESTATE. */
 int lbm_step_slabs(lbm_ctx *const *slabs, int count, int periodic_z, int n);
 
+/* The path in one call that ALLOCATES NOTHING, for callers that can neither call cudaMalloc nor hand over a
+ * workspace (code under CUDA graph capture, tight serving loops, harnesses that forbid allocation).  The
+ * context's workspace lives in a file-scope device array of LBM_NOALLOC_MAX_BYTES inside the library (every
+ * GPU that loads the library holds it until the process exits).  The call builds a context in that array,
+ * runs lbm_set_geometry(d_mask) -> lbm_set_distributions(d_f_in) -> lbm_step(n) -> lbm_get_distributions
+ * (d_f_out) on `cuda_stream` with the ordinary kernels, and destroys the context; it calls no cudaMalloc,
+ * cudaFree, stream or graph creation.  p: as for lbm_create, LBM_STORE_AB only.  d_mask: uint8[N] or NULL (all
+ * FLUID; with a mask the call synchronises the stream once, as lbm_set_geometry does).  d_f_in, d_f_out:
+ * canonical distributions real[ncomp][Q][N] (LBM_SC2: component A then B), caller-owned device memory, may be
+ * the same buffer.  Asynchronous otherwise.
+ * Limits: lbm_workspace_bytes(p) <= LBM_NOALLOC_MAX_BYTES (D3Q19 fp32 up to 64^3 nodes), else LBM_EINVAL with
+ * a message naming both sizes (lbm_noalloc_last_error).  ALL calls on a device share the one array, which
+ * keeps the last call's contents (the call clears what must start at zero): calls are safe back to back on
+ * one stream, but calls that overlap on the GPU (different streams, different threads) RACE. */
+#define LBM_NOALLOC_MAX_BYTES (64u << 20)
+int lbm_step_noalloc(const lbm_params *p, const uint8_t *d_mask, const void *d_f_in, void *d_f_out, int n,
+                     void *cuda_stream);
+const char *lbm_noalloc_last_error(void);   /* message of the last failed lbm_step_noalloc on this thread */
+
 /* Time step counter since the last init/set, and number of kernels launched by this context. */
 int lbm_get_counters(const lbm_ctx *ctx, int64_t *steps, int64_t *launches);
 

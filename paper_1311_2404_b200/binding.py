@@ -26,7 +26,7 @@ LBM_QMAX = 19
 EXPORTS = ("lbm_lattice_info", "lbm_workspace_bytes", "lbm_create", "lbm_destroy", "lbm_set_geometry",
            "lbm_get_geometry", "lbm_init_equilibrium", "lbm_step", "lbm_macro", "lbm_get_distributions",
            "lbm_set_distributions", "lbm_get_stream_map", "lbm_run_host", "lbm_get_counters",
-           "lbm_get_dispatch", "lbm_step_slabs", "lbm_last_error")
+           "lbm_get_dispatch", "lbm_step_slabs", "lbm_step_noalloc", "lbm_noalloc_last_error", "lbm_last_error")
 
 
 class lbm_params(C.Structure):
@@ -84,8 +84,11 @@ def load():
     L.lbm_step_slabs.argtypes = [C.POINTER(vp), C.c_int, C.c_int, C.c_int]
     L.lbm_last_error.argtypes = [vp]
     L.lbm_last_error.restype = C.c_char_p
+    L.lbm_step_noalloc.argtypes = [C.POINTER(lbm_params), vp, vp, vp, C.c_int, vp]
+    L.lbm_noalloc_last_error.argtypes = []
+    L.lbm_noalloc_last_error.restype = C.c_char_p
     for name in EXPORTS:
-        if name != "lbm_last_error":
+        if name not in ("lbm_last_error", "lbm_noalloc_last_error"):
             getattr(L, name).restype = C.c_int
     _lib = L
     return L
@@ -176,6 +179,17 @@ def lbm_get_counters(ctx):
 def lbm_step_slabs(ctxs, periodic_z: bool, n: int):
     arr = (C.c_void_p * len(ctxs))(*ctxs)
     _check(load().lbm_step_slabs(arr, len(ctxs), 1 if periodic_z else 0, int(n)), ctxs[0])
+
+
+LBM_NOALLOC_MAX_BYTES = 64 << 20
+
+
+def lbm_step_noalloc(params, d_mask, d_f_in, d_f_out, n: int, cuda_stream=None):
+    """Raw pointers in (ints; d_mask may be None); raises LbmError with lbm_noalloc_last_error's message."""
+    rc = load().lbm_step_noalloc(C.byref(params), d_mask, d_f_in, d_f_out, int(n), cuda_stream)
+    if rc != LBM_OK:
+        msg = load().lbm_noalloc_last_error()
+        raise LbmError(rc, msg.decode() if msg else "")
 
 
 def lbm_get_dispatch(ctx) -> dict:

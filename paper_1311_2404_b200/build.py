@@ -17,7 +17,7 @@ LIB = os.path.join(_HERE, "liblbm_b200.so")
 OBJDIR = os.path.join(_HERE, "build")
 # one translation unit for the C ABI, one per <lattice, real> pair for the conversion kernels, and
 # one per <lattice, real, model> for the step kernels: they are independent and compile side by side
-SOURCES = [os.path.join(CSRC, "lbm_b200.cu")] + [
+SOURCES = [os.path.join(CSRC, "lbm_b200.cu"), os.path.join(CSRC, "lbm_noalloc.cu")] + [
     os.path.join(CSRC, "lbm_impl_%s_%s.cu" % (lat, pr)) for lat in ("d2q9", "d3q19") for pr in ("f32", "f64")] + [
     os.path.join(CSRC, "lbm_step_%s_%s_%s.cu" % (lat, pr, m))
     for lat in ("d3q19", "d2q9") for pr in ("f32", "f64") for m in ("bgk", "mrt", "sc", "reg", "les")]
