@@ -196,14 +196,14 @@ typedef struct {
     int32_t block_threads;           /* threads per block of the step kernels                         */
     int32_t sc_split;                /* LBM_SC2: 1 = one collide launch per component, 0 = one
                                         launch for both                                               */
-    int32_t reserved_;
+    int32_t rows_strided;            /* row-walking kernel: 1 = a thread's two nodes lie one warp width apart (nx % 64 == 0) */
 } lbm_dispatch;
 int lbm_get_dispatch(const lbm_ctx *ctx, lbm_dispatch *out);
 
 /* Test-only tuning knobs.  Environment variables, read at lbm_create / lbm_set_geometry and honoured
  * ONLY if LBM_TUNING=1 is set too: LBM_VEC (1|2|4 nodes per thread), LBM_IDX64 (1: 64-bit slot indices),
  * LBM_BLOCK_X, LBM_BLOCK_THREADS (multiples of 32), LBM_ROWS (rows per block of the row-walking kernel,
- * 0 = off), LBM_NO_GRAPH, LBM_NO_RESIDENT, LBM_RESIDENT_MAX (largest lattice of the cluster-resident
+ * 0 = off), LBM_ROWS_STRIDED, LBM_NO_GRAPH, LBM_NO_RESIDENT, LBM_RESIDENT_MAX (largest lattice of the cluster-resident
  * path), LBM_SC_SPLIT (0: monolithic two-component collide kernel), LBM_SC_FIELDS_VEC, LBM_SPAN_BX.  They select among kernels that all pass the same parity tests; they are not part of the ABI. */
 
 const char *lbm_last_error(const lbm_ctx *ctx);

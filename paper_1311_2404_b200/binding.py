@@ -96,7 +96,7 @@ def load():
 
 class lbm_dispatch(C.Structure):
     _fields_ = [(n, C.c_int32) for n in ("nodes_per_thread", "index_bits", "graph_replay", "resident_nodes_per_cta",
-                                         "resident_ctas", "rows_per_block", "block_threads", "sc_split", "reserved_")]
+                                         "resident_ctas", "rows_per_block", "block_threads", "sc_split", "rows_strided")]
 
 
 def make_params(lattice, model, precision, nx, ny, nz=1, tau=(1.0, 1.0), rates=None,

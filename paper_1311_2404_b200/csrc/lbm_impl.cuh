@@ -57,6 +57,7 @@ struct lbm_ctx {
     cudaEvent_t slab_event;  // lbm_step_slabs only: "this slab's kernels up to here are enqueued", created on first use
     int sc_split;       // Shan-Chen: > 0 = split variant (one collide launch per component), nodes per thread
     int sc_fields_vec;  // Shan-Chen: nodes per thread of the macro-field pass (the collide pass uses `vec`)
+    int rows_strided;   // step_rows_strided_kernel instead of step_rows_kernel where nx allows (tuning: LBM_ROWS_STRIDED)
     int rows;           // > 0: obstacle-rich geometry (>= 20 % of the nodes not BULK): step_rows_kernel, rows per block
     bool idx32;         // Q * N < 2^32: slot numbers fit 32 bits (cheaper address arithmetic)
     int block_x;        // one-node-per-thread kernels: 1-D block along x

@@ -415,6 +415,64 @@ step_rows_kernel(Geom g, const uint32_t *__restrict__ link, const T *__restrict_
     }
 }
 
+// The same kernel with the thread's NPT nodes one warp width apart instead of adjacent (nx % (32 NPT) == 0):
+// lane l of a warp owns x = 32 NPT w + l + 32 k, k < NPT.  The per-lane source select forces scalar loads
+// either way; adjacent nodes make a warp's 4-byte loads stride 8 bytes (every sector requested twice, half of
+// it used: 330 M L1 sector requests for 4.5 GB of populations on c3), nodes a warp apart make every load and
+// store instruction of a warp one contiguous 128-byte line (4 whole sectors; 5 for the e_x = +-1 planes).
+template <class L, typename T, int NPT, typename I, int MODEL, int FORCE>
+__global__ void __launch_bounds__(128, sizeof(T) == 4 ? 6 : 3)
+step_rows_strided_kernel(Geom g, const uint32_t *__restrict__ link, const T *__restrict__ src, T *__restrict__ dst,
+                         Relax<T> rp, int rows) {
+    const unsigned per_row = (unsigned)g.nx / NPT, p = blockIdx.x * blockDim.x + threadIdx.x, chunk = p / per_row;
+    const unsigned q = p - chunk * per_row;
+    const int xb = (int)(q >> 5) * (32 * NPT) + (int)(q & 31u);  // x of node k = xb + 32 k
+    const int y0 = (int)chunk * rows, y1 = min(y0 + rows, g.ny);
+    if (y0 >= g.ny) return;
+    const int z = blockIdx.z + g.z0;
+    int xm[NPT], xp[NPT];  // periodic x - 1 / x + 1 of each node
+#pragma unroll
+    for (int k = 0; k < NPT; k++) {
+        const int x = xb + 32 * k;
+        xm[k] = x == 0 ? g.nx - 1 : x - 1;
+        xp[k] = x == g.nx - 1 ? 0 : x + 1;
+    }
+    uint32_t wn[NPT];
+#pragma unroll
+    for (int k = 0; k < NPT; k++) wn[k] = __ldg(link + ((z * g.ny + y0) * g.nx + xb + 32 * k));
+    for (int y = y0; y < y1; y++) {
+        uint32_t w[NPT];
+#pragma unroll
+        for (int k = 0; k < NPT; k++) w[k] = wn[k];
+        const int row = (z * g.ny + y) * g.nx;
+        const Nbr o = neighbours(g, 1, y, z);
+        if (y + 1 < y1) {
+#pragma unroll
+            for (int k = 0; k < NPT; k++) wn[k] = __ldg(link + (row + g.nx + xb + 32 * k));
+        }
+        const uint32_t types = types_of_links<L, NPT>(w);
+        T h[NPT][L::Q];
+#pragma unroll
+        for (int i = 0; i < L::Q; i++) {
+            const int r = row + shift_yz<L>(i, -1, o);
+            const I plane = I(i) * I(g.N), own = I(L::opp(i)) * I(g.N) + I(row + xb);
+#pragma unroll
+            for (int k = 0; k < NPT; k++) {
+                const int xs = L::ex(i) == 0 ? xb + 32 * k : L::ex(i) == 1 ? xm[k] : xp[k];
+                const I idx = (i > 0 && reflected(w[k], i)) ? own + I(32 * k) : plane + I(r + xs);
+                h[k][i] = __ldg(src + idx);
+            }
+        }
+        // SOLID nodes run through as well (on whatever their pull returned) and store: a warp's store is then
+        // always four whole sectors; nothing ever reads a SOLID node's slots
+        update_span<L, T, NPT, MODEL, FORCE>(h, types & ~PACK_SOLID, rp);
+#pragma unroll
+        for (int i = 0; i < L::Q; i++)
+#pragma unroll
+            for (int k = 0; k < NPT; k++) __stcs(dst + (I(i) * I(g.N) + I(row + xb + 32 * k)), h[k][i]);
+    }
+}
+
 // ---- z-slab decomposition: ghost-plane exchange ------------------------------------
 // A slab context holds its share of the lattice as local planes 1 .. nz-2 plus one ghost plane below
 // (0) and above (nz-1).  After a step the ghost planes receive, from the neighbouring slab's boundary

@@ -38,6 +38,20 @@ template <class L, typename T> struct Steps {
         }
         }
         if constexpr (V <= 2 && sizeof(I) == 4) {
+            if constexpr (V == 2)
+            if (c->rows > 0 && c->rows_strided && c->g.nx % 64 == 0) {  // ... with the thread's two nodes a warp apart
+                const int bx = (c->span_bx > 0 && c->span_bx <= 128) ? c->span_bx : 64;
+                const int64_t spans = (int64_t)(c->g.nx / 2) * ((c->g.ny + c->rows - 1) / c->rows);
+                const dim3 grid((unsigned)((spans + bx - 1) / bx), 1, c->zselc);
+                for (int t = 0; t < n; t++) {
+                    step_rows_strided_kernel<L, T, 2, I, MODEL, FORCE><<<grid, bx, 0, c->stream>>>(launch_geom(c), link(c), src(c, 0), dst(c, 0), rp, c->rows);
+                    if (int rc = check_launch(c, "step_rows_strided_kernel")) return rc;
+                    if (c->no_advance) continue;
+                    c->cur ^= 1;
+                    c->steps++;
+                }
+                return LBM_OK;
+            }
             if (c->rows > 0) {  // obstacle-rich geometry: row-walking kernel, link words one row ahead
                 const int bx = (c->span_bx > 0 && c->span_bx <= 128) ? c->span_bx : 64;
                 const int64_t spans = (int64_t)(c->g.nx / V) * ((c->g.ny + c->rows - 1) / c->rows);  // (x-pack, y-chunk) pairs per z-plane

@@ -90,7 +90,8 @@ def test_random_cases_with_random_forced_variants(orc, monkeypatch, seed):
         w, store, chunks = random_case(rng)
         env = dict(LBM_VEC=str(rng.choice([1, 2, 4])), LBM_ROWS=str(rng.choice([0, 1, 2, 3])), LBM_SC_SPLIT=str(rng.integers(0, 2)),
                    LBM_NO_GRAPH=str(rng.integers(0, 2)), LBM_NO_RESIDENT=str(rng.integers(0, 2)), LBM_IDX64=str(int(rng.random() < 0.15)),
-                   LBM_BLOCK_THREADS=str(rng.choice([32, 64, 128, 256])), LBM_SC_FIELDS_VEC=str(rng.integers(1, 3)))
+                   LBM_BLOCK_THREADS=str(rng.choice([32, 64, 128, 256])), LBM_SC_FIELDS_VEC=str(rng.integers(1, 3)),
+                   LBM_ROWS_STRIDED=str(rng.integers(0, 2)))
         for k, v in env.items():
             monkeypatch.setenv(k, v)
         what = (seed, case, w.lattice, w.model, w.precision, store, w.force_scheme, (w.nx, w.ny, w.nz), env)

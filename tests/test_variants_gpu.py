@@ -14,7 +14,8 @@ pytestmark = pytest.mark.gpu
 
 # the Shan-Chen variant (split per-component collide kernels | one monolithic kernel) rides on the LBM_ROWS axis
 ENVS = [dict(LBM_TUNING="1", LBM_VEC=v, LBM_IDX64=i, LBM_ROWS=r, LBM_NO_GRAPH=g, LBM_NO_RESIDENT=g,
-             LBM_SC_SPLIT="1" if r == "0" else "0", LBM_SC_FIELDS_VEC="2" if g == "1" else "1")
+             LBM_SC_SPLIT="1" if r == "0" else "0", LBM_SC_FIELDS_VEC="2" if g == "1" else "1",
+             LBM_ROWS_STRIDED="1" if g == "0" else "0")   # nx = 64: the strided row-walking kernel applies at V = 2
         for v, i, r, g in itertools.product(("1", "2", "4"), ("0", "1"), ("0", "3"), ("0", "1"))]
 
 
@@ -57,6 +58,7 @@ def test_forced_variant_matches_oracle(orc, monkeypatch, env):
                     assert d["nodes_per_thread"] == int(env["LBM_VEC"])
                 rows_ok = store == B.LBM_STORE_AB and not idx64 and d["nodes_per_thread"] <= 2
                 assert d["rows_per_block"] == (int(env["LBM_ROWS"]) if rows_ok else 0)
+                assert d["rows_strided"] == int(d["rows_per_block"] > 0 and d["nodes_per_thread"] == 2 and env["LBM_ROWS_STRIDED"] == "1")
             for s in range(w.ncomp):
                 sim.init_equilibrium(w.rho[s], w.u[s], comp=s)
                 ref.init_equilibrium(w.rho[s], w.u[s], comp=s)
