@@ -45,7 +45,7 @@ def ncu_traffic(key: str):
         with open(TRAFFIC_FILE) as f:
             t = json.load(f)
         k = t["configs"][key]
-        return float(k["dram_bytes_per_step"]), "profiles/r02_traffic.json (ncu --set full at commit %s, kernel %s)" % (t["commit"], k["kernel"])
+        return float(k["dram_bytes_per_step"]), "profiles/r02_traffic.json (ncu --set full at commit %s, kernel %s)" % (k.get("commit", t["commit"]), k["kernel"])
     except Exception as e:  # missing file or key: say so instead of inventing a number
         return None, "no committed capture for %s (%s)" % (key, type(e).__name__)
 
