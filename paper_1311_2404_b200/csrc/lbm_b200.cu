@@ -120,6 +120,8 @@ int pick_vec(const lbm_params *p, double nonbulk_fraction, bool sc_split = false
     else if (sites < (1 << 20) && v > 2) v = 2;
     v = env_int("LBM_VEC", v, 1, widest);
     if (v == 3) v = 2;
+    // MRT, regularized LBGK and Smagorinsky lose at V = 4 (above): those kernels are not built (a quarter of the build)
+    if (!sc_split && p->model != LBM_BGK && p->model != LBM_SC2 && v > 2) v = 2;
     while (v > 1 && p->nx % v) v /= 2;
     return v;
 }

@@ -128,7 +128,7 @@ template <class L, typename T> struct Steps {
             c->resident_slog2 = 0;  // fall through to the step kernels, graphs from the next call on
             c->use_graph = c->g.N <= GRAPH_MAX_SITES;
         }
-        if constexpr (sizeof(T) == 4) {
+        if constexpr (sizeof(T) == 4 && MODEL == MODEL_BGK) {  // 4-node packs are built for LBGK only (pick_vec)
             if (c->vec == 4) return step_single_v<4, MODEL, FORCE>(c, n, rp);
         }
         if (c->vec == 2) return step_single_v<2, MODEL, FORCE>(c, n, rp);
