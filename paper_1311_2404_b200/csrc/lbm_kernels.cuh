@@ -891,6 +891,59 @@ aa_odd_kernel(Geom g, const uint8_t *__restrict__ type, const uint32_t *__restri
     aa_scatter_odd_span<L, T, V, I>(f, g, s, types, live, link, h);
 }
 
+// Odd AA step for obstacle-rich geometries (nx % 64 == 0), in the manner of step_rows_strided_kernel: a thread's
+// two nodes lie one warp width apart, the link words come first and every population is then read from the slot
+// the streaming rule names -- (ibar, x - e_i), or the node's own (i, x) for a reflected link -- in one batch of
+// line-contiguous scalar loads; after the collision h*_i goes to the slot the read of ibar came from.  A node reads
+// and writes exactly its own set of slots and all of a thread's loads precede its stores: no hazards.
+// SOLID nodes touch nothing (their neighbours' populations live in the slots around them).
+template <class L, typename T, int NPT, typename I, int MODEL, int FORCE>
+__global__ void __launch_bounds__(128, sizeof(T) == 4 ? 6 : 3)
+aa_odd_strided_kernel(Geom g, const uint32_t *__restrict__ link, T *f, Relax<T> rp) {
+    const unsigned per_row = (unsigned)g.nx / NPT, p = blockIdx.x * blockDim.x + threadIdx.x;
+    const int y = (int)(p / per_row);
+    if (y >= g.ny) return;
+    const unsigned q = p - (unsigned)y * per_row;
+    const int xb = (int)(q >> 5) * (32 * NPT) + (int)(q & 31u);  // x of node k = xb + 32 k
+    const int z = blockIdx.z + g.z0, row = (z * g.ny + y) * g.nx;
+    const Nbr o = neighbours(g, 1, y, z);
+    int xm[NPT], xp[NPT];
+    uint32_t w[NPT];
+#pragma unroll
+    for (int k = 0; k < NPT; k++) {
+        const int x = xb + 32 * k;
+        xm[k] = x == 0 ? g.nx - 1 : x - 1;
+        xp[k] = x == g.nx - 1 ? 0 : x + 1;
+        w[k] = __ldg(link + (row + x));
+    }
+    const uint32_t types = types_of_links<L, NPT>(w);
+    if (all_solid<NPT>(types)) return;
+    T h[NPT][L::Q];
+#pragma unroll
+    for (int i = 0; i < L::Q; i++) {
+        const int r = row + shift_yz<L>(i, -1, o);
+        const I from = I(L::opp(i)) * I(g.N), own = I(i) * I(g.N) + I(row + xb);
+#pragma unroll
+        for (int k = 0; k < NPT; k++) {
+            const int xs = L::ex(i) == 0 ? xb + 32 * k : L::ex(i) == 1 ? xm[k] : xp[k];
+            const I idx = (i > 0 && reflected(w[k], i)) ? own + I(32 * k) : from + I(r + xs);
+            h[k][i] = (w[k] & LINK_SELF_SOLID) ? T(0) : f[idx];
+        }
+    }
+    update_span<L, T, NPT, MODEL, FORCE>(h, types & ~PACK_SOLID, rp);
+#pragma unroll
+    for (int i = 0; i < L::Q; i++) {
+        const int r = row + shift_yz<L>(i, +1, o);
+        const I to = I(i) * I(g.N), own = I(L::opp(i)) * I(g.N) + I(row + xb);
+#pragma unroll
+        for (int k = 0; k < NPT; k++) {
+            const int xs = L::ex(i) == 0 ? xb + 32 * k : L::ex(i) == 1 ? xp[k] : xm[k];
+            const I idx = (i > 0 && reflected(w[k], L::opp(i))) ? own + I(32 * k) : to + I(r + xs);
+            if (!(w[k] & LINK_SELF_SOLID)) f[idx] = h[k][i];
+        }
+    }
+}
+
 // Conversions for the AA store (parity 0: before an even step, 1: before an odd step).
 template <class L, typename T, int MODE>  // MODE 0: set from canonical f, 1: get canonical f, 2: init f^eq, 3: macro
 __global__ void aa_convert_kernel(Geom g, int parity, const uint8_t *__restrict__ type,

@@ -27,8 +27,15 @@ template <class L, typename T> struct Steps {
         if constexpr (sizeof(I) == 4) {
         if (c->aa) {  // in place: even steps are local, odd steps move data; V-node packs on both
             T *f = at<T>(c, c->lay.store[0][0]);
+            bool strided = false;  // obstacle-rich geometry: odd steps with per-lane source select, nodes a warp apart
+            if constexpr (V == 2) strided = c->rows > 0 && c->rows_strided && c->g.nx % 64 == 0;
+            const int64_t half_row_threads = (int64_t)(c->g.nx / 2) * c->g.ny;
+            const dim3 sgrid((unsigned)((half_row_threads + 63) / 64), 1, c->zselc);
             for (int t = 0; t < n; t++) {
                 if (c->cur == 0) aa_even_kernel<L, T, V, I, MODEL, FORCE><<<l.grid, l.block, 0, c->stream>>>(c->g, type_or_null(c), f, rp);
+                else if (strided) {
+                    if constexpr (V == 2) aa_odd_strided_kernel<L, T, 2, I, MODEL, FORCE><<<sgrid, 64, 0, c->stream>>>(c->g, link(c), f, rp);
+                }
                 else aa_odd_kernel<L, T, V, I, MODEL, FORCE><<<l.grid, l.block, 0, c->stream>>>(c->g, type_or_null(c), link(c), f, rp);
                 if (int rc = check_launch(c, "aa_step_kernel")) return rc;
                 c->cur ^= 1;
