@@ -196,7 +196,7 @@ typedef struct {
     int32_t block_threads;           /* threads per block of the step kernels                         */
     int32_t sc_split;                /* LBM_SC2: 1 = one collide launch per component, 0 = one
                                         launch for both                                               */
-    int32_t rows_strided;            /* row-walking kernel: 1 = a thread's two nodes lie one warp width apart (nx % 64 == 0) */
+    int32_t rows_strided;            /* row-walking kernel: 1 = a thread's two nodes lie half a row apart (2 nodes per thread) */
 } lbm_dispatch;
 int lbm_get_dispatch(const lbm_ctx *ctx, lbm_dispatch *out);
 

@@ -581,7 +581,7 @@ LBM_API int lbm_get_dispatch(const lbm_ctx *c, lbm_dispatch *out) {
     out->resident_ctas = out->resident_nodes_per_cta ? c->resident_ctas : 0;
     out->rows_per_block = (c->rows > 0 && !c->aa && c->p.model != LBM_SC2 && c->idx32 && c->vec <= 2) ? c->rows : 0;
     out->block_threads = c->block_threads;
-    out->rows_strided = (out->rows_per_block > 0 && c->rows_strided && c->vec == 2 && c->g.nx % 64 == 0) ? 1 : 0;
+    out->rows_strided = (out->rows_per_block > 0 && c->rows_strided && c->vec == 2) ? 1 : 0;
     return LBM_OK;
 }
 

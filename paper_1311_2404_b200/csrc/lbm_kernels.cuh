@@ -415,31 +415,35 @@ step_rows_kernel(Geom g, const uint32_t *__restrict__ link, const T *__restrict_
     }
 }
 
-// The same kernel with the thread's NPT nodes one warp width apart instead of adjacent (nx % (32 NPT) == 0):
-// lane l of a warp owns x = 32 NPT w + l + 32 k, k < NPT.  The per-lane source select forces scalar loads
+// The same kernel with the thread's NPT nodes apart instead of adjacent (nx % NPT == 0): one warp width apart where
+// whole warps tile a row (lane l of warp w owns x = 32 NPT w + l + 32 k), else thread q of a row owns x = q + k nx / NPT,
+// so that consecutive lanes own consecutive nodes.  The per-lane source select forces scalar loads
 // either way; adjacent nodes make a warp's 4-byte loads stride 8 bytes (every sector requested twice, half of
-// it used: 330 M L1 sector requests for 4.5 GB of populations on c3), nodes a warp apart make every load and
+// it used: 330 M L1 sector requests for 4.5 GB of populations on c3), nodes part of a row apart make every load and
 // store instruction of a warp one contiguous 128-byte line (4 whole sectors; 5 for the e_x = +-1 planes).
 template <class L, typename T, int NPT, typename I, int MODEL, int FORCE>
 __global__ void __launch_bounds__(128, sizeof(T) == 4 ? 6 : 3)
 step_rows_strided_kernel(Geom g, const uint32_t *__restrict__ link, const T *__restrict__ src, T *__restrict__ dst,
                          Relax<T> rp, int rows) {
     const unsigned per_row = (unsigned)g.nx / NPT, p = blockIdx.x * blockDim.x + threadIdx.x, chunk = p / per_row;
+    // x of node k = xb + k XS: one warp width apart where whole warps tile the row (3 % faster on c3: a thread's two
+    // lines lie side by side), else the row in NPT equal parts
     const unsigned q = p - chunk * per_row;
-    const int xb = (int)(q >> 5) * (32 * NPT) + (int)(q & 31u);  // x of node k = xb + 32 k
+    const bool tiled = g.nx % (32 * NPT) == 0;
+    const int xb = tiled ? (int)(q >> 5) * (32 * NPT) + (int)(q & 31u) : (int)q, XS = tiled ? 32 : (int)per_row;
     const int y0 = (int)chunk * rows, y1 = min(y0 + rows, g.ny);
     if (y0 >= g.ny) return;
     const int z = blockIdx.z + g.z0;
     int xm[NPT], xp[NPT];  // periodic x - 1 / x + 1 of each node
 #pragma unroll
     for (int k = 0; k < NPT; k++) {
-        const int x = xb + 32 * k;
+        const int x = xb + XS * k;
         xm[k] = x == 0 ? g.nx - 1 : x - 1;
         xp[k] = x == g.nx - 1 ? 0 : x + 1;
     }
     uint32_t wn[NPT];
 #pragma unroll
-    for (int k = 0; k < NPT; k++) wn[k] = __ldg(link + ((z * g.ny + y0) * g.nx + xb + 32 * k));
+    for (int k = 0; k < NPT; k++) wn[k] = __ldg(link + ((z * g.ny + y0) * g.nx + xb + XS * k));
     for (int y = y0; y < y1; y++) {
         uint32_t w[NPT];
 #pragma unroll
@@ -448,7 +452,7 @@ step_rows_strided_kernel(Geom g, const uint32_t *__restrict__ link, const T *__r
         const Nbr o = neighbours(g, 1, y, z);
         if (y + 1 < y1) {
 #pragma unroll
-            for (int k = 0; k < NPT; k++) wn[k] = __ldg(link + (row + g.nx + xb + 32 * k));
+            for (int k = 0; k < NPT; k++) wn[k] = __ldg(link + (row + g.nx + xb + XS * k));
         }
         const uint32_t types = types_of_links<L, NPT>(w);
         T h[NPT][L::Q];
@@ -458,8 +462,8 @@ step_rows_strided_kernel(Geom g, const uint32_t *__restrict__ link, const T *__r
             const I plane = I(i) * I(g.N), own = I(L::opp(i)) * I(g.N) + I(row + xb);
 #pragma unroll
             for (int k = 0; k < NPT; k++) {
-                const int xs = L::ex(i) == 0 ? xb + 32 * k : L::ex(i) == 1 ? xm[k] : xp[k];
-                const I idx = (i > 0 && reflected(w[k], i)) ? own + I(32 * k) : plane + I(r + xs);
+                const int xs = L::ex(i) == 0 ? xb + XS * k : L::ex(i) == 1 ? xm[k] : xp[k];
+                const I idx = (i > 0 && reflected(w[k], i)) ? own + I(XS * k) : plane + I(r + xs);
                 h[k][i] = __ldg(src + idx);
             }
         }
@@ -469,7 +473,7 @@ step_rows_strided_kernel(Geom g, const uint32_t *__restrict__ link, const T *__r
 #pragma unroll
         for (int i = 0; i < L::Q; i++)
 #pragma unroll
-            for (int k = 0; k < NPT; k++) __stcs(dst + (I(i) * I(g.N) + I(row + xb + 32 * k)), h[k][i]);
+            for (int k = 0; k < NPT; k++) __stcs(dst + (I(i) * I(g.N) + I(row + xb + XS * k)), h[k][i]);
     }
 }
 
@@ -904,14 +908,15 @@ aa_odd_strided_kernel(Geom g, const uint32_t *__restrict__ link, T *f, Relax<T> 
     const int y = (int)(p / per_row);
     if (y >= g.ny) return;
     const unsigned q = p - (unsigned)y * per_row;
-    const int xb = (int)(q >> 5) * (32 * NPT) + (int)(q & 31u);  // x of node k = xb + 32 k
+    const bool tiled = g.nx % (32 * NPT) == 0;  // x of node k = xb + k XS, as in step_rows_strided_kernel
+    const int xb = tiled ? (int)(q >> 5) * (32 * NPT) + (int)(q & 31u) : (int)q, XS = tiled ? 32 : (int)per_row;
     const int z = blockIdx.z + g.z0, row = (z * g.ny + y) * g.nx;
     const Nbr o = neighbours(g, 1, y, z);
     int xm[NPT], xp[NPT];
     uint32_t w[NPT];
 #pragma unroll
     for (int k = 0; k < NPT; k++) {
-        const int x = xb + 32 * k;
+        const int x = xb + XS * k;
         xm[k] = x == 0 ? g.nx - 1 : x - 1;
         xp[k] = x == g.nx - 1 ? 0 : x + 1;
         w[k] = __ldg(link + (row + x));
@@ -925,8 +930,8 @@ aa_odd_strided_kernel(Geom g, const uint32_t *__restrict__ link, T *f, Relax<T> 
         const I from = I(L::opp(i)) * I(g.N), own = I(i) * I(g.N) + I(row + xb);
 #pragma unroll
         for (int k = 0; k < NPT; k++) {
-            const int xs = L::ex(i) == 0 ? xb + 32 * k : L::ex(i) == 1 ? xm[k] : xp[k];
-            const I idx = (i > 0 && reflected(w[k], i)) ? own + I(32 * k) : from + I(r + xs);
+            const int xs = L::ex(i) == 0 ? xb + XS * k : L::ex(i) == 1 ? xm[k] : xp[k];
+            const I idx = (i > 0 && reflected(w[k], i)) ? own + I(XS * k) : from + I(r + xs);
             h[k][i] = (w[k] & LINK_SELF_SOLID) ? T(0) : f[idx];
         }
     }
@@ -937,8 +942,8 @@ aa_odd_strided_kernel(Geom g, const uint32_t *__restrict__ link, T *f, Relax<T> 
         const I to = I(i) * I(g.N), own = I(L::opp(i)) * I(g.N) + I(row + xb);
 #pragma unroll
         for (int k = 0; k < NPT; k++) {
-            const int xs = L::ex(i) == 0 ? xb + 32 * k : L::ex(i) == 1 ? xp[k] : xm[k];
-            const I idx = (i > 0 && reflected(w[k], L::opp(i))) ? own + I(32 * k) : to + I(r + xs);
+            const int xs = L::ex(i) == 0 ? xb + XS * k : L::ex(i) == 1 ? xp[k] : xm[k];
+            const I idx = (i > 0 && reflected(w[k], L::opp(i))) ? own + I(XS * k) : to + I(r + xs);
             if (!(w[k] & LINK_SELF_SOLID)) f[idx] = h[k][i];
         }
     }

@@ -28,7 +28,7 @@ template <class L, typename T> struct Steps {
         if (c->aa) {  // in place: even steps are local, odd steps move data; V-node packs on both
             T *f = at<T>(c, c->lay.store[0][0]);
             bool strided = false;  // obstacle-rich geometry: odd steps with per-lane source select, nodes a warp apart
-            if constexpr (V == 2) strided = c->rows > 0 && c->rows_strided && c->g.nx % 64 == 0;
+            if constexpr (V == 2) strided = c->rows > 0 && c->rows_strided;
             const int64_t half_row_threads = (int64_t)(c->g.nx / 2) * c->g.ny;
             const dim3 sgrid((unsigned)((half_row_threads + 63) / 64), 1, c->zselc);
             for (int t = 0; t < n; t++) {
@@ -46,7 +46,7 @@ template <class L, typename T> struct Steps {
         }
         if constexpr (V <= 2 && sizeof(I) == 4) {
             if constexpr (V == 2)
-            if (c->rows > 0 && c->rows_strided && c->g.nx % 64 == 0) {  // ... with the thread's two nodes a warp apart
+            if (c->rows > 0 && c->rows_strided) {  // ... with the thread's two nodes half a row apart
                 const int bx = (c->span_bx > 0 && c->span_bx <= 128) ? c->span_bx : 64;
                 const int64_t spans = (int64_t)(c->g.nx / 2) * ((c->g.ny + c->rows - 1) / c->rows);
                 const dim3 grid((unsigned)((spans + bx - 1) / bx), 1, c->zselc);

@@ -120,9 +120,9 @@ def test_big_c3_default_dispatch_is_the_row_walking_kernel(B, orc, precision):
 
 
 @pytest.mark.parametrize("precision", [W.F32, W.F64])
-def test_big_c3_where_nx_is_not_a_multiple_of_64(B, orc, precision):
-    """nx = 96: the row-walking kernel with adjacent nodes (the strided one needs nx % 64 == 0)."""
-    check_big(B, orc, W.c3_mrt_obstacles(96, 112, 112, precision=precision), dict(nodes_per_thread=2, rows_per_block=2, rows_strided=0))
+def test_big_c3_where_warps_straddle_rows(B, orc, precision):
+    """nx = 90: 45 threads per row, so the warps of the row-walking kernel straddle rows and half rows."""
+    check_big(B, orc, W.c3_mrt_obstacles(90, 112, 112, precision=precision), dict(nodes_per_thread=2, rows_per_block=2, rows_strided=1))
 
 
 def test_big_c4_default_dispatch_fp64_v2(B, orc):

@@ -15,7 +15,7 @@ pytestmark = pytest.mark.gpu
 # the Shan-Chen variant (split per-component collide kernels | one monolithic kernel) rides on the LBM_ROWS axis
 ENVS = [dict(LBM_TUNING="1", LBM_VEC=v, LBM_IDX64=i, LBM_ROWS=r, LBM_NO_GRAPH=g, LBM_NO_RESIDENT=g,
              LBM_SC_SPLIT="1" if r == "0" else "0", LBM_SC_FIELDS_VEC="2" if g == "1" else "1",
-             LBM_ROWS_STRIDED="1" if g == "0" else "0")   # nx = 64: the strided row-walking kernel applies at V = 2
+             LBM_ROWS_STRIDED="1" if g == "0" else "0")
         for v, i, r, g in itertools.product(("1", "2", "4"), ("0", "1"), ("0", "3"), ("0", "1"))]
 
 
